@@ -1,0 +1,221 @@
+"""Seeded synthetic workloads (host, NumPy only).
+
+This module serves BOTH the CUDA path and the CPU oracle and therefore holds none of
+the method's arithmetic (no force law, no Runge-Kutta, no observables): it only turns
+uniform random numbers into initial conditions ``y0[12][N]`` and carries the physical
+parameters of the five BASELINE.json configs.  It imports neither the CUDA binding
+nor anything under ``oracle/``.
+
+State layout (section 2.1): rows 0-2 ion position, 3-5 ion velocity,
+6-8 atom position, 9-11 atom velocity; element (k, i) at offset k*N + i (SoA).
+
+Generator recipe:
+``U = Generator(PCG64(seed)).random((N, 10))``, row i <-> trajectory i, so any
+prefix or slice of a larger run is reproducible (``offset`` uses PCG64.advance).
+Only uniform doubles are drawn; every transform is explicit below.
+
+Unit literals are the ones printed in the paper's Fig. 10 (PAPER.md:295-297, :322,
+:341-342).
+"""
+from __future__ import annotations
+
+import copy
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+# PAPER.md:295-297 (amu -> electron masses), :322 (k_B in Hartree/K), :341 (a.u. of time in s)
+AMU = 1822.88848628276014097
+KB = 3.16681156345647751469e-06
+AU_TIME_S = 2.4188843265864e-17
+
+DRAWS_PER_TRAJECTORY = 10
+
+
+@dataclass
+class Workload:
+    """One BASELINE.json config: physical parameters + sampling recipe."""
+
+    name: str
+    N: int
+    seed: int
+    kind: str  # "thermal" (configs 0, 2-4) or "two_body" (config 1)
+    # aig_params fields (paper's per-axis trap convention, eq. (4)-(6))
+    m_ion: float
+    m_atom: float
+    C4: float
+    C8: float
+    a: tuple
+    q: tuple
+    omega_rf: float
+    t0: float = 0.0
+    r_exit: float = 5050.0
+    r_turn: float = math.inf
+    max_steps: int = 1_000_000
+    # integration controls
+    t_max: float = 2e11
+    rtol: float = 1e-10
+    atol: float = 1e-12
+    # sampling
+    T_ion: float = 0.5e-3
+    T_atom: float = 1e-3
+    R0: float = 5000.0
+    b_max: float = 600.0
+    E_coll: float = 0.0  # two_body only: fixed collision energy (Hartree)
+    notes: dict = field(default_factory=dict)
+
+    def params(self) -> dict:
+        """Fields of ``aig_params`` / the oracle's parameter struct, as plain Python values."""
+        return dict(m_ion=self.m_ion, m_atom=self.m_atom, C4=self.C4, C8=self.C8,
+                    a=tuple(self.a), q=tuple(self.q), omega_rf=self.omega_rf, t0=self.t0,
+                    r_exit=self.r_exit, r_turn=self.r_turn, max_steps=self.max_steps)
+
+    def replace(self, **kw) -> "Workload":
+        w = copy.deepcopy(self)
+        for k, v in kw.items():
+            if not hasattr(w, k):
+                raise AttributeError(k)
+            setattr(w, k, v)
+        return w
+
+
+def trap_axes(a: float, q: float):
+    """BASELINE.json trap (x'' = -(W^2/4)(a - 2q cos Wt) x, same for y,
+    z'' = +(W^2/2)(a - 2q cos Wt) z) in the paper's per-axis convention
+    acc_k = -(a_k + 2 q_k cos Wt) W^2/4 x_k (eq. (4)-(6)):
+    a[] = (a, a, -2a), q[] = (-q, -q, +2q)   (reading S2)."""
+    return (a, a, -2.0 * a), (-q, -q, 2.0 * q)
+
+
+def omega_from_mhz(f_mhz: float) -> float:
+    """2*pi*f in atomic units of 1/time (OmegaRF = 2*pi*f*2.4188843265864e-17)."""
+    return 2.0 * math.pi * f_mhz * 1e6 * AU_TIME_S
+
+
+def potential_CnDe(n: int, m: int, Cn: float, De: float):
+    """'CnDe' front-end of PAPER.md:428: given V = -Cn/r^n + Cm/r^m with well depth De,
+    return (Cm, Re).  From V'(Re) = 0 and V(Re) = -De:
+    Re^(m-n) = m Cm / (n Cn),  De = Cn (1 - n/m) / Re^n."""
+    Re = (Cn * (1.0 - n / m) / De) ** (1.0 / n)
+    Cm = n * Cn * Re ** (m - n) / m
+    return Cm, Re
+
+
+def config(i: int, **overrides) -> Workload:
+    """The five BASELINE.json configs (index 0..4).  Config 4's sweep point is chosen with
+    ``q=...``/``rtol=...`` overrides (atol follows as rtol*1e-2 unless given)."""
+    omega = omega_from_mhz(2.0)
+    if i in (0, 2, 4):
+        a, q = trap_axes(0.0, 0.1)
+        w = Workload(name=f"cfg{i}", N=256, seed=0, kind="thermal",
+                     m_ion=138.0 * AMU, m_atom=87.0 * AMU, C4=159.5, C8=5.23e5,
+                     a=a, q=q, omega_rf=omega)
+        if i == 2:
+            a, q = trap_axes(0.0, 0.2)
+            w = w.replace(name="cfg2", N=65536, seed=2, a=a, q=q, T_atom=0.5e-3, rtol=1e-9)
+        if i == 4:
+            w = w.replace(name="cfg4", N=4194304, seed=4)
+    elif i == 1:
+        m_ion, m_atom = 138.0 * AMU, 87.0 * AMU
+        E = KB * 1e-3
+        C4 = 159.5
+        w = Workload(name="cfg1", N=65536, seed=1, kind="two_body",
+                     m_ion=m_ion, m_atom=m_atom, C4=C4, C8=5.23e5,
+                     a=(0.0, 0.0, 0.0), q=(0.0, 0.0, 0.0), omega_rf=0.0,
+                     T_ion=0.0, T_atom=0.0, E_coll=E,
+                     b_max=1.5 * (2.0 * C4 / E) ** 0.25)  # DESIGN.md reading S13
+    elif i == 3:
+        a, q = trap_axes(0.001, 0.3)
+        w = Workload(name="cfg3", N=1048576, seed=3, kind="thermal",
+                     m_ion=174.0 * AMU, m_atom=7.0 * AMU, C4=82.0, C8=2.7e5,
+                     a=a, q=q, omega_rf=omega, T_ion=0.1e-3, T_atom=0.1e-3,
+                     b_max=400.0, t_max=1e12)
+    else:
+        raise ValueError("config index must be 0..4")
+    if "q_trap" in overrides:  # scalar BASELINE-style q (config 4 sweep)
+        qq = overrides.pop("q_trap")
+        aa = overrides.pop("a_trap", 0.0 if i != 3 else 0.001)
+        a, q = trap_axes(aa, qq)
+        w = w.replace(a=a, q=q)
+    if "rtol" in overrides and "atol" not in overrides and i == 4:
+        overrides["atol"] = overrides["rtol"] * 1e-2
+    return w.replace(**overrides) if overrides else w
+
+
+def uniforms(seed: int, n: int, offset: int = 0) -> np.ndarray:
+    """Rows [offset, offset+n) of the (N, 10) uniform matrix of stream ``seed``."""
+    bg = np.random.PCG64(seed)
+    if offset:
+        bg.advance(offset * DRAWS_PER_TRAJECTORY)  # one 64-bit output per double
+    return np.random.Generator(bg).random((n, DRAWS_PER_TRAJECTORY))
+
+
+def generate_y0(w: Workload, n: int | None = None, offset: int = 0) -> np.ndarray:
+    """Initial conditions ``y0[12][n]`` (float64, C-contiguous) for trajectories
+    offset .. offset+n-1 of workload ``w`` (default: all ``w.N``)."""
+    n = w.N if n is None else int(n)
+    U = uniforms(w.seed, n, offset)
+    y0 = np.zeros((12, n), dtype=np.float64)
+    two_pi = 2.0 * math.pi
+
+    # isotropic approach direction and the two unit vectors spanning the impact plane
+    ct = 1.0 - 2.0 * U[:, 4]
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = two_pi * U[:, 5]
+    cp, sp = np.cos(ph), np.sin(ph)
+    nhat = np.stack([st * cp, st * sp, ct])
+    e1 = np.stack([ct * cp, ct * sp, -st])
+    e2 = np.stack([-sp, cp, np.zeros(n)])
+    b = w.b_max * np.sqrt(U[:, 6])
+    psi = two_pi * U[:, 7]
+    rel = np.sqrt(w.R0 * w.R0 - b * b) * nhat + b * (np.cos(psi) * e1 + np.sin(psi) * e2)
+
+    if w.kind == "thermal":
+        # ion at the trap centre, Maxwell-Boltzmann velocity (Box-Muller on explicit uniforms)
+        s_i = math.sqrt(KB * w.T_ion / w.m_ion)
+        r01 = s_i * np.sqrt(-2.0 * np.log1p(-U[:, 0]))
+        y0[3] = r01 * np.cos(two_pi * U[:, 1])
+        y0[4] = r01 * np.sin(two_pi * U[:, 1])
+        y0[5] = s_i * np.sqrt(-2.0 * np.log1p(-U[:, 2])) * np.cos(two_pi * U[:, 3])
+        # atom on the sphere of radius R0 about the ion, flux-weighted speed pdf ~ v^3 exp(-m v^2/2kT)
+        s_a = math.sqrt(KB * w.T_atom / w.m_atom)
+        v = s_a * np.sqrt(-2.0 * (np.log1p(-U[:, 8]) + np.log1p(-U[:, 9])))
+        y0[6:9] = rel
+        y0[9:12] = -v * nhat
+    elif w.kind == "two_body":
+        # fixed collision energy E = mu v^2 / 2 (v = relative speed), centre-of-mass frame:
+        # total momentum and centre of mass are both zero (reading S16).
+        M = w.m_ion + w.m_atom
+        mu = w.m_ion * w.m_atom / M
+        v = math.sqrt(2.0 * w.E_coll / mu)
+        vrel = -v * nhat  # atom velocity minus ion velocity
+        y0[0:3] = -(w.m_atom / M) * rel
+        y0[3:6] = -(w.m_atom / M) * vrel
+        y0[6:9] = (w.m_ion / M) * rel
+        y0[9:12] = (w.m_ion / M) * vrel
+    else:
+        raise ValueError(w.kind)
+    return np.ascontiguousarray(y0)
+
+
+def impact_parameters(w: Workload, n: int | None = None, offset: int = 0) -> np.ndarray:
+    """The impact parameters b_i the generator used (for the Langevin / quadrature checks)."""
+    n = w.N if n is None else int(n)
+    return w.b_max * np.sqrt(uniforms(w.seed, n, offset)[:, 6])
+
+
+def shard_range(N: int, rank: int, world: int):
+    """Contiguous index range [lo, hi) of trajectories owned by ``rank`` (paper: trajectories
+    'distributed evenly across the ncores cores')."""
+    base, rem = divmod(int(N), int(world))
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def histogram_edges(n_angle: int = 180, n_life: int = 120, life_lo: float = 1e6, life_hi: float = 1e12):
+    """Default bin edges (SURVEY.md 8(d) 'Histogram spec'): angle uniform on [0, pi],
+    lifetime log-uniform on [life_lo, life_hi] atomic units of time."""
+    angle_edges = np.linspace(0.0, math.pi, n_angle + 1)
+    life_edges = np.logspace(math.log10(life_lo), math.log10(life_hi), n_life + 1)
+    return np.ascontiguousarray(angle_edges), np.ascontiguousarray(life_edges)

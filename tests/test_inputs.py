@@ -1,0 +1,78 @@
+"""Seeded input generator: structure of the synthetic workloads (no GPU)."""
+import math
+
+import numpy as np
+
+from paper_2509_12381_b200 import inputs
+
+
+def test_configs_match_baseline_json():
+    Ns = [256, 65536, 65536, 1048576, 4194304]
+    for i in range(5):
+        w = inputs.config(i)
+        assert w.N == Ns[i] and w.seed == i
+    w0 = inputs.config(0)
+    assert w0.m_ion == 138 * inputs.AMU and w0.m_atom == 87 * inputs.AMU
+    assert (w0.C4, w0.C8, w0.t_max, w0.rtol, w0.atol) == (159.5, 5.23e5, 2e11, 1e-10, 1e-12)
+    assert w0.r_exit == 1.01 * w0.R0
+    # BASELINE trap -> paper's per-axis convention; Laplace: sum a = sum q = 0
+    assert w0.a == (0.0, 0.0, -0.0) and w0.q == (-0.1, -0.1, 0.2)
+    w3 = inputs.config(3)
+    assert abs(sum(w3.a)) < 1e-18 and abs(sum(w3.q)) < 1e-18 and w3.q[2] == 0.6 and w3.a[2] == -0.002
+    assert abs(w0.omega_rf - 2 * math.pi * 2e6 * 2.4188843265864e-17) < 1e-25
+    w1 = inputs.config(1)
+    assert w1.omega_rf == 0 and abs(w1.b_max - 845.05) < 0.01
+    w4 = inputs.config(4, q_trap=0.4, rtol=1e-12)
+    assert w4.q == (-0.4, -0.4, 0.8) and w4.atol == 1e-14 and w4.N == 4194304
+    assert inputs.config(2).rtol == 1e-9 and inputs.config(2).T_atom == 0.5e-3
+
+
+def test_thermal_generator_geometry_and_statistics():
+    w = inputs.config(0)
+    n = 20000
+    y0 = inputs.generate_y0(w, n=n)
+    assert y0.shape == (12, n) and y0.flags.c_contiguous and y0.dtype == np.float64
+    assert np.all(y0[0:3] == 0)
+    rel = y0[6:9]
+    assert np.allclose(np.linalg.norm(rel, axis=0), w.R0, rtol=1e-14)
+    v = y0[9:12]
+    speed = np.linalg.norm(v, axis=0)
+    nhat = -v / speed
+    # impact parameter = |rel - (rel.n) n| and equals the generator's b; uniform in area
+    b = np.linalg.norm(rel - (rel * nhat).sum(0) * nhat, axis=0)
+    assert np.allclose(b, inputs.impact_parameters(w, n=n), rtol=1e-9, atol=1e-9)
+    assert abs((b**2).mean() / (w.b_max**2 / 2) - 1) < 0.02 and b.max() <= w.b_max
+    # isotropic directions
+    assert np.all(np.abs(nhat.mean(axis=1)) < 0.02) and abs((nhat[2] ** 2).mean() - 1 / 3) < 0.01
+    # flux-weighted speed: <v^2> = 4 kT/m ; ion Maxwell-Boltzmann: <v_k^2> = kT/m
+    assert abs((speed**2).mean() / (4 * inputs.KB * w.T_atom / w.m_atom) - 1) < 0.03
+    for k in range(3):
+        assert abs((y0[3 + k] ** 2).mean() / (inputs.KB * w.T_ion / w.m_ion) - 1) < 0.04
+    # atom moves toward the ion: radial velocity negative
+    assert np.all((rel * v).sum(0) < 0)
+
+
+def test_two_body_generator_cm_frame():
+    w = inputs.config(1)
+    y0 = inputs.generate_y0(w, n=1000)
+    P = w.m_ion * y0[3:6] + w.m_atom * y0[9:12]
+    R = w.m_ion * y0[0:3] + w.m_atom * y0[6:9]
+    mu = w.m_ion * w.m_atom / (w.m_ion + w.m_atom)
+    vrel = y0[9:12] - y0[3:6]
+    assert np.max(np.abs(P)) < 1e-12 * mu * 2.6e-7 * 100 and np.max(np.abs(R)) < 1e-9 * w.m_ion
+    assert np.allclose(0.5 * mu * (vrel**2).sum(0), inputs.KB * 1e-3, rtol=1e-13)
+    assert np.allclose(np.linalg.norm(y0[6:9] - y0[0:3], axis=0), w.R0, rtol=1e-14)
+    assert abs(math.sqrt(2 * w.E_coll / mu) - 2.5518e-7) < 1e-10
+
+
+def test_prefix_and_offset_reproducibility_and_sharding():
+    w = inputs.config(4)
+    full = inputs.generate_y0(w, n=300)
+    assert np.array_equal(inputs.generate_y0(w, n=100), full[:, :100])
+    assert np.array_equal(inputs.generate_y0(w, n=120, offset=57), full[:, 57:177])
+    for N, world in ((10, 3), (4194304, 8), (7, 8)):
+        spans = [inputs.shard_range(N, r, world) for r in range(world)]
+        assert spans[0][0] == 0 and spans[-1][1] == N
+        assert all(spans[i][1] == spans[i + 1][0] for i in range(world - 1))
+        sizes = [hi - lo for lo, hi in spans]
+        assert max(sizes) - min(sizes) <= 1
