@@ -1,0 +1,160 @@
+/*
+ * aig.h -- C ABI of libaig: B200-native (sm_100a) atom-ion trajectory integrator.
+ *
+ * Hot path of arxiv/paper_2509_12381 ("GPU-Accelerated MATLAB Software for Atom-Ion
+ * Dynamics"): integrate N independent 12-component atom-ion trajectories (PAPER.md:69,
+ * eq. (3)-(10) at :71-90) with the adaptive Dormand-Prince 5(4) Runge-Kutta scheme behind
+ * MATLAB's ode45, keeping only the final state and a few scalar
+ * observables computed on the fly, then bin the observables on the
+ * device ("their distributions").
+ *
+ * Conventions
+ *   - plain C, no torch / C++ types; every pointer is marked HOST or DEVICE;
+ *   - all quantities in atomic units, FP64; counters int32; flags uint8;
+ *   - state layout: row k (0-based) of y0 / y_final is the paper's y_{k+1}:
+ *     rows 0-2 ion position, 3-5 ion velocity, 6-8 atom position, 9-11 atom velocity;
+ *     SoA: element (k, i) at offset k*N + i;
+ *   - the caller owns every buffer; nothing allocated by the library outlives a call
+ *     (aig_run_host frees what it allocates before returning);
+ *   - work is enqueued on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
+ *     stream); no host synchronisation inside unless stated; outputs are valid once the
+ *     stream has synchronised;
+ *   - return value: 0 = AIG_OK, negative = error (see aig_strerror).  Numerical failure of one
+ *     trajectory is NOT an error return: it is reported in status[i].
+ *   - there is no CPU fallback: without a CUDA device every compute call returns
+ *     AIG_ERR_CUDA.
+ */
+#ifndef AIG_H_
+#define AIG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AIG_VERSION 100 /* 0.1.0 */
+
+/* error codes */
+#define AIG_OK 0
+#define AIG_ERR_NULL (-1)      /* required pointer is NULL */
+#define AIG_ERR_SIZE (-2)      /* N < 0, N too large, bad bin count */
+#define AIG_ERR_TOL (-3)       /* rtol <= 0, atol < 0, non-finite tolerances */
+#define AIG_ERR_TIME (-4)      /* t_max <= t0 or non-finite */
+#define AIG_ERR_PARAM (-5)     /* masses <= 0, max_steps < 1, non-finite parameter */
+#define AIG_ERR_ALIGN (-6)     /* device pointer not aligned to its element size */
+#define AIG_ERR_CUDA (-7)      /* CUDA runtime error (no device, launch failure, out of memory) */
+
+/* status[i] of one trajectory */
+#define AIG_STATUS_EXIT 0      /* r > r_exit after the first radial minimum */
+#define AIG_STATUS_TMAX 1      /* reached t_max */
+#define AIG_STATUS_MAXSTEPS 2  /* max_steps accepted steps */
+#define AIG_STATUS_FAILED 3    /* step size underflow / non-finite error estimate */
+
+/* Physical and stop parameters shared by all trajectories of a call (HOST struct).
+ * The paper replicates every constant N times as a gpuArray; here they are
+ * kernel arguments (constant bank). */
+typedef struct aig_params {
+    double m_ion, m_atom; /* masses */
+    double C4, C8;        /* V(r) = C8/r^8 - C4/r^4 */
+    double a[3], q[3];    /* the PAPER'S per-axis trap convention, eq. (4)-(6):
+                             acc_k = -(a_k + 2 q_k cos(Omega t)) * Omega^2/4 * x_k  (ion only) */
+    double omega_rf;      /* Omega_rf; with a = q = 0 the trap is off */
+    double t0;            /* start time = RF phase origin */
+    double r_exit;        /* stop when r > r_exit after the first radial minimum; <= 0 disables */
+    double r_turn;        /* a radial minimum counts as a turning point only if r < r_turn;
+                             +inf counts all of them */
+    int64_t max_steps;    /* accepted-step cap, paper default 1,000,000 */
+} aig_params;
+
+/* Per-trajectory outputs: caller-allocated DEVICE buffers, each of length N
+ * (y_final: 12*N, SoA like y0).  Any pointer except y_final/status may NOT be NULL. */
+typedef struct aig_out {
+    double *y_final;       /* state at the last accepted step end (PAPER.md:192 yend1..12) */
+    double *t_final;       /* time of that step end (tend) */
+    double *lifetime;      /* t(last turning point) - t(first), 0 if fewer than two */
+    double *angle;         /* angle in [0, pi] between initial and final atom velocity */
+    double *r_min;         /* smallest atom-ion distance seen at t0 and accepted step ends */
+    int32_t *n_acc;        /* accepted steps ("nsteps") */
+    int32_t *n_rej;        /* failed attempts */
+    int32_t *n_turn;       /* counted inner turning points ("bounces") */
+    int32_t *status;       /* AIG_STATUS_* */
+    uint8_t *complex_flag; /* 1 if n_turn >= 2 (one bounce = simple) */
+} aig_out;
+
+/* Bin edges of the observable histograms: DEVICE pointers to strictly increasing doubles
+ * (n_bins + 1 of them).  Bin j holds edges[j] <= v < edges[j+1]. */
+typedef struct aig_hist_spec {
+    const double *angle_edges;
+    int32_t n_angle_bins;
+    const double *life_edges;
+    int32_t n_life_bins;
+    int32_t n_turn_bins; /* n_turn is clamped to n_turn_bins - 1 */
+} aig_hist_spec;
+
+/* Histogram outputs: DEVICE uint64 arrays, ACCUMULATED into (the caller zeroes them):
+ *   angle    [n_angle_bins + 2]: [0] underflow, [1 + j] bin j, [n + 1] overflow and NaN
+ *   lifetime [n_life_bins + 2] : same layout, over trajectories with complex_flag = 1 only
+ *   n_turn   [n_turn_bins], status [4]
+ *   totals   [4]: sum n_acc, sum n_rej, number of complexes, number of trajectories */
+typedef struct aig_hist {
+    uint64_t *angle, *lifetime, *n_turn, *status, *totals;
+} aig_hist;
+
+/* Bytes of DEVICE scratch aig_integrate needs for N trajectories (work-queue counter). */
+size_t aig_workspace_bytes(int64_t N);
+
+/* Integrate N trajectories from t0 to the first stop (exit radius, t_max, max_steps).
+ *   p         HOST   parameters (copied into the launch)
+ *   y0        DEVICE [12][N] initial conditions, never written
+ *   t_max     end of the time span (> p->t0);  rtol > 0, atol >= 0: ode45 tolerances
+ *   out       HOST struct of DEVICE pointers
+ *   workspace DEVICE scratch of >= aig_workspace_bytes(N) bytes, 8-byte aligned
+ * One persistent kernel: each thread integrates one trajectory at a time and refills from
+ * a global work queue when it finishes (PAPER.md:186-202 runs one array element per thread). */
+int aig_integrate(const aig_params *p, const double *y0, int64_t N, double t_max, double rtol,
+                  double atol, const aig_out *out, void *workspace, void *cuda_stream);
+
+/* Reduce the observables of N trajectories into histograms and totals (PAPER.md:23, :457,
+ * :517; the paper does this on the host after gather()).  obs: HOST struct of DEVICE
+ * pointers as written by aig_integrate (uses angle, lifetime, n_acc, n_rej, n_turn, status,
+ * complex_flag); spec: HOST struct of DEVICE edge pointers; out: HOST struct of DEVICE
+ * pointers. */
+int aig_histogram(const aig_out *obs, int64_t N, const aig_hist_spec *spec, const aig_hist *out,
+                  void *cuda_stream);
+
+/* Test hook: ONE attempted DP5(4) step of size h[i] from (t[i], y[:, i]) for each of N
+ * states.  DEVICE: y [12][N], t [N], h [N], ynew [12][N] (5th-order solution), err [N]
+ * (ode45's scaled error estimate; the step would be accepted iff err <= rtol). */
+int aig_step_once(const aig_params *p, const double *y, const double *t, const double *h,
+                  int64_t N, double rtol, double atol, double *ynew, double *err,
+                  void *cuda_stream);
+
+/* End-to-end convenience entry with HOST buffers: allocates device memory, copies y0 to the
+ * device, runs aig_integrate (+ aig_histogram when hist_spec/hist_out are non-NULL, with
+ * HOST edge pointers and HOST uint64 outputs, zeroed by the call), copies every non-NULL
+ * member of `out` (HOST pointers here) back, frees the device memory and synchronises.
+ * Blocking. */
+int aig_run_host(const aig_params *p, const double *y0_host, int64_t N, double t_max, double rtol,
+                 double atol, const aig_out *out_host, const aig_hist_spec *hist_spec_host,
+                 const aig_hist *hist_out_host);
+
+/* Measurement aid: run a register-resident FP64 FMA chain kernel on every SM and return the
+ * achieved non-tensor FP64 rate in FLOP/s through *flops_per_s (blocking; used by bench.py as
+ * the measured ALU roofline denominator). ilp in [1, 16] independent chains per thread. */
+int aig_fp64_peak_probe(int iters, int ilp, double *flops_per_s, double *elapsed_ms);
+
+/* Launch geometry the integrator would use on the current device (for reporting):
+ * writes SM count, resident blocks per SM, threads per block, registers per thread and
+ * local-memory (spill) bytes per thread of the RF-trap integrator kernel. */
+int aig_kernel_info(int *sm_count, int *blocks_per_sm, int *threads_per_block,
+                    int *regs_per_thread, int *local_bytes_per_thread);
+
+const char *aig_strerror(int code);
+int aig_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AIG_H_ */

@@ -1,0 +1,337 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json's north_star, written out here:
+  * one attempted step: ynew within 1e-14, relative to the magnitude of the position /
+    velocity 3-vector the component belongs to;
+  * direct (non-complex) trajectories at rtol = 1e-10: accepted step counts within +-2,
+    final states within 1e-6 (same metric) where the step counts agree;
+  * ensemble: complex fraction within 3 binomial sigma, two-sample KS p > 0.01 on the
+    scattering angle and lifetime; chaotic complex trajectories are not compared pointwise.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy import stats
+
+from oracle import aig_oracle as orc
+from paper_2509_12381_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+BLOCKS = (slice(0, 3), slice(3, 6), slice(6, 9), slice(9, 12))
+
+
+@pytest.fixture(scope="module")
+def aig():
+    import torch
+    from paper_2509_12381_b200 import binding
+    binding.lib()  # fail loudly if libaig.so is missing
+    assert torch.cuda.is_available()
+    return binding
+
+
+def _dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def _host(out):
+    import torch
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in out.items() if not k.startswith("_")}
+
+
+def block_rel(a, b, ref_extra=None):
+    """max over components of |a-b| / (inf-norm of the 3-vector block), per trajectory."""
+    worst = np.zeros(a.shape[1])
+    for blk in BLOCKS:
+        scale = np.max(np.abs(b[blk]), axis=0)
+        if ref_extra is not None:
+            scale = np.maximum(scale, np.max(np.abs(ref_extra[blk]), axis=0))
+        scale = np.where(scale > 0, scale, 1.0)
+        worst = np.maximum(worst, np.max(np.abs(a[blk] - b[blk]), axis=0) / scale)
+    return worst
+
+
+def step_tolerance(y):
+    """north_star's 1e-14, plus the conditioning of eq. (4)-(10) in the lab frame: the force
+    ~ r^-9 sees d = x_ion - x_atom, so a 1-ulp change of a position of size |x| changes it by
+    ~10 eps |x| / r relatively.  Only states deep in the well
+    (r ~ 7.6 a0 at |x| ~ 1e3 a0) ever need the second term."""
+    r = np.linalg.norm(y[6:9] - y[0:3], axis=0)
+    xmax = np.max(np.abs(np.vstack([y[0:3], y[6:9]])), axis=0)
+    return 1e-14 + 10 * np.finfo(float).eps * xmax / r
+
+
+def run_gpu(aig, w, y0):
+    p = aig.make_params(**w.params())
+    return _host(aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol))
+
+
+def run_orc(w, y0, threads=8):
+    p = orc.make_params(**w.params())
+    return orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=threads)
+
+
+# ---------------------------------------------------------------------------------------------
+# single step
+# ---------------------------------------------------------------------------------------------
+
+def _mid_flight_states(w, n, seed):
+    """States spread along real trajectories: far field, approach, and deep in the well."""
+    rng = np.random.default_rng(seed)
+    y0 = inputs.generate_y0(w, n=n)
+    p = orc.make_params(**w.params())
+    ys, ts, hs = [], [], []
+    for i in range(n):
+        tt, yy, _ = orc.integrate_trace(p, y0[:, i], w.t_max, w.rtol, w.atol, cap=4000)
+        if len(tt) < 3:
+            continue
+        for j in rng.choice(len(tt) - 1, size=min(6, len(tt) - 1), replace=False):
+            ys.append(yy[j])
+            ts.append(tt[j])
+            hs.append((tt[j + 1] - tt[j]) * rng.uniform(0.3, 1.5))
+        k = int(np.argmin(np.linalg.norm(yy[:, 6:9] - yy[:, 0:3], axis=1)))
+        if 0 < k < len(tt) - 1:
+            ys.append(yy[k])
+            ts.append(tt[k])
+            hs.append(tt[k + 1] - tt[k])
+    return np.ascontiguousarray(np.array(ys).T), np.array(ts), np.array(hs)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 3])
+def test_step_once_parity(aig, cfg):
+    w = inputs.config(cfg)
+    y, t, h = _mid_flight_states(w, 96, seed=cfg)
+    assert y.shape[1] > 300        # several blocks of 128 threads and a ragged tail
+    yo, eo = orc.step_once(orc.make_params(**w.params()), y, t, h, w.rtol, w.atol)
+    yg, eg = aig.aig_step_once(aig.make_params(**w.params()), _dev(y), _dev(t), _dev(h), w.rtol, w.atol)
+    yg, eg = yg.cpu().numpy(), eg.cpu().numpy()
+    rel = block_rel(yg, yo, ref_extra=y)
+    assert np.all(rel <= step_tolerance(y)), (rel / step_tolerance(y)).max()
+    assert np.mean(rel <= 1e-14) > 0.9
+    # the estimate is a cancelling sum (rounding-order sensitive): compare loosely, and only
+    # where it is not itself at rounding level
+    big = eo > 1e-3 * w.rtol
+    assert np.all(np.abs(eg[big] - eo[big]) <= 1e-3 * eo[big])
+    assert np.all(eg[~big] <= 2e-3 * w.rtol)
+
+
+def test_step_once_static_trap_and_edge_sizes(aig):
+    # harmonic-trap mode (q = 0) exercises the TRAP_STATIC kernel; N = 1 and N = 0
+    om2 = (4e-18, 9e-18, 2.5e-17)
+    kw = dict(m_ion=138 * inputs.AMU, m_atom=87 * inputs.AMU, C4=159.5, C8=5.23e5, a=om2, q=(0, 0, 0),
+              omega_rf=2.0)
+    y = np.array([[100.0, -50, 20, 1e-7, 2e-7, -3e-7, 130, -40, 60, -2e-6, 1e-6, 3e-6]]).T.copy()
+    t, h = np.array([1e9]), np.array([2e4])
+    yo, eo = orc.step_once(orc.make_params(**kw), y, t, h, 1e-10, 1e-12)
+    yg, eg = aig.aig_step_once(aig.make_params(**kw), _dev(y), _dev(t), _dev(h), 1e-10, 1e-12)
+    assert block_rel(yg.cpu().numpy(), yo, ref_extra=y).max() <= 1e-14
+    assert abs(eg.cpu().numpy()[0] - eo[0]) <= 1e-3 * eo[0] + 1e-16
+    import torch
+    e = torch.empty((12, 0), dtype=torch.float64, device="cuda")
+    z = torch.empty(0, dtype=torch.float64, device="cuda")
+    yg, eg = aig.aig_step_once(aig.make_params(**kw), e, z, z, 1e-10, 1e-12)
+    assert yg.shape == (12, 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# whole trajectories
+# ---------------------------------------------------------------------------------------------
+
+def _compare_direct(w, g, o, frac_equal=0.97, tol=1e-6):
+    direct = (o["n_turn"] <= 1) & (g["n_turn"] <= 1) & (o["status"] == 0)
+    assert direct.mean() > 0.5
+    dn = np.abs(g["n_acc"][direct].astype(int) - o["n_acc"][direct].astype(int))
+    assert dn.max() <= 2, dn.max()
+    same = direct & (g["n_acc"] == o["n_acc"]) & (g["status"] == o["status"])
+    assert same.sum() >= frac_equal * direct.sum()
+    rel = block_rel(g["y_final"][:, same], o["y_final"][:, same])
+    assert rel.max() <= tol, rel.max()
+    assert np.max(np.abs(g["t_final"][same] / o["t_final"][same] - 1)) <= 1e-9
+    assert np.max(np.abs(g["angle"][same] - o["angle"][same])) <= 1e-6
+    assert np.max(np.abs(g["r_min"][same] / o["r_min"][same] - 1)) <= 1e-6
+    assert np.array_equal(g["n_turn"][same], o["n_turn"][same])
+    return same
+
+
+def test_config0_trajectories(aig):
+    w = inputs.config(0)
+    y0 = inputs.generate_y0(w)
+    g, o = run_gpu(aig, w, y0), run_orc(w, y0)
+    _compare_direct(w, g, o)
+    # invariants of the outputs
+    assert np.array_equal(g["complex_flag"], (g["n_turn"] >= 2).astype(np.uint8))
+    assert np.all(g["lifetime"][g["n_turn"] < 2] == 0)
+    assert np.all((g["status"] == 0) | (g["status"] == 1))
+    assert abs(int(g["complex_flag"].sum()) - int(o["complex_flag"].sum())) <= 3
+
+
+def test_config1_two_body_physics(aig):
+    """Trap off, N = 65,536: parity on a prefix + physics at full size."""
+    w = inputs.config(1)
+    y0 = inputs.generate_y0(w)
+    g = run_gpu(aig, w, y0)
+    n_o = 4096
+    o = run_orc(w, y0[:, :n_o].copy())
+    gp = {k: (v[..., :n_o]) for k, v in g.items()}
+    b = inputs.impact_parameters(w)
+    bc = (4 * w.C4 / w.E_coll) ** 0.25
+    # direct comparison away from the orbiting window (there the energy error decides the fate)
+    clear = np.abs(b[:n_o] / bc - 1) > 1e-2
+    dn = np.abs(gp["n_acc"][clear].astype(int) - o["n_acc"][clear].astype(int))
+    assert dn.max() <= 2
+    miss = clear & (b[:n_o] > bc) & (gp["n_acc"] == o["n_acc"])
+    assert block_rel(gp["y_final"][:, miss], o["y_final"][:, miss]).max() <= 1e-6
+    # Langevin capture at full size
+    clear_all = np.abs(b / bc - 1) > 1e-3
+    captured = g["r_min"] < bc / 2
+    assert np.array_equal(captured[clear_all], (b < bc)[clear_all])
+    pexp = math.sqrt(2) / 2.25
+    assert abs(captured.mean() - pexp) < 3 * math.sqrt(pexp * (1 - pexp) / w.N)
+    # conservation laws from the final states (CM frame: P = 0, R_cm = 0, E and |L| fixed)
+    mi, ma = w.m_ion, w.m_atom
+    mu = mi * ma / (mi + ma)
+    v = math.sqrt(2 * w.E_coll / mu)
+    yf = g["y_final"]
+    r = np.linalg.norm(yf[6:9] - yf[0:3], axis=0)
+    E = 0.5 * mi * (yf[3:6] ** 2).sum(0) + 0.5 * ma * (yf[9:12] ** 2).sum(0) - w.C4 / r**4 + w.C8 / r**8
+    E0 = w.E_coll - w.C4 / w.R0**4 + w.C8 / w.R0**8
+    De = w.C4**2 / (4 * w.C8)
+    ok = clear_all & (g["status"] == 0)
+    assert ok.mean() > 0.99
+    assert np.max(np.abs(E[ok] - E0)) < 1e-8 * De
+    assert np.max(np.abs(E[ok & ~captured] - E0)) < 1e-8 * w.E_coll
+    L = mi * np.cross(yf[0:3].T, yf[3:6].T) + ma * np.cross(yf[6:9].T, yf[9:12].T)
+    assert np.max(np.abs(np.linalg.norm(L, axis=1)[ok] - mu * v * b[ok])) < 1e-8 * mu * v * w.b_max
+    P = mi * yf[3:6] + ma * yf[9:12]
+    assert np.max(np.abs(P[:, ok])) < 1e-8 * mu * v
+    # one turning point each, no complexes in a two-body problem
+    assert np.all(g["n_turn"][ok] == 1) and g["complex_flag"][ok].sum() == 0
+
+
+def _ensemble_checks(g, o, n_g, n_o):
+    pg, po = g["complex_flag"].mean(), o["complex_flag"].mean()
+    pool = (g["complex_flag"].sum() + o["complex_flag"].sum()) / (n_g + n_o)
+    sigma = math.sqrt(max(pool * (1 - pool), 1e-12) * (1 / n_g + 1 / n_o))
+    assert abs(pg - po) <= 3 * sigma, (pg, po, sigma)
+    assert stats.ks_2samp(g["angle"], o["angle"]).pvalue > 0.01
+    lg, lo = g["lifetime"][g["complex_flag"] == 1], o["lifetime"][o["complex_flag"] == 1]
+    if len(lg) > 20 and len(lo) > 20:
+        assert stats.ks_2samp(lg, lo).pvalue > 0.01
+    assert stats.ks_2samp(g["n_acc"], o["n_acc"]).pvalue > 0.01
+
+
+def test_config2_ensemble_statistics(aig):
+    w = inputs.config(2)
+    y0 = inputs.generate_y0(w)
+    g = run_gpu(aig, w, y0)
+    n_o = 16384
+    o = run_orc(w, y0[:, :n_o].copy())
+    gp = {k: v[..., :n_o] for k, v in g.items()}
+    _compare_direct(w, gp, o, tol=1e-5)      # rtol = 1e-9 here (config 2)
+    _ensemble_checks(gp, o, n_o, n_o)        # same trajectories: must agree far inside 3 sigma
+    rest = {k: v[..., n_o:] for k, v in g.items()}
+    _ensemble_checks(rest, o, w.N - n_o, n_o)  # disjoint samples of the same distribution
+
+
+def test_config3_prefix_heavy_light(aig):
+    """Config 3 system (long-lived complexes, step-count imbalance) on a prefix of its inputs."""
+    w = inputs.config(3)
+    n = 6144
+    y0 = inputs.generate_y0(w, n=n)
+    g, o = run_gpu(aig, w, y0), run_orc(w, y0)
+    _compare_direct(w, g, o, frac_equal=0.9, tol=1e-5)
+    _ensemble_checks(g, o, n, n)
+    assert g["n_acc"].max() > 20 * np.median(g["n_acc"])   # the imbalance the refill queue is for
+
+
+def test_degenerate_inputs(aig):
+    import torch
+    w = inputs.config(0)
+    p = aig.make_params(**w.params())
+    # N = 0: nothing launched, no error
+    out = aig.aig_integrate(p, torch.empty((12, 0), dtype=torch.float64, device="cuda"), w.t_max, w.rtol, w.atol)
+    assert out["t_final"].numel() == 0
+    # N = 1, and a trajectory whose atom sits ON the ion (r = 0): non-finite force -> status 3
+    y0 = inputs.generate_y0(w, n=3)
+    y0[6:9, 1] = y0[0:3, 1]
+    g, o = run_gpu(aig, w, y0), run_orc(w, y0, threads=1)
+    assert g["status"][1] == 3 and o["status"][1] == 3
+    assert g["n_acc"][1] == 0 and g["n_rej"][1] == o["n_rej"][1]
+    assert np.array_equal(g["y_final"][:, 1], y0[:, 1])
+    for i in (0, 2):
+        assert abs(int(g["n_acc"][i]) - int(o["n_acc"][i])) <= 2
+    # max_steps stop and t_max stop (no exit radius)
+    w2 = w.replace(max_steps=25)
+    g2, o2 = run_gpu(aig, w2, y0[:, :1].copy()), run_orc(w2, y0[:, :1].copy(), threads=1)
+    assert g2["status"][0] == 2 and o2["status"][0] == 2 and g2["n_acc"][0] == 25
+    assert abs(g2["t_final"][0] / o2["t_final"][0] - 1) < 1e-9
+    w3 = w.replace(r_exit=0.0, t_max=3e10)
+    g3, o3 = run_gpu(aig, w3, y0[:, :1].copy()), run_orc(w3, y0[:, :1].copy(), threads=1)
+    assert g3["status"][0] == 1 and g3["t_final"][0] == 3e10 and o3["status"][0] == 1
+    assert block_rel(g3["y_final"], o3["y_final"]).max() < 1e-6
+
+
+def test_argument_errors(aig):
+    import torch
+    w = inputs.config(0)
+    y0 = _dev(inputs.generate_y0(w, n=4))
+    with pytest.raises(aig.AigError):
+        aig.aig_integrate(aig.make_params(**w.params()), y0, w.t_max, 0.0, w.atol)       # rtol <= 0
+    with pytest.raises(aig.AigError):
+        aig.aig_integrate(aig.make_params(**w.params()), y0, -1.0, w.rtol, w.atol)       # t_max <= t0
+    with pytest.raises(aig.AigError):
+        aig.aig_integrate(aig.make_params(**{**w.params(), "m_ion": 0.0}), y0, w.t_max, w.rtol, w.atol)
+    torch.cuda.synchronize()
+
+
+# ---------------------------------------------------------------------------------------------
+# histogram: integer-exact against the definition
+# ---------------------------------------------------------------------------------------------
+
+def test_histogram_exact(aig):
+    import torch
+    w = inputs.config(0)
+    n = 5000  # several blocks + ragged tail
+    y0 = inputs.generate_y0(w.replace(seed=11), n=n)
+    p = aig.make_params(**w.params())
+    out = aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol)
+    ae, le = inputs.histogram_edges()
+    hist = aig.aig_histogram(out, _dev(ae), _dev(le), 64)
+    H = aig.hist_to_numpy(hist)
+    ref = orc.histogram(_host(out), ae, le, 64)
+    for k in ("angle", "lifetime", "n_turn", "status", "totals"):
+        assert np.array_equal(H[k], ref[k]), k
+    # accumulation semantics: a second call doubles every count
+    aig.aig_histogram(out, _dev(ae), _dev(le), 64, hist=hist)
+    H2 = aig.hist_to_numpy(hist)
+    assert all(np.array_equal(H2[k], 2 * ref[k]) for k in ref)
+    # synthetic observables hitting edges, under/overflow and NaN
+    rng = np.random.default_rng(0)
+    m = 3001
+    obs = dict(angle=rng.uniform(-0.2, 3.4, m), lifetime=10 ** rng.uniform(5, 13, m),
+               n_turn=rng.integers(0, 200, m).astype(np.int32), status=rng.integers(0, 4, m).astype(np.int32),
+               n_acc=rng.integers(0, 2**20, m).astype(np.int32), n_rej=rng.integers(0, 50, m).astype(np.int32))
+    obs["angle"][:5] = [ae[0], ae[-1], ae[7], np.nan, np.nextafter(ae[7], 0)]
+    obs["complex_flag"] = (obs["n_turn"] >= 2).astype(np.uint8)
+    dev = {k: _dev(v) for k, v in obs.items()}
+    for k in ("y_final", "t_final", "r_min"):
+        dev[k] = torch.zeros(1, device="cuda", dtype=torch.float64)
+    H3 = aig.hist_to_numpy(aig.aig_histogram(dev, _dev(ae), _dev(le), 64))
+    ref3 = orc.histogram(obs, ae, le, 64)
+    assert all(np.array_equal(H3[k], ref3[k]) for k in ref3)
+
+
+def test_run_host_end_to_end(aig):
+    w = inputs.config(0)
+    y0 = inputs.generate_y0(w)
+    ae, le = inputs.histogram_edges()
+    p = aig.make_params(**w.params())
+    res = aig.aig_run_host(p, y0, w.t_max, w.rtol, w.atol, ae, le)
+    dev = run_gpu(aig, w, y0)
+    for k in ("y_final", "t_final", "angle", "lifetime", "n_acc", "n_rej", "n_turn", "status", "complex_flag"):
+        assert np.array_equal(res[k], dev[k]), k       # same kernels, same inputs: bit-identical
+    ref = orc.histogram(dev, ae, le, 64)
+    assert all(np.array_equal(res["hist"][k], ref[k]) for k in ref)
