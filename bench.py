@@ -1,0 +1,375 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the atom-ion DP5(4) hot path on B200 (BASELINE.json metric).
+
+    python bench.py --gpus N --steps K --warmup W            # our arm (libaig, CUDA)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle as it stands
+
+One "step" = one pass of the whole hot path (a1-a10) over one batch of
+synthetic input: aig_integrate (load, DP5(4) loop, observables, store) + aig_histogram, on
+BASELINE.json configs[4] at its central sweep point (N = 4,194,304 trajectories per GPU, config-0
+system, q = 0.1, rtol = 1e-10, atol = rtol*1e-2, seed 4).  The other eight points of that
+config's 3x3 sweep are run once each after the timed region and reported under "sweep".
+
+Prints ONE JSON line (rank 0).  `value` = trajectories/s over all ranks with inputs resident in
+HBM; `e2e` = the same through aig_run_host (pinned HOST buffers in, HOST buffers out, device
+allocation + H2D + kernels + D2H inside the timed region); `roofline` = algorithmic FP64
+flops of the integrator kernel / its CUDA-event duration against the FP64 non-tensor peak;
+`cpu_baseline` = the oracle timed on this box's host cores on a bounded prefix sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2509_12381_b200 import inputs  # noqa: E402  (NumPy only)
+
+# SURVEY.md 8(d) / DESIGN.md "Flop accounting": nominal flops of one attempted DP5(4) step of the
+# 12-component system as the paper states it (6 f-evals x 38 + 240 stage FMAs + error + controller).
+FLOPS_PER_ATTEMPT = 900.0
+# 148 SMs x 4 sub-partitions x 16 FP64 FMA lanes x 2 flop x 1.965 GHz (max SM clock)
+FP64_PEAK_NOMINAL = 148 * 4 * 16 * 2 * 1.965e9
+# dram__bytes_read.sum + dram__bytes_write.sum of one integrate_kernel launch at the bench
+# workload, from the ncu --set full capture summarised in profiles/ (None until captured).
+INTEGRATE_DRAM_TRAFFIC_BYTES = None
+
+WORKLOAD_NAME = "configs[4] N=4194304 q=0.1 rtol=1e-10 atol=1e-12 seed=4"
+SWEEP_Q = (0.1, 0.2, 0.4)
+SWEEP_RTOL = (1e-8, 1e-10, 1e-12)
+
+
+def _workload(n, q=0.1, rtol=1e-10):
+    w = inputs.config(4, q_trap=q, rtol=rtol)
+    return w.replace(N=int(n))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        for row in self.rows:
+            parts = [x.strip() for x in row.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax.append(float(parts[1]))
+                power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(self.NAMES, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(smax)) if smax else None,
+                "power_w_max": float(max(power)) if power else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _oracle_sample(w, n_sample: int, threads: int):
+    """Time the oracle, as it stands, on the first n_sample trajectories of workload w."""
+    from oracle import aig_oracle as orc
+    y0 = inputs.generate_y0(w, n=n_sample)
+    p = orc.make_params(**w.params())
+    t0 = time.perf_counter()
+    o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=threads)
+    dt = time.perf_counter() - t0
+    return dt, int(o["n_acc"].sum()), int(o["n_rej"].sum())
+
+
+def run_reference(args) -> int:
+    """--impl reference: there is no reference implementation to install (the paper's MATLAB sources
+    are not in the container); this arm is the CPU oracle, timed as it stands on this box's host cores.
+    One step = a bounded prefix sample of the bench workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import aig_oracle as orc
+    orc.build()
+    cores = os.cpu_count() or 1
+    n_sample = args.ref_sample
+    w = _workload(args.n)
+    for _ in range(args.warmup):
+        _oracle_sample(w, n_sample, cores)
+    tot, acc = 0.0, 0
+    for _ in range(args.steps):
+        dt, a, _r = _oracle_sample(w, n_sample, cores)
+        tot += dt
+        acc += a
+    value = n_sample * args.steps / tot
+    sample = f"first {n_sample} trajectories of {WORKLOAD_NAME} per step, {cores} threads (one trajectory per thread at a time)"
+    line = {
+        "impl": "reference", "metric": "trajectories_per_s", "value": value, "unit": "trajectories/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD_NAME, "sample": sample},
+        "accepted_steps_per_s": acc / tot,
+        "cpu_baseline": {"value": value, "unit": "trajectories/s", "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "trajectories/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_ours(args) -> int:
+    import torch
+    import torch.distributed as dist
+    from paper_2509_12381_b200 import binding as aig
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: CUDA device required (libaig has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    aig.lib()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x: int) -> int:
+        if world == 1:
+            return int(x)
+        t = torch.tensor([int(x)], dtype=torch.int64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return int(t.item())
+
+    N = int(args.n)                       # trajectories PER GPU (weak scaling)
+    w = _workload(N)
+    # rank r integrates trajectories [r*N, (r+1)*N) of the same seeded stream (no overlap)
+    y0_host = torch.from_numpy(inputs.generate_y0(w, n=N, offset=rank * N)).pin_memory()
+    y0 = y0_host.to(dev, non_blocking=True)
+    ae, le = inputs.histogram_edges()
+    ae_d, le_d = torch.from_numpy(ae).to(dev), torch.from_numpy(le).to(dev)
+    out = aig.alloc_out(N, dev)
+    ws = torch.zeros(aig.workspace_bytes(N), dtype=torch.uint8, device=dev)
+    hist = aig.alloc_hist(len(ae) - 1, len(le) - 1, 64, dev)
+
+    def step(wl, ev=None):
+        p = aig.make_params(**wl.params())
+        for v in hist.values():
+            v.zero_()
+        if ev:
+            ev[0].record()
+        aig.aig_integrate(p, y0, wl.t_max, wl.rtol, wl.atol, out=out, workspace=ws)
+        if ev:
+            ev[1].record()
+        aig.aig_histogram(out, ae_d, le_d, 64, hist=hist)
+        if world > 1:  # whole-ensemble distribution: one KB-sized sum over ranks (PAPER.md:485 concatenates on the host)
+            flat = torch.cat([hist[k] for k in ("angle", "lifetime", "n_turn", "status", "totals")])
+            dist.all_reduce(flat, op=dist.ReduceOp.SUM)
+
+    launches0 = aig.kernel_launches()
+    for _ in range(max(args.warmup, 0)):
+        step(w)
+    barrier()
+    launches_warm = aig.kernel_launches()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    e_begin, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e_begin.record()
+    for k in range(args.steps):
+        step(w, kev[k])
+    e_end.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches_timed = aig.kernel_launches() - launches_warm
+    ms_total = max_over_ranks(e_begin.elapsed_time(e_end))
+    ms_int = max_over_ranks(float(np.mean([a.elapsed_time(b) for a, b in kev])))
+
+    n_acc = int(out["n_acc"].sum(dtype=torch.int64).item())
+    n_rej = int(out["n_rej"].sum(dtype=torch.int64).item())
+    totals = aig.hist_to_numpy(hist)["totals"] if world == 1 else None
+    if totals is not None:
+        assert int(totals[0]) == n_acc and int(totals[1]) == n_rej and int(totals[3]) == N
+    acc_all, rej_all = sum_over_ranks(n_acc), sum_over_ranks(n_rej)
+    n_complex = sum_over_ranks(int(out["complex_flag"].sum(dtype=torch.int64).item()))
+    n_tmax = sum_over_ranks(int((out["status"] == 1).sum().item()))
+    max_steps_seen = int(max_over_ranks(float(out["n_acc"].max().item())))
+
+    sec = ms_total * 1e-3
+    value = world * N * args.steps / sec
+    # roofline of the dominant kernel (integrate_kernel), per launch, this rank's launches
+    flops_launch = FLOPS_PER_ATTEMPT * (n_acc + n_rej)
+    achieved = flops_launch / (ms_int * 1e-3) / 1e12
+    peak_meas, _ = aig.fp64_peak_probe(20000, 8)
+    info = aig.kernel_info()
+
+    # ---- end to end: HOST buffers through aig_run_host (alloc + H2D + kernels + D2H inside)
+    e2e = None
+    if not args.no_e2e:
+        host_out = {
+            "y_final": torch.empty((12, N), dtype=torch.float64).pin_memory(),
+            **{k: torch.empty(N, dtype=torch.float64).pin_memory() for k in ("t_final", "lifetime", "angle", "r_min")},
+            **{k: torch.empty(N, dtype=torch.int32).pin_memory() for k in ("n_acc", "n_rej", "n_turn", "status")},
+            "complex_flag": torch.empty(N, dtype=torch.uint8).pin_memory()}
+        host_np = {k: v.numpy() for k, v in host_out.items()}
+        p = aig.make_params(**w.params())
+        y0_np = y0_host.numpy()
+        ne = max(1, min(args.steps, args.e2e_steps))
+        aig.aig_run_host(p, y0_np, w.t_max, w.rtol, w.atol, ae, le, 64, out=host_np)  # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ne):
+            res = aig.aig_run_host(p, y0_np, w.t_max, w.rtol, w.atol, ae, le, 64, out=host_np)
+        torch.cuda.synchronize()
+        dt = max_over_ranks(time.perf_counter() - t0)
+        assert int(res["hist"]["totals"][0]) == n_acc  # same kernels, same inputs
+        hist_bytes = 8 * sum(len(v) for v in res["hist"].values())
+        e2e = {"value": world * N * ne / dt, "unit": "trajectories/s",
+               "h2d_bytes_per_step": int(y0_np.nbytes + ae.nbytes + le.nbytes),
+               "d2h_bytes_per_step": int(sum(v.nbytes for v in host_np.values() if isinstance(v, np.ndarray)) + hist_bytes),
+               "steps": ne, "ms_per_step": 1e3 * dt / ne, "host_memory": "pinned",
+               "api": "aig_run_host (C ABI, host pointers)"}
+        del host_out, host_np
+
+    # ---- the other points of configs[4]'s 3x3 sweep, once each, outside the timed region
+    sweep = []
+    if not args.no_sweep:
+        for q in SWEEP_Q:
+            for rtol in SWEEP_RTOL:
+                wl = _workload(N, q, rtol)
+                ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                barrier()
+                step(wl, ev)
+                barrier()
+                ms = max_over_ranks(ev[0].elapsed_time(ev[1]))
+                a = sum_over_ranks(int(out["n_acc"].sum(dtype=torch.int64).item()))
+                r = sum_over_ranks(int(out["n_rej"].sum(dtype=torch.int64).item()))
+                c = sum_over_ranks(int(out["complex_flag"].sum(dtype=torch.int64).item()))
+                tf = FLOPS_PER_ATTEMPT * (a + r) / world / (ms * 1e-3) / 1e12
+                sweep.append({"q": q, "rtol": rtol, "atol": wl.atol, "ms_integrate": ms,
+                              "trajectories_per_s": world * N / (ms * 1e-3),
+                              "accepted_steps_per_s": a / (ms * 1e-3),
+                              "alg_tflops_per_gpu": tf, "frac_fp64_peak": tf * 1e12 / FP64_PEAK_NOMINAL,
+                              "complex_fraction": c / (world * N)})
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import aig_oracle as orc
+        orc.build()
+        cores = os.cpu_count() or 1
+        dt, a, _r = _oracle_sample(w, args.cpu_sample, cores)
+        cpu = {"value": args.cpu_sample / dt, "unit": "trajectories/s", "cores": cores, "kind": "oracle",
+               "sample": f"first {args.cpu_sample} trajectories of the bench workload, {cores} threads, {dt:.2f} s wall",
+               "accepted_steps_per_s": a / dt}
+
+    if rank == 0:
+        line = {
+            "metric": "trajectories_per_s", "value": value, "unit": "trajectories/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAME, "trajectories_per_gpu": N,
+                       "l2": "inputs 12*8*N = %d MB and outputs %d MB per step exceed the 126 MB L2; no flush needed"
+                             % (96 * N // 2**20, 145 * N // 2**20),
+                       "parallelism": f"dp{world} (independent trajectories, contiguous index ranges)"},
+            "accepted_steps_per_s": acc_all * args.steps / sec,
+            "attempted_steps_per_s": (acc_all + rej_all) * args.steps / sec,
+            "mean_accepted_steps": acc_all / (world * N), "max_accepted_steps": max_steps_seen,
+            "complex_fraction": n_complex / (world * N), "tmax_fraction": n_tmax / (world * N),
+            "ms_integrate_kernel": ms_int,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL / 1e12, "unit": "TFLOP/s",
+                         "frac": achieved * 1e12 / FP64_PEAK_NOMINAL, "traffic": INTEGRATE_DRAM_TRAFFIC_BYTES,
+                         "kernel": "integrate_kernel<TRAP_RF>",
+                         "flops_per_attempted_step": FLOPS_PER_ATTEMPT,
+                         "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md)",
+                         "peak_measured_dfma": peak_meas / 1e12,
+                         "frac_of_measured_dfma": achieved * 1e12 / peak_meas,
+                         "hbm_bytes_algorithmic": 241 * N},
+            "kernel": info,
+            "e2e": e2e, "gpu_launches": int(launches_timed), "clocks": clocks,
+            "cpu_baseline": cpu, "sweep": sweep,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main() -> int:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=4194304, help="trajectories per GPU (default: configs[4])")
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-sample", type=int, default=65536)
+    ap.add_argument("--ref-sample", type=int, default=16384)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

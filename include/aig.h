@@ -151,6 +151,11 @@ int aig_fp64_peak_probe(int iters, int ilp, double *flops_per_s, double *elapsed
 int aig_kernel_info(int *sm_count, int *blocks_per_sm, int *threads_per_block,
                     int *regs_per_thread, int *local_bytes_per_thread);
 
+/* Number of CUDA kernels libaig has launched in this process so far (integrator, histogram and
+ * step-once kernels; the FP64 probe is not counted).  bench.py reports the difference over its
+ * timed region as "gpu_launches". */
+uint64_t aig_kernel_launches(void);
+
 const char *aig_strerror(int code);
 int aig_version(void);
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libaig.so")
 _lib = None
 
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
-           "aig_fp64_peak_probe", "aig_kernel_info", "aig_strerror", "aig_version"]
+           "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_strerror", "aig_version"]
 
 
 class AigError(RuntimeError):
@@ -80,6 +80,8 @@ def lib():
         L.aig_strerror.restype = C.c_char_p
         L.aig_strerror.argtypes = [C.c_int]
         L.aig_version.restype = C.c_int
+        L.aig_kernel_launches.restype = C.c_uint64
+        L.aig_kernel_launches.argtypes = []
         _lib = L
     return _lib
 
@@ -235,6 +237,11 @@ def kernel_info() -> dict:
     _check(lib().aig_kernel_info(*[C.byref(x) for x in v]), "aig_kernel_info")
     keys = ("sm_count", "blocks_per_sm", "threads_per_block", "regs_per_thread", "local_bytes_per_thread")
     return dict(zip(keys, [x.value for x in v]))
+
+
+def kernel_launches() -> int:
+    """Kernels libaig has launched in this process so far."""
+    return int(lib().aig_kernel_launches())
 
 
 def hist_to_numpy(hist) -> dict:

@@ -13,6 +13,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <atomic>
 #include <cuda_runtime.h>
 
 #include "../../include/aig.h"
@@ -277,6 +278,8 @@ using namespace aig;
 
 namespace {
 
+std::atomic<unsigned long long> g_kernel_launches{0};  // aig_kernel_launches()
+
 bool finite(double x) { return std::isfinite(x); }
 
 int check_params(const aig_params* p, double t_max, double rtol, double atol)
@@ -359,6 +362,7 @@ int launch_integrate(const KParams& K, const double* y0, long long N, const OutP
     const long long needed = (N + kBlock - 1) / kBlock;
     if (blocks > needed) blocks = needed;
     integrate_kernel<TRAP><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, queue);
+    g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
 
@@ -367,6 +371,8 @@ int launch_integrate(const KParams& K, const double* y0, long long N, const OutP
 extern "C" {
 
 int aig_version(void) { return AIG_VERSION; }
+
+uint64_t aig_kernel_launches(void) { return g_kernel_launches.load(); }
 
 const char* aig_strerror(int code)
 {
@@ -438,6 +444,7 @@ int aig_step_once(const aig_params* p, const double* y, const double* t, const d
         case TRAP_STATIC: step_once_kernel<TRAP_STATIC><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
         default: step_once_kernel<TRAP_NONE><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
     }
+    g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
 
@@ -486,6 +493,7 @@ int aig_histogram(const aig_out* obs, int64_t N, const aig_hist_spec* spec, cons
     const long long cap = (long long)sms * 8;
     if (blocks > cap) blocks = cap;
     histogram_kernel<<<(unsigned)blocks, 256, smem, st>>>(a, N);
+    g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
 

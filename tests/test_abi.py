@@ -1,0 +1,106 @@
+"""Host-side checks of the C ABI that need no GPU: libaig.so builds for sm_100a, loads, exports
+every symbol include/aig.h declares, validates arguments before touching the device, and the
+ctypes structs match the header's layout."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2509_12381_b200 import binding, build as aig_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    aig_build.build()
+    return binding.lib()
+
+
+def _declared_functions():
+    src = open(os.path.join(ROOT, "include", "aig.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(aig_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = _declared_functions()
+    assert {"aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host", "aig_workspace_bytes",
+            "aig_strerror", "aig_version"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(binding.EXPORTS) == names     # the binding covers the whole header, nothing else
+
+
+def test_version_strerror_workspace(lib):
+    assert lib.aig_version() == 100
+    assert lib.aig_strerror(0) == b"ok"
+    for code in range(-7, 0):
+        assert lib.aig_strerror(code) not in (b"ok", b"unknown error code")
+    assert lib.aig_strerror(-99) == b"unknown error code"
+    assert lib.aig_workspace_bytes(0) >= 8 and lib.aig_workspace_bytes(1 << 22) >= 8
+    assert lib.aig_kernel_launches() == 0       # nothing launched by loading
+
+
+def test_struct_layouts_match_header():
+    # aig_params: 13 doubles + int64 ; aig_out: 10 pointers ; aig_hist_spec: ptr,i32,ptr,i32,i32
+    assert C.sizeof(binding.Params) == 15 * 8 + 8 - 8  # 14 doubles (2+2+3+3+1+1+1+1) + int64
+    assert binding.Params.max_steps.offset == 14 * 8
+    assert C.sizeof(binding.Out) == 10 * C.sizeof(C.c_void_p)
+    assert binding.HistSpec.life_edges.offset == 16 and binding.HistSpec.n_turn_bins.offset == 28
+    assert C.sizeof(binding.Hist) == 5 * C.sizeof(C.c_void_p)
+
+
+def test_argument_validation_happens_before_any_device_work(lib):
+    p = binding.make_params(1.0, 1.0, 1.0, 1.0, (0, 0, 0), (0, 0, 0), 0.0)
+    o = binding.Out()
+    # invalid tolerances / time span / parameters are rejected on the host
+    assert lib.aig_integrate(C.byref(p), None, 4, 1.0, 0.0, 0.0, C.byref(o), None, None) == -3
+    assert lib.aig_integrate(C.byref(p), None, 4, 1.0, 1e-6, -1.0, C.byref(o), None, None) == -3
+    assert lib.aig_integrate(C.byref(p), None, 4, -1.0, 1e-6, 0.0, C.byref(o), None, None) == -4
+    assert lib.aig_integrate(C.byref(p), None, -1, 1.0, 1e-6, 0.0, C.byref(o), None, None) == -2
+    assert lib.aig_integrate(C.byref(p), None, 4, 1.0, 1e-6, 0.0, C.byref(o), None, None) == -1
+    assert lib.aig_integrate(None, None, 4, 1.0, 1e-6, 0.0, C.byref(o), None, None) == -1
+    bad = binding.make_params(0.0, 1.0, 1.0, 1.0, (0, 0, 0), (0, 0, 0), 0.0)
+    assert lib.aig_integrate(C.byref(bad), None, 4, 1.0, 1e-6, 0.0, C.byref(o), None, None) == -5
+    bad = binding.make_params(1.0, 1.0, 1.0, 1.0, (0, 0, 0), (0, 0, 0), 0.0, max_steps=0)
+    assert lib.aig_integrate(C.byref(bad), None, 4, 1.0, 1e-6, 0.0, C.byref(o), None, None) == -5
+    # N = 0 is a no-op, even without a device
+    assert lib.aig_integrate(C.byref(p), None, 0, 1.0, 1e-6, 0.0, None, None, None) == 0
+    assert lib.aig_step_once(C.byref(p), None, None, None, 0, 1e-6, 0.0, None, None, None) == 0
+    # misaligned pointers
+    o2 = binding.Out(*([0x1000] * 10))
+    assert lib.aig_integrate(C.byref(p), 0x1004, 4, 1.0, 1e-6, 0.0, C.byref(o2), 0x1000, None) == -6
+    spec = binding.HistSpec(0x1000, 0, 0x1000, 4, 4)
+    h = binding.Hist(*([0x1000] * 5))
+    assert lib.aig_histogram(C.byref(o2), 4, C.byref(spec), C.byref(h), None) == -2
+
+
+def test_no_cpu_fallback_without_cuda():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present")
+    import numpy as np
+    p = binding.make_params(1.0, 1.0, 1.0, 1.0, (0, 0, 0), (0, 0, 0), 0.0)
+    with pytest.raises(binding.AigError):
+        binding.aig_run_host(p, np.ones((12, 4)), 1.0, 1e-6, 1e-9)
+    with pytest.raises(binding.AigError):
+        binding.aig_integrate(p, None, 1.0, 1e-6, 1e-9)
+
+
+def test_product_does_not_import_oracle():
+    """The product path may not import, load, link or execute anything under oracle/ (comments
+    that mention it are fine; code that names its modules or library is not)."""
+    import re
+    pat = re.compile(r"^\s*(from|import)\s+oracle\b|aig_oracle|liboracle|oracle\.(integrate|step_once|lib|build)",
+                     re.MULTILINE)
+    pkg = os.path.join(ROOT, "paper_2509_12381_b200")
+    seen = 0
+    for dirpath, _dirs, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".inc")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not pat.search(text), f
+                seen += 1
+    assert seen >= 5
