@@ -161,7 +161,7 @@ def run_reference(args) -> int:
 def run_ours(args) -> int:
     import torch
     import torch.distributed as dist
-    from paper_2509_12381_b200 import binding as aig
+    from paper_2509_12381_b200 import binding as aig, sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -181,23 +181,15 @@ def run_ours(args) -> int:
         torch.cuda.synchronize()
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return sharding.max_over_ranks(x, dev)
 
     def sum_over_ranks(x: int) -> int:
-        if world == 1:
-            return int(x)
-        t = torch.tensor([int(x)], dtype=torch.int64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return int(t.item())
+        return sharding.sum_over_ranks(x, dev)
 
     N = int(args.n)                       # trajectories PER GPU (weak scaling)
     w = _workload(N)
     # rank r integrates trajectories [r*N, (r+1)*N) of the same seeded stream (no overlap)
-    y0_host = torch.from_numpy(inputs.generate_y0(w, n=N, offset=rank * N)).pin_memory()
+    y0_host = torch.from_numpy(sharding.shard_y0(w, rank, world, per_rank=N)[0]).pin_memory()
     y0 = y0_host.to(dev, non_blocking=True)
     ae, le = inputs.histogram_edges()
     ae_d, le_d = torch.from_numpy(ae).to(dev), torch.from_numpy(le).to(dev)
@@ -216,8 +208,7 @@ def run_ours(args) -> int:
             ev[1].record()
         aig.aig_histogram(out, ae_d, le_d, 64, hist=hist)
         if world > 1:  # whole-ensemble distribution: one KB-sized sum over ranks (PAPER.md:485 concatenates on the host)
-            flat = torch.cat([hist[k] for k in ("angle", "lifetime", "n_turn", "status", "totals")])
-            dist.all_reduce(flat, op=dist.ReduceOp.SUM)
+            sharding.allreduce_hist(hist)
 
     launches0 = aig.kernel_launches()
     for _ in range(max(args.warmup, 0)):
