@@ -6,10 +6,21 @@
 //   * the force depends on positions and time only, so the seven stages carry the six
 //     ACCELERATION components only (Nystrom form, see gen_nystrom_tableau.py) -- 42 stage
 //     doubles instead of 84, which is what lets a whole trajectory live in registers;
+//   * in that form the position of stage s needs the accelerations of stages <= s-2 only, so
+//     the six new force evaluations of a step form THREE dependent levels of two independent
+//     evaluations each (stages 2|3, 4|5, 6|7).  The step is written level by level and is
+//     branch-free (own reciprocal and cos), so the scheduler interleaves the two chains of a
+//     level: FP64 latency is 8 cycles at 2 cycles issue per warp on sm_100a, a lone dependent
+//     chain leaves 3/4 of the pipe idle;
 //   * (dV/dr)/r = 4 C4/r^6 - 8 C8/r^10 needs even powers of r only: no square root;
-//   * cos(Omega t) is evaluated five times per attempt (c6 = c7 = 1 share one, k1 is FSAL);
-//   * the error norm is a running maximum of ratios compared by cross-multiplication and
-//     divided once; the controller's fifth root is a float seed + two Newton steps.
+//     1/r^2 = MUFU.RCP64H seed + one cubic and one Newton correction (no slow-path branch);
+//   * cos(Omega t): Cody-Waite reduction + Taylor kernel (trig_constants.inc), five per attempt
+//     (c6 = c7 = 1 share one, k1 is FSAL), all issued up front;
+//   * the error norm is a maximum of ratios found by cross-multiplication in a fixed binary
+//     tree and divided once; the controller's fifth root is a float seed + one cubic correction.
+// Every product-sum is an explicit fma() and the library is compiled with -fmad=false, so the
+// arithmetic of a trajectory does not depend on which kernel (one trajectory per thread, or
+// the two-lanes-per-trajectory tail kernel) executes it: both call the functions below.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -17,8 +28,11 @@
 namespace aig {
 
 #include "dp45_nystrom_tableau.inc"
+#include "trig_constants.inc"
 
-enum TrapMode { TRAP_NONE = 0, TRAP_STATIC = 1, TRAP_RF = 2 };
+// TRAP_RF_BIG: RF trap with |Omega t| >= kCosMaxArg somewhere in the time span: libdevice cos
+// (Payne-Hanek slow path available); chosen on the host, never needed by BASELINE.json's configs.
+enum TrapMode { TRAP_NONE = 0, TRAP_STATIC = 1, TRAP_RF = 2, TRAP_RF_BIG = 3 };
 
 // Derived constants of one call; passed by value as a kernel argument (constant bank).
 struct KParams {
@@ -33,38 +47,96 @@ struct KParams {
     long long max_steps;
 };
 
+// 1/x for normal x > 0: MUFU.RCP64H seed (20 bits), cubic correction y(1 + e + e^2), one Newton
+// step.  Agrees with the IEEE quotient 1.0/x on every sampled input (measured on B200); no range
+// check: x = 0, inf or NaN give NaN or 0, which the caller's finiteness test turns into a reject.
+__device__ __forceinline__ double rcp_nr(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    const double t = fma(e, e, e);
+    y = fma(y, t, y);
+    const double e1 = fma(-x, y, 1.0);
+    return fma(y, e1, y);
+}
+
+// cos(x) for |x| < kCosMaxArg, branch-free (gen_trig_constants.py): k = round(x 2/pi),
+// r = x - k pi/2 in three FMA steps, then the cos or sin Taylor kernel in z = r^2 chosen by k mod 2
+// (coefficient table indexed, no select chain) and the sign by (k+1) mod 4 >= 2.
+__device__ __forceinline__ double cos_cw(double x)
+{
+    const double kd = fma(x, kTwoOverPi, kRoundMagic);
+    const int q = __double2loint(kd);
+    const double k = kd - kRoundMagic;
+    double r = fma(-k, kPio2_1, x);
+    r = fma(-k, kPio2_2, r);
+    r = fma(-k, kPio2_3, r);
+    const int odd = q & 1;
+    const double z = r * r;
+    double p = kTrig[odd][kTrigTerms - 1];
+#pragma unroll
+    for (int i = kTrigTerms - 2; i >= 0; --i) p = fma(p, z, kTrig[odd][i]);
+    const double base = odd ? r : 1.0;
+    const double res = fma(base * z, p, base);
+    return ((q + 1) & 2) ? -res : res;
+}
+
+template <int TRAP>
+__device__ __forceinline__ double trap_cos(const KParams& P, double t)
+{
+    if (TRAP == TRAP_RF) return cos_cw(P.omega * t);
+    if (TRAP == TRAP_RF_BIG) return cos(P.omega * t);
+    return 1.0;
+}
+
 // (dV/dr)/r and the accelerations of both particles at positions (xi, xa), cos(Omega t) = cs.
 // eq. (4)-(6): ion  acc_k = -(1/m_i)(dV/dr)(d_k/r) - w_k(t) x_k ;  eq. (8)-(10): atom acc_k = +(1/m_a)(dV/dr)(d_k/r)
-// with d = x_ion - x_atom.
+// with d = x_ion - x_atom.  X = (xi, xa), Aout = (Ai, Aa).
 template <int TRAP>
-__device__ __forceinline__ void accel(const KParams& P, double cs, const double (&xi)[3],
-                                      const double (&xa)[3], double (&Ai)[3], double (&Aa)[3],
+__device__ __forceinline__ void accel(const KParams& P, double cs, const double (&X)[6], double (&Aout)[6],
                                       double& r2_out)
 {
-    const double d0 = xi[0] - xa[0], d1 = xi[1] - xa[1], d2 = xi[2] - xa[2];
+    const double d0 = X[0] - X[3], d1 = X[1] - X[4], d2 = X[2] - X[5];
     const double r2 = fma(d2, d2, fma(d1, d1, d0 * d0));
-    const double inv2 = 1.0 / r2;
+    const double inv2 = rcp_nr(r2);
     const double inv4 = inv2 * inv2;
     const double inv6 = inv4 * inv2;
     const double g = inv6 * fma(-P.c8x8, inv4, P.c4x4);  // 4C4/r^6 - 8C8/r^10
     const double ga = g * P.inv_ma;
     const double gi = -(g * P.inv_mi);
-    Aa[0] = ga * d0;
-    Aa[1] = ga * d1;
-    Aa[2] = ga * d2;
+    Aout[3] = ga * d0;
+    Aout[4] = ga * d1;
+    Aout[5] = ga * d2;
     if (TRAP == TRAP_NONE) {
-        Ai[0] = gi * d0;
-        Ai[1] = gi * d1;
-        Ai[2] = gi * d2;
+        Aout[0] = gi * d0;
+        Aout[1] = gi * d1;
+        Aout[2] = gi * d2;
     } else {
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const double w = (TRAP == TRAP_RF) ? fma(P.wb[k], cs, P.wa[k]) : P.wa[k];
+            const double w = (TRAP == TRAP_STATIC) ? P.wa[k] : fma(P.wb[k], cs, P.wa[k]);
             const double dk = (k == 0) ? d0 : (k == 1 ? d1 : d2);
-            Ai[k] = fma(-w, xi[k], gi * dk);
+            Aout[k] = fma(-w, X[k], gi * dk);
         }
     }
     r2_out = r2;
+}
+
+// Position component of stage S+1 (S = 1..6): x + c h v + h^2 sum_{l <= S-2} abar_{S,l} A_l
+// (older stages first, so the newest acceleration closes the chain).  A[l] = this component's A_l.
+template <int S>
+__device__ __forceinline__ double stage_pos(double x, double v, double hc, double h2, const double (&A)[7])
+{
+    const double base = fma(hc, v, x);
+    if (S < 2) return base;
+    double acc = kAbar[S][0] * A[0];
+#pragma unroll
+    for (int l = 1; l <= S - 2; ++l) {
+        if (S == 6 && l == 1) continue;  // abar_72 = 0 exactly
+        acc = fma(kAbar[S][l], A[l], acc);
+    }
+    return fma(h2, acc, base);
 }
 
 // 16 * (spacing of doubles above |t|): ode45's hmin = 16 eps(t)
@@ -75,149 +147,181 @@ __device__ __forceinline__ double hmin_of(double t)
     return 16.0 * (up - at);
 }
 
-// q^(-1/5) for q > 0: float seed (MUFU lg2/ex2) + 2 Newton steps z <- z (1.2 - 0.2 q z^5);
-// relative error ~1e-15.  q is clamped to [1e-30, 1e30] (the result is clamped by the caller).
+// q^(-1/5) for q > 0: float seed (MUFU lg2/ex2, ~1e-7) + one cubic correction
+// z (1 + rho/5 + 3 rho^2/25), rho = 1 - q z^5 (Taylor of (1-rho)^(-1/5)); relative error ~1e-16.
+// q is clamped to [1e-30, 1e30] (the result is clamped by the caller).
 __device__ __forceinline__ double inv_fifth_root(double q)
 {
     q = fmin(fmax(q, 1e-30), 1e30);
-    double z = (double)exp2f(-0.2f * __log2f((float)q));
-    const double mq = -0.2 * q;
-#pragma unroll
-    for (int it = 0; it < 2; ++it) {
-        const double z2 = z * z;
-        const double z4 = z2 * z2;
-        z = z * fma(mq, z4 * z, 1.2);
-    }
-    return z;
+    const double z = (double)exp2f(-0.2f * __log2f((float)q));
+    const double z2 = z * z;
+    const double z4 = z2 * z2;
+    const double rho = fma(-q, z4 * z, 1.0);
+    const double t = rho * fma(0.12, rho, 0.2);
+    return fma(z, t, z);
 }
 
-// Per-lane state of one trajectory (registers).
+// A candidate of the error norm: the ratio n/d with d > 0, kept unevaluated.
+struct Ratio {
+    double n, d;
+};
+// the larger of two ratios by cross-multiplication (all denominators > 0); ties keep a
+__device__ __forceinline__ Ratio ratio_max(const Ratio a, const Ratio b)
+{
+    const bool gt = b.n * a.d > a.n * b.d;
+    Ratio r;
+    r.n = gt ? b.n : a.n;
+    r.d = gt ? b.d : a.d;
+    return r;
+}
+
+// Step end of component i (velocity and both error rows), from its seven stage accelerations:
+//   v_new = v + h sum b_l A_l ; e_v = sum E_l A_l ; e_x = h sum Ebar_l A_l  (b_2 = E_2 = Ebar_2 = b_7 = Ebar_7 = 0)
+// returns v_new and the two norm candidates |e_v| / max(|v|,|v_new|,thr), |e_x| / max(|x|,|x_new|,thr).
+__device__ __forceinline__ double step_end_component(const KParams& P, double h, double x, double xn, double v,
+                                                     const double (&A)[7], Ratio& cv, Ratio& cx)
+{
+    double sb = kB[0] * A[0];
+    sb = fma(kB[2], A[2], sb);
+    sb = fma(kB[3], A[3], sb);
+    sb = fma(kB[4], A[4], sb);
+    sb = fma(kB[5], A[5], sb);
+    const double vn = fma(h, sb, v);
+    double ev = kE[0] * A[0];
+    ev = fma(kE[2], A[2], ev);
+    ev = fma(kE[3], A[3], ev);
+    ev = fma(kE[4], A[4], ev);
+    ev = fma(kE[5], A[5], ev);
+    ev = fma(kE[6], A[6], ev);
+    double ex = kEbar[0] * A[0];
+    ex = fma(kEbar[2], A[2], ex);
+    ex = fma(kEbar[3], A[3], ex);
+    ex = fma(kEbar[4], A[4], ex);
+    ex = fma(kEbar[5], A[5], ex);
+    ex = ex * h;
+    cv.n = fabs(ev);
+    cv.d = fmax(fmax(fabs(v), fabs(vn)), P.thr);
+    cx.n = fabs(ex);
+    cx.d = fmax(fmax(fabs(x), fabs(xn)), P.thr);
+    return vn;
+}
+
+// max over the six candidates of one particle (fixed tree: ((v0,x0),(v1,x1)) , (v2,x2))
+__device__ __forceinline__ Ratio particle_norm(const Ratio (&cv)[3], const Ratio (&cx)[3])
+{
+    const Ratio a = ratio_max(cv[0], cx[0]);
+    const Ratio b = ratio_max(cv[1], cx[1]);
+    const Ratio c = ratio_max(cv[2], cx[2]);
+    return ratio_max(ratio_max(a, b), c);
+}
+
+// Per-lane state of one trajectory (registers).  X = (x_ion, x_atom), V likewise, A1 = the
+// accelerations at (t, y): stage 1, FSAL.
 struct Traj {
-    double xi[3], vi[3], xa[3], va[3];  // y at time t
-    double Ai[3], Aa[3];                // accelerations at (t, y): stage 1, FSAL
-    double t, h;
-    double rmin2, sprev, t_first, t_last;
-    int n_acc, n_rej, n_turn;
-    bool any_min, last, nofailed;
+    double X[6], V[6], A1[6];
+    double t, h, sprev;
+    int n_acc;
+    unsigned flags;  // kAnyMin | kLast | kNoFailed (one register instead of three)
+};
+constexpr unsigned kAnyMin = 1u;    // a radial minimum has been seen (arms the exit test)
+constexpr unsigned kLast = 2u;      // this attempt ends exactly at t_max
+constexpr unsigned kNoFailed = 4u;  // no failed attempt since the last accepted step
+
+// The rarely touched part of a trajectory's state (observables and counters).  The per-thread
+// integrator keeps it in shared memory (ColdShared in aig_kernels.cu: one slot per thread, SoA)
+// to stay within 168 registers at three blocks per SM; ColdRegs is the same thing in registers.
+struct ColdRegs {
+    double rmin2_, t_first_, t_last_;
+    int n_rej_, n_turn_;
+    __device__ __forceinline__ double& rmin2() { return rmin2_; }
+    __device__ __forceinline__ double& t_first() { return t_first_; }
+    __device__ __forceinline__ double& t_last() { return t_last_; }
+    __device__ __forceinline__ int& n_rej() { return n_rej_; }
+    __device__ __forceinline__ int& n_turn() { return n_turn_; }
 };
 
 // Result of one attempted step (before accept / reject).
 struct Attempt {
-    double xi[3], vi[3], xa[3], va[3];  // ynew
-    double Ai[3], Aa[3];                // stage 7 = f(t_new, ynew) accelerations
-    double t_new, err, r2, s;           // r2, s: |d|^2 and d.u at ynew (observables)
+    double X[6], V[6], A7[6];  // ynew and f(t_new, ynew) accelerations (stage 7)
+    double t_new, err, r2, s;  // r2, s: |d|^2 and d.u at ynew (observables)
 };
 
-// One attempted Dormand-Prince step of size T.h from (T.t, y), stage 1 taken from T.Ai/T.Aa.
+// scaled error estimate from the two particle norms, NaN when the new state is not finite
+__device__ __forceinline__ double error_estimate(double h, const Ratio ion, const Ratio atom, double r2, double s)
+{
+    const Ratio m = ratio_max(ion, atom);
+    double err = h * (m.n * rcp_nr(m.d));
+    // a non-finite state or force makes the estimate NaN (it must reject, like the oracle's NaN)
+    const bool finite_ok = (r2 > 0.0) && (r2 < 1.0e300) && (fabs(s) < 1.0e300);
+    if (!finite_ok) err = __longlong_as_double(0x7ff8000000000000LL);
+    return err;
+}
+
+// radial observable s = (x_atom - x_ion).(v_atom - v_ion)
+__device__ __forceinline__ double radial_s(const double (&X)[6], const double (&V)[6])
+{
+    const double u0 = V[3] - V[0], u1 = V[4] - V[1], u2 = V[5] - V[2];
+    const double e0 = X[3] - X[0], e1 = X[4] - X[1], e2 = X[5] - X[2];
+    return fma(e2, u2, fma(e1, u1, e0 * u0));
+}
+
+// One attempted Dormand-Prince step of size T.h from (T.t, y), stage 1 taken from T.A1.
 template <int TRAP>
 __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, Attempt& R)
 {
     const double h = T.h;
     const double h2 = h * h;
-    const double t_new = T.last ? P.t_max : T.t + h;
+    const double t_new = (T.flags & kLast) ? P.t_max : T.t + h;
 
-    // stage accelerations: A[l][0..2] ion, A[l][3..5] atom
-    double A[7][6];
+    // A[i][l]: acceleration component i (0-2 ion, 3-5 atom) of stage l+1
+    double A[6][7];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        A[0][k] = T.Ai[k];
-        A[0][3 + k] = T.Aa[k];
-    }
-    const double x[6] = {T.xi[0], T.xi[1], T.xi[2], T.xa[0], T.xa[1], T.xa[2]};
-    const double v[6] = {T.vi[0], T.vi[1], T.vi[2], T.va[0], T.va[1], T.va[2]};
-
-    double r2 = 0.0;
-    double xs[6];
+    for (int i = 0; i < 6; ++i) A[i][0] = T.A1[i];
+    double Xs[2][6], r2[2];
+    // three levels; the two stages of a level are independent of each other
 #pragma unroll
-    for (int s = 1; s <= 6; ++s) {
-        const double hc = h * kC[s];
+    for (int lev = 0; lev < 3; ++lev) {
+        // cos(Omega t) at the stage times of this level (independent of the positions; c6 = c7 = 1)
+        double cs[2];
+        cs[0] = trap_cos<TRAP>(P, (lev == 2) ? t_new : fma(kC[2 * lev + 1], h, T.t));
+        cs[1] = (lev == 2) ? cs[0] : trap_cos<TRAP>(P, fma(kC[2 * lev + 2], h, T.t));
 #pragma unroll
-        for (int i = 0; i < 6; ++i) {
-            double base = fma(hc, v[i], x[i]);
-            if (s >= 2) {
-                double acc = kAbar[s][0] * A[0][i];
+        for (int e = 0; e < 2; ++e) {
+            const int s = 2 * lev + 1 + e;  // stage s+1
+            const double hc = h * kC[s];
 #pragma unroll
-                for (int l = 1; l <= s - 2; ++l) {
-                    if (s == 6 && l == 1) continue;  // abar_72 = 0 exactly
-                    acc = fma(kAbar[s][l], A[l][i], acc);
-                }
-                base = fma(h2, acc, base);
+            for (int i = 0; i < 6; ++i) {
+                Xs[e][i] = (s == 1)   ? stage_pos<1>(T.X[i], T.V[i], hc, h2, A[i])
+                           : (s == 2) ? stage_pos<2>(T.X[i], T.V[i], hc, h2, A[i])
+                           : (s == 3) ? stage_pos<3>(T.X[i], T.V[i], hc, h2, A[i])
+                           : (s == 4) ? stage_pos<4>(T.X[i], T.V[i], hc, h2, A[i])
+                           : (s == 5) ? stage_pos<5>(T.X[i], T.V[i], hc, h2, A[i])
+                                      : stage_pos<6>(T.X[i], T.V[i], hc, h2, A[i]);
             }
-            xs[i] = base;
         }
-        double cs = 1.0;
-        if (TRAP == TRAP_RF) cs = cos(P.omega * ((s >= 5) ? t_new : fma(kC[s], h, T.t)));
-        const double sxi[3] = {xs[0], xs[1], xs[2]};
-        const double sxa[3] = {xs[3], xs[4], xs[5]};
-        double ai[3], aa[3];
-        // stages 6 and 7 (c = 1) have different positions, so both are evaluated; they share cs
-        accel<TRAP>(P, cs, sxi, sxa, ai, aa, r2);
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            A[s][k] = ai[k];
-            A[s][3 + k] = aa[k];
+        for (int e = 0; e < 2; ++e) {
+            const int s = 2 * lev + 1 + e;
+            double a[6];
+            accel<TRAP>(P, cs[e], Xs[e], a, r2[e]);
+#pragma unroll
+            for (int i = 0; i < 6; ++i) A[i][s] = a[i];
         }
     }
-    // xs now holds x_new (stage 7 position = 5th-order solution), A[6] = f(t_new, ynew)
-    double vn[6], emax_n = 0.0, emax_d = 1.0;  // running max of ratios n/d
+    // Xs[1] = x_new (stage 7 position = 5th-order solution), A[.][6] = f(t_new, ynew)
+    Ratio cv[6], cx[6];
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
-        // v_new = v + h sum b_l A_l   (b_2 = b_7 = 0)
-        double sb = kB[0] * A[0][i];
-        sb = fma(kB[2], A[2][i], sb);
-        sb = fma(kB[3], A[3][i], sb);
-        sb = fma(kB[4], A[4][i], sb);
-        sb = fma(kB[5], A[5][i], sb);
-        vn[i] = fma(h, sb, v[i]);
-        // velocity rows of the error estimate: sum_l E_l A_l  (E_2 = 0)
-        double ev = kE[0] * A[0][i];
-        ev = fma(kE[2], A[2][i], ev);
-        ev = fma(kE[3], A[3][i], ev);
-        ev = fma(kE[4], A[4][i], ev);
-        ev = fma(kE[5], A[5][i], ev);
-        ev = fma(kE[6], A[6][i], ev);
-        // position rows: h sum_l Ebar_l A_l  (Ebar_2 = Ebar_7 = 0)
-        double ex = kEbar[0] * A[0][i];
-        ex = fma(kEbar[2], A[2][i], ex);
-        ex = fma(kEbar[3], A[3][i], ex);
-        ex = fma(kEbar[4], A[4][i], ex);
-        ex = fma(kEbar[5], A[5][i], ex);
-        ex = ex * h;
-        const double sv = fmax(fmax(fabs(v[i]), fabs(vn[i])), P.thr);
-        const double sx = fmax(fmax(fabs(x[i]), fabs(xs[i])), P.thr);
-        const double nv = fabs(ev), nx = fabs(ex);
-        // n/d > emax_n/emax_d  <=>  n*emax_d > emax_n*d   (all denominators > 0)
-        if (nv * emax_d > emax_n * sv) {
-            emax_n = nv;
-            emax_d = sv;
-        }
-        if (nx * emax_d > emax_n * sx) {
-            emax_n = nx;
-            emax_d = sx;
-        }
+        R.X[i] = Xs[1][i];
+        R.V[i] = step_end_component(P, h, T.X[i], Xs[1][i], T.V[i], A[i], cv[i], cx[i]);
+        R.A7[i] = A[i][6];
     }
-    double err = h * (emax_n / emax_d);
-
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        R.xi[k] = xs[k];
-        R.xa[k] = xs[3 + k];
-        R.vi[k] = vn[k];
-        R.va[k] = vn[3 + k];
-        R.Ai[k] = A[6][k];
-        R.Aa[k] = A[6][3 + k];
-    }
-    // observables at the step end: d = x_atom - x_ion, u = v_atom - v_ion
-    const double u0 = vn[3] - vn[0], u1 = vn[4] - vn[1], u2 = vn[5] - vn[2];
-    const double e0 = xs[3] - xs[0], e1 = xs[4] - xs[1], e2 = xs[5] - xs[2];
-    const double s = fma(e2, u2, fma(e1, u1, e0 * u0));
-    // a non-finite state or force makes the estimate NaN (it must reject, like the oracle's NaN)
-    const bool finite_ok = (r2 > 0.0) && (r2 < 1.0e300) && (fabs(s) < 1.0e300);
-    if (!finite_ok) err = __longlong_as_double(0x7ff8000000000000LL);
+    const Ratio cvi[3] = {cv[0], cv[1], cv[2]}, cxi[3] = {cx[0], cx[1], cx[2]};
+    const Ratio cva[3] = {cv[3], cv[4], cv[5]}, cxa[3] = {cx[3], cx[4], cx[5]};
+    R.s = radial_s(R.X, R.V);
+    R.r2 = r2[1];
     R.t_new = t_new;
-    R.err = err;
-    R.r2 = r2;
-    R.s = s;
+    R.err = error_estimate(h, particle_norm(cvi, cxi), particle_norm(cva, cxa), R.r2, R.s);
 }
 
 // O3.3: clamp the step, detect the last step; called at t0 and after every accepted step.
@@ -226,40 +330,37 @@ __device__ __forceinline__ void prepare_step(const KParams& P, Traj& T)
     const double hmin = hmin_of(T.t);
     double h = fmin(P.hmax, fmax(hmin, T.h));
     const double rem = P.t_max - T.t;
-    T.last = false;
+    unsigned f = (T.flags & kAnyMin) | kNoFailed;
     if (1.1 * h >= rem) {
         h = rem;
-        T.last = true;
+        f |= kLast;
     }
     T.h = h;
-    T.nofailed = true;
+    T.flags = f;
 }
 
-// Load-time initialisation (O3.1-O3.2 + observables at t0).  y = y0 of this trajectory.
-template <int TRAP>
-__device__ __forceinline__ void init_traj(const KParams& P, Traj& T)
+// Load-time initialisation (O3.1-O3.2 + observables at t0).  T.X, T.V = y0 of this trajectory.
+template <int TRAP, class Cold>
+__device__ __forceinline__ void init_traj(const KParams& P, Traj& T, Cold& C)
 {
     T.t = P.t0;
-    double cs = 1.0;
-    if (TRAP == TRAP_RF) cs = cos(P.omega * P.t0);
+    const double cs = trap_cos<TRAP>(P, P.t0);
     double r2;
-    accel<TRAP>(P, cs, T.xi, T.xa, T.Ai, T.Aa, r2);
-    const double u0 = T.va[0] - T.vi[0], u1 = T.va[1] - T.vi[1], u2 = T.va[2] - T.vi[2];
-    const double e0 = T.xa[0] - T.xi[0], e1 = T.xa[1] - T.xi[1], e2 = T.xa[2] - T.xi[2];
-    T.sprev = fma(e2, u2, fma(e1, u1, e0 * u0));
-    T.rmin2 = r2;
-    T.t_first = 0.0;
-    T.t_last = 0.0;
-    T.n_acc = T.n_rej = T.n_turn = 0;
-    T.any_min = false;
+    accel<TRAP>(P, cs, T.X, T.A1, r2);
+    T.sprev = radial_s(T.X, T.V);
+    C.rmin2() = r2;
+    C.t_first() = 0.0;
+    C.t_last() = 0.0;
+    T.n_acc = 0;
+    C.n_rej() = 0;
+    C.n_turn() = 0;
+    T.flags = 0u;
     // initial step: rho = max_i |f_i| / max(|y_i|, thr) / (0.8 rtol^(1/5))
     double rho = 0.0;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        rho = fmax(rho, fabs(T.vi[k]) / fmax(fabs(T.xi[k]), P.thr));
-        rho = fmax(rho, fabs(T.Ai[k]) / fmax(fabs(T.vi[k]), P.thr));
-        rho = fmax(rho, fabs(T.va[k]) / fmax(fabs(T.xa[k]), P.thr));
-        rho = fmax(rho, fabs(T.Aa[k]) / fmax(fabs(T.va[k]), P.thr));
+    for (int i = 0; i < 6; ++i) {
+        rho = fmax(rho, fabs(T.V[i]) / fmax(fabs(T.X[i]), P.thr));
+        rho = fmax(rho, fabs(T.A1[i]) / fmax(fabs(T.V[i]), P.thr));
     }
     rho *= P.rho_scale;
     double h = fmin(P.hmax, P.t_max - P.t0);
@@ -271,50 +372,45 @@ __device__ __forceinline__ void init_traj(const KParams& P, Traj& T)
 // Accept / reject logic of one attempt (O3.5-O3.8).  Returns the stop status (>= 0) when the
 // trajectory has ended, -1 otherwise.  On return T holds the state to continue from (or the
 // final state).
-__device__ __forceinline__ int finish_attempt(const KParams& P, Traj& T, const Attempt& R)
+template <class Cold>
+__device__ __forceinline__ int finish_attempt(const KParams& P, Traj& T, Cold& C, const Attempt& R)
 {
     const double err = R.err;
     const double z = inv_fifth_root(err * P.inv_rtol);  // (err/rtol)^(-1/5)
     if (!(err <= P.rtol)) {
         // failed attempt
-        T.n_rej++;
+        C.n_rej()++;
         const double hmin = hmin_of(T.t);
         if (T.h <= hmin) return 3;
         double fac = 0.5;
-        if (T.nofailed) {
-            fac = (err == err) ? fmax(0.1, 0.8 * z) : 0.1;
-            T.nofailed = false;
-        }
+        if (T.flags & kNoFailed) fac = (err == err) ? fmax(0.1, 0.8 * z) : 0.1;
         T.h = fmax(hmin, T.h * fac);
-        T.last = false;
+        T.flags &= kAnyMin;  // clears kNoFailed and kLast
         return -1;
     }
     // accepted
     T.n_acc++;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        T.xi[k] = R.xi[k];
-        T.vi[k] = R.vi[k];
-        T.xa[k] = R.xa[k];
-        T.va[k] = R.va[k];
-        T.Ai[k] = R.Ai[k];
-        T.Aa[k] = R.Aa[k];
+    for (int i = 0; i < 6; ++i) {
+        T.X[i] = R.X[i];
+        T.V[i] = R.V[i];
+        T.A1[i] = R.A7[i];
     }
     T.t = R.t_new;
-    T.rmin2 = fmin(T.rmin2, R.r2);
+    if (R.r2 < C.rmin2()) C.rmin2() = R.r2;
     if (T.sprev < 0.0 && R.s >= 0.0) {  // radial minimum
-        T.any_min = true;
+        T.flags |= kAnyMin;
         if (R.r2 < P.r_turn2) {
-            T.n_turn++;
-            if (T.n_turn == 1) T.t_first = R.t_new;
-            T.t_last = R.t_new;
+            const int nt = ++C.n_turn();
+            if (nt == 1) C.t_first() = R.t_new;
+            C.t_last() = R.t_new;
         }
     }
     T.sprev = R.s;
-    if (T.any_min && R.r2 > P.r_exit2) return 0;
-    if (T.last) return 1;
+    if ((T.flags & kAnyMin) && R.r2 > P.r_exit2) return 0;
+    if (T.flags & kLast) return 1;
     if ((long long)T.n_acc >= P.max_steps) return 2;
-    if (T.nofailed) T.h = (z < 6.25) ? T.h * (0.8 * z) : 5.0 * T.h;
+    if (T.flags & kNoFailed) T.h = (z < 6.25) ? T.h * (0.8 * z) : 5.0 * T.h;
     prepare_step(P, T);
     return -1;
 }
@@ -322,9 +418,9 @@ __device__ __forceinline__ int finish_attempt(const KParams& P, Traj& T, const A
 // angle in [0, pi] between two 3-vectors: atan2(|u x v|, u.v)
 __device__ __forceinline__ double angle_between(const double (&u)[3], const double (&v)[3])
 {
-    const double cx = u[1] * v[2] - u[2] * v[1];
-    const double cy = u[2] * v[0] - u[0] * v[2];
-    const double cz = u[0] * v[1] - u[1] * v[0];
+    const double cx = fma(u[1], v[2], -(u[2] * v[1]));
+    const double cy = fma(u[2], v[0], -(u[0] * v[2]));
+    const double cz = fma(u[0], v[1], -(u[1] * v[0]));
     const double dot = fma(u[2], v[2], fma(u[1], v[1], u[0] * v[0]));
     return atan2(sqrt(fma(cz, cz, fma(cy, cy, cx * cx))), dot);
 }

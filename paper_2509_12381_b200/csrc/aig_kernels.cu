@@ -13,7 +13,9 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <algorithm>
 #include <atomic>
+#include <cstdlib>
 #include <cuda_runtime.h>
 
 #include "../../include/aig.h"
@@ -21,7 +23,14 @@
 
 namespace aig {
 
-constexpr int kBlock = 128;  // threads per block of the integrator
+#ifndef AIG_BLOCK
+#define AIG_BLOCK 128
+#endif
+#ifndef AIG_MIN_BLOCKS
+#define AIG_MIN_BLOCKS 2
+#endif
+constexpr int kBlock = AIG_BLOCK;             // threads per block of the integrator
+constexpr int kBlocksPerSM = AIG_MIN_BLOCKS;  // resident blocks per SM the register budget is sized for
 
 struct OutPtrs {
     double *y_final, *t_final, *lifetime, *angle, *r_min;
@@ -32,85 +41,202 @@ struct OutPtrs {
 // ------------------------------------------------------------------------------------------
 // integrator
 // ------------------------------------------------------------------------------------------
-template <int TRAP>
+// Cold state of the per-thread integrator: one shared-memory slot per thread, SoA (conflict-free).
+struct ColdShared {
+    __device__ __forceinline__ double& rmin2() { return s_rmin2[threadIdx.x]; }
+    __device__ __forceinline__ double& t_first() { return s_tfirst[threadIdx.x]; }
+    __device__ __forceinline__ double& t_last() { return s_tlast[threadIdx.x]; }
+    __device__ __forceinline__ int& n_rej() { return s_nrej[threadIdx.x]; }
+    __device__ __forceinline__ int& n_turn() { return s_nturn[threadIdx.x]; }
+    double* s_rmin2;
+    double* s_tfirst;
+    double* s_tlast;
+    int* s_nrej;
+    int* s_nturn;
+};
+
+template <int TRAP, class Cold>
 __device__ __forceinline__ void load_traj(const KParams& P, const double* __restrict__ y0,
-                                          long long N, long long idx, Traj& T)
+                                          long long N, long long idx, Traj& T, Cold& C)
 {
+    // rows of y0: 0-2 ion position, 3-5 ion velocity, 6-8 atom position, 9-11 atom velocity
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        T.xi[k] = __ldg(y0 + (0 + k) * N + idx);
-        T.vi[k] = __ldg(y0 + (3 + k) * N + idx);
-        T.xa[k] = __ldg(y0 + (6 + k) * N + idx);
-        T.va[k] = __ldg(y0 + (9 + k) * N + idx);
+        T.X[k] = __ldg(y0 + (0 + k) * N + idx);
+        T.V[k] = __ldg(y0 + (3 + k) * N + idx);
+        T.X[3 + k] = __ldg(y0 + (6 + k) * N + idx);
+        T.V[3 + k] = __ldg(y0 + (9 + k) * N + idx);
     }
-    init_traj<TRAP>(P, T);
+    init_traj<TRAP>(P, T, C);
 }
 
+template <class Cold>
 __device__ __forceinline__ void store_traj(const KParams& P, const double* __restrict__ y0,
-                                           long long N, long long idx, const Traj& T, int status,
+                                           long long N, long long idx, const Traj& T, Cold& C, int status,
                                            const OutPtrs& O)
 {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        O.y_final[(0 + k) * N + idx] = T.xi[k];
-        O.y_final[(3 + k) * N + idx] = T.vi[k];
-        O.y_final[(6 + k) * N + idx] = T.xa[k];
-        O.y_final[(9 + k) * N + idx] = T.va[k];
+        O.y_final[(0 + k) * N + idx] = T.X[k];
+        O.y_final[(3 + k) * N + idx] = T.V[k];
+        O.y_final[(6 + k) * N + idx] = T.X[3 + k];
+        O.y_final[(9 + k) * N + idx] = T.V[3 + k];
     }
     O.t_final[idx] = T.t;
     const double v0[3] = {__ldg(y0 + 9 * N + idx), __ldg(y0 + 10 * N + idx), __ldg(y0 + 11 * N + idx)};
-    O.angle[idx] = angle_between(v0, T.va);
-    O.r_min[idx] = sqrt(T.rmin2);
-    const bool cplx = T.n_turn >= 2;
-    O.lifetime[idx] = cplx ? T.t_last - T.t_first : 0.0;
+    const double v1[3] = {T.V[3], T.V[4], T.V[5]};
+    O.angle[idx] = angle_between(v0, v1);
+    O.r_min[idx] = sqrt(C.rmin2());
+    const int n_turn = C.n_turn();
+    const bool cplx = n_turn >= 2;
+    O.lifetime[idx] = cplx ? C.t_last() - C.t_first() : 0.0;
     O.n_acc[idx] = T.n_acc;
-    O.n_rej[idx] = T.n_rej;
-    O.n_turn[idx] = T.n_turn;
+    O.n_rej[idx] = C.n_rej();
+    O.n_turn[idx] = n_turn;
     O.status[idx] = status;
     O.complex_flag[idx] = cplx ? 1 : 0;
 }
 
-template <int TRAP>
-__global__ void __launch_bounds__(kBlock)
-integrate_kernel(const KParams P, const double* __restrict__ y0, const long long N, const OutPtrs O,
-                 unsigned long long* __restrict__ queue)
+// Checkpoint slots: the full state of a suspended trajectory, SoA over `cap` slots
+// (d: 24 doubles per slot, i: 4 ints, idx: the trajectory's global index).
+struct Ckpt {
+    double* d;
+    int* i;
+    long long* idx;
+    int cap;
+};
+constexpr int kCkptDoubles = 24, kCkptInts = 4;
+constexpr size_t kCkptBytesPerSlot = kCkptDoubles * 8 + kCkptInts * 4 + 8;
+
+template <class Cold>
+__device__ __forceinline__ void ckpt_store(const Ckpt& K, int slot, long long idx, const Traj& T, Cold& C)
 {
+    double* d = K.d + slot;
+    const size_t cap = (size_t)K.cap;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        d[(0 + j) * cap] = T.X[j];
+        d[(6 + j) * cap] = T.V[j];
+        d[(12 + j) * cap] = T.A1[j];
+    }
+    d[18 * cap] = T.t;
+    d[19 * cap] = T.h;
+    d[20 * cap] = T.sprev;
+    d[21 * cap] = C.rmin2();
+    d[22 * cap] = C.t_first();
+    d[23 * cap] = C.t_last();
+    int* q = K.i + slot;
+    q[0 * cap] = T.n_acc;
+    q[1 * cap] = (int)T.flags;
+    q[2 * cap] = C.n_rej();
+    q[3 * cap] = C.n_turn();
+    K.idx[slot] = idx;
+}
+
+template <class Cold>
+__device__ __forceinline__ long long ckpt_load(const Ckpt& K, int slot, Traj& T, Cold& C)
+{
+    const double* d = K.d + slot;
+    const size_t cap = (size_t)K.cap;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        T.X[j] = d[(0 + j) * cap];
+        T.V[j] = d[(6 + j) * cap];
+        T.A1[j] = d[(12 + j) * cap];
+    }
+    T.t = d[18 * cap];
+    T.h = d[19 * cap];
+    T.sprev = d[20 * cap];
+    C.rmin2() = d[21 * cap];
+    C.t_first() = d[22 * cap];
+    C.t_last() = d[23 * cap];
+    const int* q = K.i + slot;
+    T.n_acc = q[0 * cap];
+    T.flags = (unsigned)q[1 * cap];
+    C.n_rej() = q[2 * cap];
+    C.n_turn() = q[3 * cap];
+    return K.idx[slot];
+}
+
+// Scheduling arguments of one integrator launch (a stage of the schedule in aig_integrate).
+//   fresh stage  (RESUME = 0): work items are trajectory indices [0, N), state from y0;
+//   resume stage (RESUME = 1): work items are the slots [0, *n_in) of `in`, state from the slot.
+// A lane whose trajectory has neither ended nor been suspended keeps stepping; it is suspended
+// (state written to `out`, slot taken from *n_out) when it has taken `budget` accepted steps
+// in this stage, or -- fresh stage only -- `tail_iters` iterations after its warp has seen the
+// queue empty.  Suspension never changes a trajectory's arithmetic, only where it continues.
+struct Sched {
+    unsigned long long* queue;
+    const unsigned long long* n_in;
+    unsigned long long* n_out;
+    Ckpt in, out;
+    int budget;
+    int tail_iters;
+};
+
+template <int TRAP, int RESUME, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+integrate_kernel(const KParams P, const double* __restrict__ y0, const long long N, const OutPtrs O,
+                 const Sched S)
+{
+    __shared__ double s_rmin2[BLOCK], s_tfirst[BLOCK], s_tlast[BLOCK];
+    __shared__ int s_nrej[BLOCK], s_nturn[BLOCK];
+    ColdShared C{s_rmin2, s_tfirst, s_tlast, s_nrej, s_nturn};
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
+    const long long total = RESUME ? (long long)*S.n_in : N;
     Traj T;
     long long idx = -1;
+    int stop_at = 0;     // suspend when n_acc reaches this
+    int since_dry = 0;   // warp-uniform: iterations since the queue was seen empty
     bool live = false;
-    bool dry = false;  // warp-uniform: the queue has been seen empty
+    bool dry = false;    // warp-uniform: the queue has been seen empty
 
     for (;;) {
-        // ---- refill: lanes without a trajectory take the next indices of the queue
+        // ---- refill: lanes without a trajectory take the next items of the queue
         const unsigned need = __ballot_sync(FULL, !live);
         if (need) {
             if (!dry) {
                 const int cnt = __popc(need);
                 const int leader = __ffs(need) - 1;
                 unsigned long long base = 0;
-                if (lane == leader) base = atomicAdd(queue, (unsigned long long)cnt);
+                if (lane == leader) base = atomicAdd(S.queue, (unsigned long long)cnt);
                 base = __shfl_sync(FULL, base, leader);
                 if (!live) {
                     const long long cand = (long long)base + __popc(need & ((1u << lane) - 1u));
-                    if (cand < N) {
-                        idx = cand;
-                        load_traj<TRAP>(P, y0, N, idx, T);
+                    if (cand < total) {
+                        if (RESUME) {
+                            idx = ckpt_load(S.in, (int)cand, T, C);
+                        } else {
+                            idx = cand;
+                            load_traj<TRAP>(P, y0, N, idx, T, C);
+                        }
+                        stop_at = (S.budget > 0x7fffffff - T.n_acc) ? 0x7fffffff : T.n_acc + S.budget;
                         live = true;
                     }
                 }
-                if ((long long)base + cnt >= N) dry = true;
+                if ((long long)base + cnt >= total) dry = true;
             }
             if (!__any_sync(FULL, live)) break;
         }
+        bool suspend = false;
+        if (!RESUME && dry) suspend = (++since_dry > S.tail_iters);
         // ---- one attempted step for every live lane
         if (live) {
-            Attempt R;
-            dp45_attempt<TRAP>(P, T, R);
-            const int st = finish_attempt(P, T, R);
-            if (st >= 0) {
-                store_traj(P, y0, N, idx, T, st, O);
+            if (!suspend) {
+                Attempt R;
+                dp45_attempt<TRAP>(P, T, R);
+                const int st = finish_attempt(P, T, C, R);
+                if (st >= 0) {
+                    store_traj(P, y0, N, idx, T, C, st, O);
+                    live = false;
+                } else {
+                    suspend = T.n_acc >= stop_at;
+                }
+            }
+            if (live && suspend) {
+                const int slot = (int)atomicAdd(S.n_out, 1ULL);
+                ckpt_store(S.out, slot, idx, T, C);
                 live = false;
             }
         }
@@ -131,26 +257,31 @@ step_once_kernel(const KParams P, const double* __restrict__ y, const double* __
     Traj T;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        T.xi[k] = y[(0 + k) * N + i];
-        T.vi[k] = y[(3 + k) * N + i];
-        T.xa[k] = y[(6 + k) * N + i];
-        T.va[k] = y[(9 + k) * N + i];
+        T.X[k] = y[(0 + k) * N + i];
+        T.V[k] = y[(3 + k) * N + i];
+        T.X[3 + k] = y[(6 + k) * N + i];
+        T.V[3 + k] = y[(9 + k) * N + i];
     }
     T.t = t[i];
     T.h = h[i];
-    T.last = false;
-    double cs = 1.0;
-    if (TRAP == TRAP_RF) cs = cos(P.omega * T.t);
+    T.flags = 0u;
     double r2;
-    accel<TRAP>(P, cs, T.xi, T.xa, T.Ai, T.Aa, r2);
     Attempt R;
-    dp45_attempt<TRAP>(P, T, R);
+    // RF trap: the branch-free cos where it is valid, libdevice's beyond (the integrator makes
+    // this choice once per call on the host, from t0 and t_max)
+    if (TRAP == TRAP_RF && !(fabs(P.omega) * (fabs(T.t) + fabs(T.h)) < 0.99 * kCosMaxArg)) {
+        accel<TRAP_RF_BIG>(P, trap_cos<TRAP_RF_BIG>(P, T.t), T.X, T.A1, r2);
+        dp45_attempt<TRAP_RF_BIG>(P, T, R);
+    } else {
+        accel<TRAP>(P, trap_cos<TRAP>(P, T.t), T.X, T.A1, r2);
+        dp45_attempt<TRAP>(P, T, R);
+    }
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        ynew[(0 + k) * N + i] = R.xi[k];
-        ynew[(3 + k) * N + i] = R.vi[k];
-        ynew[(6 + k) * N + i] = R.xa[k];
-        ynew[(9 + k) * N + i] = R.va[k];
+        ynew[(0 + k) * N + i] = R.X[k];
+        ynew[(3 + k) * N + i] = R.V[k];
+        ynew[(6 + k) * N + i] = R.X[3 + k];
+        ynew[(9 + k) * N + i] = R.V[3 + k];
     }
     err[i] = R.err;
 }
@@ -297,7 +428,7 @@ int check_params(const aig_params* p, double t_max, double rtol, double atol)
     return AIG_OK;
 }
 
-int trap_mode(const aig_params* p)
+int trap_mode(const aig_params* p, double t_max)
 {
     const double w2 = p->omega_rf * p->omega_rf;
     bool any_a = false, any_q = false;
@@ -305,7 +436,10 @@ int trap_mode(const aig_params* p)
         any_a = any_a || (p->a[k] * w2 != 0.0);
         any_q = any_q || (p->q[k] * w2 != 0.0);
     }
-    return any_q ? TRAP_RF : (any_a ? TRAP_STATIC : TRAP_NONE);
+    if (!any_q) return any_a ? TRAP_STATIC : TRAP_NONE;
+    // the branch-free cos is valid for |Omega t| < kCosMaxArg; beyond that use libdevice's cos
+    const double phase = std::fabs(p->omega_rf) * std::fmax(std::fabs(p->t0), std::fabs(t_max));
+    return (phase < 0.99 * kCosMaxArg) ? TRAP_RF : TRAP_RF_BIG;
 }
 
 KParams make_kparams(const aig_params* p, double t_max, double rtol, double atol)
@@ -337,33 +471,129 @@ KParams make_kparams(const aig_params* p, double t_max, double rtol, double atol
 
 bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(ptr) % a) == 0; }
 
-template <int TRAP>
-int integrator_geometry(int* blocks_per_sm, int* sm_count)
+// ---- schedule of one aig_integrate call ------------------------------------------------------
+// Stage 0 (fresh): persistent grid of kBlock-thread blocks over the trajectory indices; lanes still
+// running kTailIters iterations after their warp saw the queue empty are suspended into checkpoint
+// buffer 0.  Stages 1..kRounds (resume): one-warp blocks over the slots the previous stage
+// wrote, so the few long-lived trajectories (bound complexes take 10^2..10^3 times the mean number
+// of steps) are packed densely into few warps spread over all SMs instead of idling 31 lanes of
+// many warps that share a sub-partition's FP64 pipe; each round suspends what exceeds its step
+// budget (x4 per round) into the other buffer, the last round has no budget.
+constexpr int kRounds = 6;
+constexpr int kRoundBlock = 32;
+constexpr int kMaxSlots = 65536;  // checkpoint slots per buffer = upper bound on stage-0 lanes
+
+struct SchedConfig {
+    int tail_iters = 256;     // stage 0: iterations a warp keeps stepping after the queue ran dry
+    int budget0 = 1 << 30;    // stage 0: accepted-step budget per trajectory (off)
+    int round_budget = 1024;  // round 1 budget; x4 per round; the last round is unbounded
+    int rounds = kRounds;
+};
+
+const SchedConfig& sched_config()
+{
+    static const SchedConfig cfg = [] {
+        SchedConfig c;  // AIG_SCHED="tail_iters,budget0,round_budget,rounds" overrides (tuning aid)
+        if (const char* e = std::getenv("AIG_SCHED")) {
+            int a = c.tail_iters, b = c.budget0, r = c.round_budget, n = c.rounds;
+            const int got = std::sscanf(e, "%d,%d,%d,%d", &a, &b, &r, &n);
+            if (got >= 1 && a >= 0) c.tail_iters = a;
+            if (got >= 2 && b >= 1) c.budget0 = b;
+            if (got >= 3 && r >= 1) c.round_budget = r;
+            if (got >= 4 && n >= 0 && n <= kRounds) c.rounds = n;
+        }
+        return c;
+    }();
+    return cfg;
+}
+
+int slot_capacity(long long N) { return (int)(N < kMaxSlots ? (N < 1 ? 1 : N) : kMaxSlots); }
+
+size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// workspace: 64 uint64 counters | checkpoint buffer 0 | checkpoint buffer 1
+constexpr size_t kCounterBytes = 64 * sizeof(unsigned long long);
+size_t ckpt_buffer_bytes(int cap) { return round_up((size_t)cap * kCkptBytesPerSlot, 256); }
+
+Ckpt ckpt_at(unsigned char* base, int cap)
+{
+    Ckpt c;
+    c.d = reinterpret_cast<double*>(base);
+    c.idx = reinterpret_cast<long long*>(base + (size_t)cap * kCkptDoubles * 8);
+    c.i = reinterpret_cast<int*>(base + (size_t)cap * (kCkptDoubles * 8 + 8));
+    c.cap = cap;
+    return c;
+}
+
+template <int TRAP, int RESUME, int BLOCK, int MINB>
+int stage_capacity(int* blocks_per_sm, int* sm_count)
 {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return AIG_ERR_CUDA;
     if (cudaDeviceGetAttribute(sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
         return AIG_ERR_CUDA;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, integrate_kernel<TRAP>, kBlock, 0) !=
-        cudaSuccess)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, integrate_kernel<TRAP, RESUME, BLOCK, MINB>,
+                                                      BLOCK, 0) != cudaSuccess)
         return AIG_ERR_CUDA;
     if (*blocks_per_sm < 1) return AIG_ERR_CUDA;
     return AIG_OK;
 }
 
+constexpr int kRoundMinBlocks = kBlock * kBlocksPerSM / kRoundBlock;  // same register budget as stage 0
+
 template <int TRAP>
-int launch_integrate(const KParams& K, const double* y0, long long N, const OutPtrs& O,
-                     unsigned long long* queue, cudaStream_t st)
+int launch_integrate(const KParams& K, const double* y0, long long N, const OutPtrs& O, void* workspace,
+                     cudaStream_t st)
 {
+    const SchedConfig& cfg = sched_config();
+    const int cap = slot_capacity(N);
+    unsigned long long* counters = static_cast<unsigned long long*>(workspace);
+    unsigned char* bufs = static_cast<unsigned char*>(workspace) + kCounterBytes;
+    const Ckpt buf[2] = {ckpt_at(bufs, cap), ckpt_at(bufs + ckpt_buffer_bytes(cap), cap)};
+    if (cudaMemsetAsync(counters, 0, kCounterBytes, st) != cudaSuccess) return AIG_ERR_CUDA;
+
     int bps = 0, sms = 0;
-    const int rc = integrator_geometry<TRAP>(&bps, &sms);
+    int rc = stage_capacity<TRAP, 0, kBlock, kBlocksPerSM>(&bps, &sms);
     if (rc) return rc;
+    // stage 0: counters[0] = queue, counters[8] = slots written to buffer 0
     long long blocks = (long long)bps * sms;
-    const long long needed = (N + kBlock - 1) / kBlock;
-    if (blocks > needed) blocks = needed;
-    integrate_kernel<TRAP><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, queue);
+    blocks = std::min(blocks, (N + kBlock - 1) / kBlock);
+    blocks = std::min(blocks, (long long)std::max(1, cap / kBlock));  // lanes <= slots
+    const bool single = (cfg.rounds == 0);
+    Sched S;
+    S.queue = counters + 0;
+    S.n_in = nullptr;
+    S.n_out = counters + 8;
+    S.in = buf[1];
+    S.out = buf[0];
+    S.budget = single ? 0x7fffffff : cfg.budget0;
+    S.tail_iters = single ? 0x7fffffff : cfg.tail_iters;
+    integrate_kernel<TRAP, 0, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
     g_kernel_launches++;
-    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
+    if (cudaGetLastError() != cudaSuccess) return AIG_ERR_CUDA;
+    if (single) return AIG_OK;
+
+    // rounds: at most `lanes0` trajectories can be suspended by stage 0, fewer by every later round
+    const long long lanes0 = blocks * kBlock;
+    rc = stage_capacity<TRAP, 1, kRoundBlock, kRoundMinBlocks>(&bps, &sms);
+    if (rc) return rc;
+    long long rblocks = std::min((long long)bps * sms, (std::min(lanes0, N) + kRoundBlock - 1) / kRoundBlock);
+    long long budget = cfg.round_budget;
+    for (int r = 1; r <= cfg.rounds; ++r) {
+        Sched R;
+        R.queue = counters + 16 + r;
+        R.n_in = counters + 8 + (r - 1);
+        R.n_out = counters + 8 + r;
+        R.in = buf[(r - 1) & 1];
+        R.out = buf[r & 1];
+        R.budget = (r == cfg.rounds) ? 0x7fffffff : (int)std::min<long long>(budget, 0x7fffffff);
+        R.tail_iters = 0x7fffffff;
+        integrate_kernel<TRAP, 1, kRoundBlock, kRoundMinBlocks><<<(unsigned)rblocks, kRoundBlock, 0, st>>>(K, y0, N, O, R);
+        g_kernel_launches++;
+        if (cudaGetLastError() != cudaSuccess) return AIG_ERR_CUDA;
+        budget *= 4;
+    }
+    return AIG_OK;
 }
 
 }  // namespace
@@ -391,8 +621,8 @@ const char* aig_strerror(int code)
 
 size_t aig_workspace_bytes(int64_t N)
 {
-    (void)N;
-    return 256;  // work-queue counter (8 bytes used), padded to its own cache lines
+    // queue / slot counters + two checkpoint buffers of min(N, 65536) suspended trajectories
+    return kCounterBytes + 2 * ckpt_buffer_bytes(slot_capacity(N));
 }
 
 int aig_integrate(const aig_params* p, const double* y0, int64_t N, double t_max, double rtol,
@@ -415,12 +645,11 @@ int aig_integrate(const aig_params* p, const double* y0, int64_t N, double t_max
     const KParams K = make_kparams(p, t_max, rtol, atol);
     OutPtrs O{out->y_final, out->t_final, out->lifetime, out->angle, out->r_min,
               out->n_acc,   out->n_rej,   out->n_turn,   out->status, out->complex_flag};
-    unsigned long long* queue = static_cast<unsigned long long*>(workspace);
-    if (cudaMemsetAsync(queue, 0, sizeof(unsigned long long), st) != cudaSuccess) return AIG_ERR_CUDA;
-    switch (trap_mode(p)) {
-        case TRAP_RF: return launch_integrate<TRAP_RF>(K, y0, N, O, queue, st);
-        case TRAP_STATIC: return launch_integrate<TRAP_STATIC>(K, y0, N, O, queue, st);
-        default: return launch_integrate<TRAP_NONE>(K, y0, N, O, queue, st);
+    switch (trap_mode(p, t_max)) {
+        case TRAP_RF: return launch_integrate<TRAP_RF>(K, y0, N, O, workspace, st);
+        case TRAP_RF_BIG: return launch_integrate<TRAP_RF_BIG>(K, y0, N, O, workspace, st);
+        case TRAP_STATIC: return launch_integrate<TRAP_STATIC>(K, y0, N, O, workspace, st);
+        default: return launch_integrate<TRAP_NONE>(K, y0, N, O, workspace, st);
     }
 }
 
@@ -439,7 +668,8 @@ int aig_step_once(const aig_params* p, const double* y, const double* t, const d
     KParams K = make_kparams(p, p->t0 + 1.0, rtol, atol);
     K.t_max = INFINITY;
     const unsigned blocks = (unsigned)((N + kBlock - 1) / kBlock);
-    switch (trap_mode(p)) {
+    switch (trap_mode(p, p->t0 + 1.0)) {
+        case TRAP_RF_BIG:
         case TRAP_RF: step_once_kernel<TRAP_RF><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
         case TRAP_STATIC: step_once_kernel<TRAP_STATIC><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
         default: step_once_kernel<TRAP_NONE><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
@@ -517,7 +747,8 @@ int aig_run_host(const aig_params* p, const double* y0_host, int64_t N, double t
         edge_words = (size_t)(hs->n_angle_bins + 1) + (hs->n_life_bins + 1);
     }
     const size_t flag_bytes = (n + 255) / 256 * 256;
-    const size_t total = 2 * b_y + 4 * b_d + 4 * b_i + flag_bytes + 256 + 8 * (hist_words + edge_words) + 4096;
+    const size_t ws_bytes = round_up(aig_workspace_bytes(N), 256);
+    const size_t total = 2 * b_y + 4 * b_d + 4 * b_i + flag_bytes + ws_bytes + 8 * (hist_words + edge_words) + 8192;
     unsigned char* slab = nullptr;
     cudaStream_t st = nullptr;
     if (cudaMalloc(&slab, total) != cudaSuccess) return AIG_ERR_CUDA;
@@ -545,7 +776,7 @@ int aig_run_host(const aig_params* p, const double* y0_host, int64_t N, double t
     d.n_turn = reinterpret_cast<int32_t*>(take(b_i));
     d.status = reinterpret_cast<int32_t*>(take(b_i));
     d.complex_flag = take(flag_bytes);
-    void* ws = take(256);
+    void* ws = take(ws_bytes);
     if (cudaMemcpyAsync(d_y0, y0_host, b_y, cudaMemcpyHostToDevice, st) != cudaSuccess) return fail(AIG_ERR_CUDA);
     rc = aig_integrate(p, d_y0, N, t_max, rtol, atol, &d, ws, st);
     if (rc) return fail(rc);
@@ -645,9 +876,9 @@ int aig_kernel_info(int* sm_count, int* blocks_per_sm, int* threads_per_block, i
                     int* local_bytes_per_thread)
 {
     cudaFuncAttributes fa;
-    if (cudaFuncGetAttributes(&fa, integrate_kernel<TRAP_RF>) != cudaSuccess) return AIG_ERR_CUDA;
+    if (cudaFuncGetAttributes(&fa, integrate_kernel<TRAP_RF, 0, kBlock, kBlocksPerSM>) != cudaSuccess) return AIG_ERR_CUDA;
     int bps = 0, sms = 0;
-    const int rc = integrator_geometry<TRAP_RF>(&bps, &sms);
+    const int rc = stage_capacity<TRAP_RF, 0, kBlock, kBlocksPerSM>(&bps, &sms);
     if (rc) return rc;
     if (sm_count) *sm_count = sms;
     if (blocks_per_sm) *blocks_per_sm = bps;
