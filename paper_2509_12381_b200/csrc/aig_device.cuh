@@ -19,8 +19,11 @@
 //   * the error norm is a maximum of ratios found by cross-multiplication in a fixed binary
 //     tree and divided once; the controller's fifth root is a float seed + one cubic correction.
 // Every product-sum is an explicit fma() and the library is compiled with -fmad=false, so the
-// arithmetic of a trajectory does not depend on which kernel (one trajectory per thread, or
-// the two-lanes-per-trajectory tail kernel) executes it: both call the functions below.
+// arithmetic of a trajectory does not depend on which kernel executes it: the per-thread
+// integrator below and the six-lanes-per-trajectory one (aig_split.cuh) call the same scalar
+// functions, and every sum that the split kernel forms across lanes (|d|^2, d.u, the error-norm
+// tree) is written here with the same operands in the same order.  Results are therefore
+// bit-identical whatever the schedule decides (tests/test_gpu_parity.py::test_schedule_invariance).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -90,7 +93,28 @@ __device__ __forceinline__ double trap_cos(const KParams& P, double t)
     return 1.0;
 }
 
-// (dV/dr)/r and the accelerations of both particles at positions (xi, xa), cos(Omega t) = cs.
+// (a + b) + c: the one order in which every three-component sum is formed (both kernels)
+__device__ __forceinline__ double sum3(double a, double b, double c) { return (a + b) + c; }
+
+// -(dV/dr)/(r m_ion) and +(dV/dr)/(r m_atom) from r^2:  (dV/dr)/r = 4 C4/r^6 - 8 C8/r^10
+__device__ __forceinline__ void force_factors(const KParams& P, double r2, double& gi, double& ga)
+{
+    const double inv2 = rcp_nr(r2);
+    const double inv4 = inv2 * inv2;
+    const double inv6 = inv4 * inv2;
+    const double g = inv6 * fma(-P.c8x8, inv4, P.c4x4);
+    ga = g * P.inv_ma;
+    gi = -(g * P.inv_mi);
+}
+
+// trap stiffness of one axis at cos(Omega t) = cs: w = wa + wb cs
+template <int TRAP>
+__device__ __forceinline__ double trap_w(double wa, double wb, double cs)
+{
+    return (TRAP == TRAP_STATIC) ? wa : fma(wb, cs, wa);
+}
+
+// Accelerations of both particles at positions (xi, xa), cos(Omega t) = cs.
 // eq. (4)-(6): ion  acc_k = -(1/m_i)(dV/dr)(d_k/r) - w_k(t) x_k ;  eq. (8)-(10): atom acc_k = +(1/m_a)(dV/dr)(d_k/r)
 // with d = x_ion - x_atom.  X = (xi, xa), Aout = (Ai, Aa).
 template <int TRAP>
@@ -98,13 +122,9 @@ __device__ __forceinline__ void accel(const KParams& P, double cs, const double 
                                       double& r2_out)
 {
     const double d0 = X[0] - X[3], d1 = X[1] - X[4], d2 = X[2] - X[5];
-    const double r2 = fma(d2, d2, fma(d1, d1, d0 * d0));
-    const double inv2 = rcp_nr(r2);
-    const double inv4 = inv2 * inv2;
-    const double inv6 = inv4 * inv2;
-    const double g = inv6 * fma(-P.c8x8, inv4, P.c4x4);  // 4C4/r^6 - 8C8/r^10
-    const double ga = g * P.inv_ma;
-    const double gi = -(g * P.inv_mi);
+    const double r2 = sum3(d0 * d0, d1 * d1, d2 * d2);
+    double gi, ga;
+    force_factors(P, r2, gi, ga);
     Aout[3] = ga * d0;
     Aout[4] = ga * d1;
     Aout[5] = ga * d2;
@@ -115,7 +135,7 @@ __device__ __forceinline__ void accel(const KParams& P, double cs, const double 
     } else {
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const double w = (TRAP == TRAP_STATIC) ? P.wa[k] : fma(P.wb[k], cs, P.wa[k]);
+            const double w = trap_w<TRAP>(P.wa[k], P.wb[k], cs);
             const double dk = (k == 0) ? d0 : (k == 1 ? d1 : d2);
             Aout[k] = fma(-w, X[k], gi * dk);
         }
@@ -215,10 +235,9 @@ __device__ __forceinline__ Ratio particle_norm(const Ratio (&cv)[3], const Ratio
     return ratio_max(ratio_max(a, b), c);
 }
 
-// Per-lane state of one trajectory (registers).  X = (x_ion, x_atom), V likewise, A1 = the
-// accelerations at (t, y): stage 1, FSAL.
-struct Traj {
-    double X[6], V[6], A1[6];
+// Controller state of one trajectory: time, step size, radial observable at t, accepted-step
+// count and flags.  The split kernel keeps a copy on each of a trajectory's six lanes.
+struct Core {
     double t, h, sprev;
     int n_acc;
     unsigned flags;  // kAnyMin | kLast | kNoFailed (one register instead of three)
@@ -226,6 +245,13 @@ struct Traj {
 constexpr unsigned kAnyMin = 1u;    // a radial minimum has been seen (arms the exit test)
 constexpr unsigned kLast = 2u;      // this attempt ends exactly at t_max
 constexpr unsigned kNoFailed = 4u;  // no failed attempt since the last accepted step
+
+// Per-lane state of one trajectory in the per-thread integrator (registers).  X = (x_ion, x_atom),
+// V likewise, A1 = the accelerations at (t, y): stage 1, FSAL.
+struct Traj {
+    double X[6], V[6], A1[6];
+    Core c;
+};
 
 // The rarely touched part of a trajectory's state (observables and counters).  The per-thread
 // integrator keeps it in shared memory (ColdShared in aig_kernels.cu: one slot per thread, SoA)
@@ -262,16 +288,16 @@ __device__ __forceinline__ double radial_s(const double (&X)[6], const double (&
 {
     const double u0 = V[3] - V[0], u1 = V[4] - V[1], u2 = V[5] - V[2];
     const double e0 = X[3] - X[0], e1 = X[4] - X[1], e2 = X[5] - X[2];
-    return fma(e2, u2, fma(e1, u1, e0 * u0));
+    return sum3(e0 * u0, e1 * u1, e2 * u2);
 }
 
-// One attempted Dormand-Prince step of size T.h from (T.t, y), stage 1 taken from T.A1.
+// One attempted Dormand-Prince step of size T.c.h from (T.c.t, y), stage 1 taken from T.A1.
 template <int TRAP>
 __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, Attempt& R)
 {
-    const double h = T.h;
+    const double h = T.c.h;
     const double h2 = h * h;
-    const double t_new = (T.flags & kLast) ? P.t_max : T.t + h;
+    const double t_new = (T.c.flags & kLast) ? P.t_max : T.c.t + h;
 
     // A[i][l]: acceleration component i (0-2 ion, 3-5 atom) of stage l+1
     double A[6][7];
@@ -283,8 +309,8 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
     for (int lev = 0; lev < 3; ++lev) {
         // cos(Omega t) at the stage times of this level (independent of the positions; c6 = c7 = 1)
         double cs[2];
-        cs[0] = trap_cos<TRAP>(P, (lev == 2) ? t_new : fma(kC[2 * lev + 1], h, T.t));
-        cs[1] = (lev == 2) ? cs[0] : trap_cos<TRAP>(P, fma(kC[2 * lev + 2], h, T.t));
+        cs[0] = trap_cos<TRAP>(P, (lev == 2) ? t_new : fma(kC[2 * lev + 1], h, T.c.t));
+        cs[1] = (lev == 2) ? cs[0] : trap_cos<TRAP>(P, fma(kC[2 * lev + 2], h, T.c.t));
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
             const int s = 2 * lev + 1 + e;  // stage s+1
@@ -325,36 +351,37 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
 }
 
 // O3.3: clamp the step, detect the last step; called at t0 and after every accepted step.
-__device__ __forceinline__ void prepare_step(const KParams& P, Traj& T)
+__device__ __forceinline__ void prepare_step(const KParams& P, Core& K)
 {
-    const double hmin = hmin_of(T.t);
-    double h = fmin(P.hmax, fmax(hmin, T.h));
-    const double rem = P.t_max - T.t;
-    unsigned f = (T.flags & kAnyMin) | kNoFailed;
+    const double hmin = hmin_of(K.t);
+    double h = fmin(P.hmax, fmax(hmin, K.h));
+    const double rem = P.t_max - K.t;
+    unsigned f = (K.flags & kAnyMin) | kNoFailed;
     if (1.1 * h >= rem) {
         h = rem;
         f |= kLast;
     }
-    T.h = h;
-    T.flags = f;
+    K.h = h;
+    K.flags = f;
 }
 
 // Load-time initialisation (O3.1-O3.2 + observables at t0).  T.X, T.V = y0 of this trajectory.
 template <int TRAP, class Cold>
 __device__ __forceinline__ void init_traj(const KParams& P, Traj& T, Cold& C)
 {
-    T.t = P.t0;
+    Core& K = T.c;
+    K.t = P.t0;
     const double cs = trap_cos<TRAP>(P, P.t0);
     double r2;
     accel<TRAP>(P, cs, T.X, T.A1, r2);
-    T.sprev = radial_s(T.X, T.V);
+    K.sprev = radial_s(T.X, T.V);
     C.rmin2() = r2;
     C.t_first() = 0.0;
     C.t_last() = 0.0;
-    T.n_acc = 0;
+    K.n_acc = 0;
     C.n_rej() = 0;
     C.n_turn() = 0;
-    T.flags = 0u;
+    K.flags = 0u;
     // initial step: rho = max_i |f_i| / max(|y_i|, thr) / (0.8 rtol^(1/5))
     double rho = 0.0;
 #pragma unroll
@@ -365,54 +392,67 @@ __device__ __forceinline__ void init_traj(const KParams& P, Traj& T, Cold& C)
     rho *= P.rho_scale;
     double h = fmin(P.hmax, P.t_max - P.t0);
     if (h * rho > 1.0) h = 1.0 / rho;
-    T.h = fmax(h, hmin_of(T.t));
-    prepare_step(P, T);
+    K.h = fmax(h, hmin_of(K.t));
+    prepare_step(P, K);
 }
 
-// Accept / reject logic of one attempt (O3.5-O3.8).  Returns the stop status (>= 0) when the
-// trajectory has ended, -1 otherwise.  On return T holds the state to continue from (or the
-// final state).
+// Accept / reject logic of one attempt (O3.5-O3.8) on the controller state: err = the scaled
+// error estimate, (t_new, r2, s) = time, |d|^2 and d.u at the attempted step end.  Sets
+// `accepted`; returns the stop status (>= 0) when the trajectory has ended, -1 otherwise.  The
+// caller moves ynew into y when `accepted` (also when the trajectory ends on this step).
+template <class Cold>
+__device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, double err, double t_new,
+                                           double r2, double s, bool& accepted)
+{
+    const double z = inv_fifth_root(err * P.inv_rtol);  // (err/rtol)^(-1/5)
+    accepted = (err <= P.rtol);
+    if (!accepted) {
+        // failed attempt
+        C.n_rej()++;
+        const double hmin = hmin_of(K.t);
+        if (K.h <= hmin) return 3;
+        double fac = 0.5;
+        if (K.flags & kNoFailed) fac = (err == err) ? fmax(0.1, 0.8 * z) : 0.1;
+        K.h = fmax(hmin, K.h * fac);
+        K.flags &= kAnyMin;  // clears kNoFailed and kLast
+        return -1;
+    }
+    K.n_acc++;
+    K.t = t_new;
+    if (r2 < C.rmin2()) C.rmin2() = r2;
+    if (K.sprev < 0.0 && s >= 0.0) {  // radial minimum
+        K.flags |= kAnyMin;
+        if (r2 < P.r_turn2) {
+            const int nt = ++C.n_turn();
+            if (nt == 1) C.t_first() = t_new;
+            C.t_last() = t_new;
+        }
+    }
+    K.sprev = s;
+    if ((K.flags & kAnyMin) && r2 > P.r_exit2) return 0;
+    if (K.flags & kLast) return 1;
+    if ((long long)K.n_acc >= P.max_steps) return 2;
+    if (K.flags & kNoFailed) K.h = (z < 6.25) ? K.h * (0.8 * z) : 5.0 * K.h;
+    prepare_step(P, K);
+    return -1;
+}
+
+// finish_core for the per-thread integrator: on return T holds the state to continue from (or
+// the final state).
 template <class Cold>
 __device__ __forceinline__ int finish_attempt(const KParams& P, Traj& T, Cold& C, const Attempt& R)
 {
-    const double err = R.err;
-    const double z = inv_fifth_root(err * P.inv_rtol);  // (err/rtol)^(-1/5)
-    if (!(err <= P.rtol)) {
-        // failed attempt
-        C.n_rej()++;
-        const double hmin = hmin_of(T.t);
-        if (T.h <= hmin) return 3;
-        double fac = 0.5;
-        if (T.flags & kNoFailed) fac = (err == err) ? fmax(0.1, 0.8 * z) : 0.1;
-        T.h = fmax(hmin, T.h * fac);
-        T.flags &= kAnyMin;  // clears kNoFailed and kLast
-        return -1;
-    }
-    // accepted
-    T.n_acc++;
+    bool accepted;
+    const int st = finish_core(P, T.c, C, R.err, R.t_new, R.r2, R.s, accepted);
+    if (accepted) {
 #pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        T.X[i] = R.X[i];
-        T.V[i] = R.V[i];
-        T.A1[i] = R.A7[i];
-    }
-    T.t = R.t_new;
-    if (R.r2 < C.rmin2()) C.rmin2() = R.r2;
-    if (T.sprev < 0.0 && R.s >= 0.0) {  // radial minimum
-        T.flags |= kAnyMin;
-        if (R.r2 < P.r_turn2) {
-            const int nt = ++C.n_turn();
-            if (nt == 1) C.t_first() = R.t_new;
-            C.t_last() = R.t_new;
+        for (int i = 0; i < 6; ++i) {
+            T.X[i] = R.X[i];
+            T.V[i] = R.V[i];
+            T.A1[i] = R.A7[i];
         }
     }
-    T.sprev = R.s;
-    if ((T.flags & kAnyMin) && R.r2 > P.r_exit2) return 0;
-    if (T.flags & kLast) return 1;
-    if ((long long)T.n_acc >= P.max_steps) return 2;
-    if (T.flags & kNoFailed) T.h = (z < 6.25) ? T.h * (0.8 * z) : 5.0 * T.h;
-    prepare_step(P, T);
-    return -1;
+    return st;
 }
 
 // angle in [0, pi] between two 3-vectors: atan2(|u x v|, u.v)

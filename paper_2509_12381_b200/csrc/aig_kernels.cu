@@ -1,12 +1,19 @@
 // aig_kernels.cu -- kernels and C ABI of libaig (include/aig.h).  sm_100a only.
 //
 // Kernels
-//   integrate_kernel<TRAP> : persistent threads, one trajectory per lane, registers only;
-//                            finished lanes refill from a global atomic work queue
-//                            (warp-aggregated: one atomicAdd per warp per refill event).
-//   step_once_kernel<TRAP> : test hook, one attempted step per thread.
-//   histogram_kernel       : shared-memory privatised bins, warp-aggregated increments.
-//   dfma_probe_kernel      : FP64 FMA chains, measures the non-tensor FP64 roofline.
+//   plan_kernel              : orders the work queue: trajectories whose impact parameter is inside
+//                              ~1.25 Langevin radii (the only ones that can reach short range and
+//                              form a long-lived complex) go first.  Scheduling only.
+//   integrate_kernel<TRAP>   : persistent threads, one trajectory per lane, registers only;
+//                              finished lanes refill from a global atomic work queue
+//                              (warp-aggregated: one atomicAdd per warp per refill event); a
+//                              trajectory that outlives the step budget is suspended into a
+//                              checkpoint slot.
+//   integrate_split_kernel<TRAP> : continues suspended trajectories, six lanes per trajectory
+//                              (aig_split.cuh): half the step latency, for the long-lived tail.
+//   step_once_kernel<TRAP>   : test hook, one attempted step per thread.
+//   histogram_kernel         : shared-memory privatised bins, warp-aggregated increments.
+//   dfma_probe_kernel        : FP64 FMA chains, measures the non-tensor FP64 roofline.
 //
 // Nothing here is a dense contraction: no tensor cores, no TMA.  The bound is the FP64 pipe;
 // global memory sees 96 B in and ~150 B out per trajectory against ~1e5 flops.
@@ -16,10 +23,12 @@
 #include <algorithm>
 #include <atomic>
 #include <cstdlib>
+#include <mutex>
 #include <cuda_runtime.h>
 
 #include "../../include/aig.h"
 #include "aig_device.cuh"
+#include "aig_split.cuh"
 
 namespace aig {
 
@@ -70,10 +79,27 @@ __device__ __forceinline__ void load_traj(const KParams& P, const double* __rest
     init_traj<TRAP>(P, T, C);
 }
 
+// scalar observables of a finished trajectory (a8); v0 / v1 = initial / final atom velocity
 template <class Cold>
-__device__ __forceinline__ void store_traj(const KParams& P, const double* __restrict__ y0,
-                                           long long N, long long idx, const Traj& T, Cold& C, int status,
-                                           const OutPtrs& O)
+__device__ __forceinline__ void store_scalars(long long idx, const Core& K, Cold& C, int status,
+                                              const double (&v0)[3], const double (&v1)[3], const OutPtrs& O)
+{
+    O.t_final[idx] = K.t;
+    O.angle[idx] = angle_between(v0, v1);
+    O.r_min[idx] = sqrt(C.rmin2());
+    const int n_turn = C.n_turn();
+    const bool cplx = n_turn >= 2;
+    O.lifetime[idx] = cplx ? C.t_last() - C.t_first() : 0.0;
+    O.n_acc[idx] = K.n_acc;
+    O.n_rej[idx] = C.n_rej();
+    O.n_turn[idx] = n_turn;
+    O.status[idx] = status;
+    O.complex_flag[idx] = cplx ? 1 : 0;
+}
+
+template <class Cold>
+__device__ __forceinline__ void store_traj(const double* __restrict__ y0, long long N, long long idx,
+                                           const Traj& T, Cold& C, int status, const OutPtrs& O)
 {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -82,34 +108,26 @@ __device__ __forceinline__ void store_traj(const KParams& P, const double* __res
         O.y_final[(6 + k) * N + idx] = T.X[3 + k];
         O.y_final[(9 + k) * N + idx] = T.V[3 + k];
     }
-    O.t_final[idx] = T.t;
     const double v0[3] = {__ldg(y0 + 9 * N + idx), __ldg(y0 + 10 * N + idx), __ldg(y0 + 11 * N + idx)};
     const double v1[3] = {T.V[3], T.V[4], T.V[5]};
-    O.angle[idx] = angle_between(v0, v1);
-    O.r_min[idx] = sqrt(C.rmin2());
-    const int n_turn = C.n_turn();
-    const bool cplx = n_turn >= 2;
-    O.lifetime[idx] = cplx ? C.t_last() - C.t_first() : 0.0;
-    O.n_acc[idx] = T.n_acc;
-    O.n_rej[idx] = C.n_rej();
-    O.n_turn[idx] = n_turn;
-    O.status[idx] = status;
-    O.complex_flag[idx] = cplx ? 1 : 0;
+    store_scalars(idx, T.c, C, status, v0, v1, O);
 }
 
 // Checkpoint slots: the full state of a suspended trajectory, SoA over `cap` slots
 // (d: 24 doubles per slot, i: 4 ints, idx: the trajectory's global index).
+//   d rows: 0-2 x_ion, 3-5 x_atom, 6-8 v_ion, 9-11 v_atom, 12-14 a_ion, 15-17 a_atom (FSAL),
+//           18 t, 19 h, 20 s(t), 21 r_min^2, 22 t_first, 23 t_last;  i rows: n_acc, flags, n_rej, n_turn
 struct Ckpt {
     double* d;
     int* i;
     long long* idx;
-    int cap;
+    long long cap;
 };
 constexpr int kCkptDoubles = 24, kCkptInts = 4;
 constexpr size_t kCkptBytesPerSlot = kCkptDoubles * 8 + kCkptInts * 4 + 8;
 
 template <class Cold>
-__device__ __forceinline__ void ckpt_store(const Ckpt& K, int slot, long long idx, const Traj& T, Cold& C)
+__device__ __forceinline__ void ckpt_store(const Ckpt& K, long long slot, long long idx, const Traj& T, Cold& C)
 {
     double* d = K.d + slot;
     const size_t cap = (size_t)K.cap;
@@ -119,62 +137,37 @@ __device__ __forceinline__ void ckpt_store(const Ckpt& K, int slot, long long id
         d[(6 + j) * cap] = T.V[j];
         d[(12 + j) * cap] = T.A1[j];
     }
-    d[18 * cap] = T.t;
-    d[19 * cap] = T.h;
-    d[20 * cap] = T.sprev;
+    d[18 * cap] = T.c.t;
+    d[19 * cap] = T.c.h;
+    d[20 * cap] = T.c.sprev;
     d[21 * cap] = C.rmin2();
     d[22 * cap] = C.t_first();
     d[23 * cap] = C.t_last();
     int* q = K.i + slot;
-    q[0 * cap] = T.n_acc;
-    q[1 * cap] = (int)T.flags;
+    q[0 * cap] = T.c.n_acc;
+    q[1 * cap] = (int)T.c.flags;
     q[2 * cap] = C.n_rej();
     q[3 * cap] = C.n_turn();
     K.idx[slot] = idx;
 }
 
-template <class Cold>
-__device__ __forceinline__ long long ckpt_load(const Ckpt& K, int slot, Traj& T, Cold& C)
-{
-    const double* d = K.d + slot;
-    const size_t cap = (size_t)K.cap;
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-        T.X[j] = d[(0 + j) * cap];
-        T.V[j] = d[(6 + j) * cap];
-        T.A1[j] = d[(12 + j) * cap];
-    }
-    T.t = d[18 * cap];
-    T.h = d[19 * cap];
-    T.sprev = d[20 * cap];
-    C.rmin2() = d[21 * cap];
-    C.t_first() = d[22 * cap];
-    C.t_last() = d[23 * cap];
-    const int* q = K.i + slot;
-    T.n_acc = q[0 * cap];
-    T.flags = (unsigned)q[1 * cap];
-    C.n_rej() = q[2 * cap];
-    C.n_turn() = q[3 * cap];
-    return K.idx[slot];
-}
-
-// Scheduling arguments of one integrator launch (a stage of the schedule in aig_integrate).
-//   fresh stage  (RESUME = 0): work items are trajectory indices [0, N), state from y0;
-//   resume stage (RESUME = 1): work items are the slots [0, *n_in) of `in`, state from the slot.
-// A lane whose trajectory has neither ended nor been suspended keeps stepping; it is suspended
-// (state written to `out`, slot taken from *n_out) when it has taken `budget` accepted steps
-// in this stage, or -- fresh stage only -- `tail_iters` iterations after its warp has seen the
-// queue empty.  Suspension never changes a trajectory's arithmetic, only where it continues.
+// Scheduling arguments of one launch of the per-thread integrator.  Work items are the entries
+// [*begin, *end) of `order` (trajectory indices; order == nullptr: the indices themselves).  A lane
+// whose trajectory has not ended is suspended (state written to slot atomicAdd(*n_out, 1) of
+// `out`) when it has taken `budget` accepted steps, or `tail_iters` iterations after its warp
+// has seen the queue empty; when the slots are exhausted it simply keeps stepping.  Suspension
+// never changes a trajectory's arithmetic, only where it continues.
 struct Sched {
     unsigned long long* queue;
-    const unsigned long long* n_in;
+    const long long* order;
+    const unsigned long long *begin, *end;
     unsigned long long* n_out;
-    Ckpt in, out;
+    Ckpt out;
     int budget;
     int tail_iters;
 };
 
-template <int TRAP, int RESUME, int BLOCK, int MINB>
+template <int TRAP, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
 integrate_kernel(const KParams P, const double* __restrict__ y0, const long long N, const OutPtrs O,
                  const Sched S)
@@ -184,13 +177,15 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
     ColdShared C{s_rmin2, s_tfirst, s_tlast, s_nrej, s_nturn};
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const long long total = RESUME ? (long long)*S.n_in : N;
+    const long long first = (long long)*S.begin;
+    const long long total = (long long)*S.end - first;
     Traj T;
     long long idx = -1;
-    int stop_at = 0;     // suspend when n_acc reaches this
-    int since_dry = 0;   // warp-uniform: iterations since the queue was seen empty
+    int stop_at = 0;      // suspend when n_acc reaches this
+    int since_dry = 0;    // warp-uniform: iterations since the queue was seen empty
     bool live = false;
-    bool dry = false;    // warp-uniform: the queue has been seen empty
+    bool dry = false;     // warp-uniform: the queue has been seen empty
+    bool may_suspend = true;
 
     for (;;) {
         // ---- refill: lanes without a trajectory take the next items of the queue
@@ -205,13 +200,10 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
                 if (!live) {
                     const long long cand = (long long)base + __popc(need & ((1u << lane) - 1u));
                     if (cand < total) {
-                        if (RESUME) {
-                            idx = ckpt_load(S.in, (int)cand, T, C);
-                        } else {
-                            idx = cand;
-                            load_traj<TRAP>(P, y0, N, idx, T, C);
-                        }
-                        stop_at = (S.budget > 0x7fffffff - T.n_acc) ? 0x7fffffff : T.n_acc + S.budget;
+                        idx = S.order ? S.order[first + cand] : first + cand;
+                        load_traj<TRAP>(P, y0, N, idx, T, C);
+                        stop_at = S.budget;
+                        may_suspend = true;
                         live = true;
                     }
                 }
@@ -219,28 +211,193 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
             }
             if (!__any_sync(FULL, live)) break;
         }
-        bool suspend = false;
-        if (!RESUME && dry) suspend = (++since_dry > S.tail_iters);
+        if (dry) ++since_dry;
         // ---- one attempted step for every live lane
         if (live) {
-            if (!suspend) {
-                Attempt R;
-                dp45_attempt<TRAP>(P, T, R);
-                const int st = finish_attempt(P, T, C, R);
-                if (st >= 0) {
-                    store_traj(P, y0, N, idx, T, C, st, O);
+            Attempt R;
+            dp45_attempt<TRAP>(P, T, R);
+            const int st = finish_attempt(P, T, C, R);
+            if (st >= 0) {
+                store_traj(y0, N, idx, T, C, st, O);
+                live = false;
+            } else if (may_suspend && (T.c.n_acc >= stop_at || since_dry > S.tail_iters)) {
+                const long long slot = (long long)atomicAdd(S.n_out, 1ULL);
+                if (slot < S.out.cap) {
+                    ckpt_store(S.out, slot, idx, T, C);
                     live = false;
                 } else {
-                    suspend = T.n_acc >= stop_at;
+                    may_suspend = false;  // no slot left: finish it here
                 }
-            }
-            if (live && suspend) {
-                const int slot = (int)atomicAdd(S.n_out, 1ULL);
-                ckpt_store(S.out, slot, idx, T, C);
-                live = false;
             }
         }
     }
+}
+
+// ---- six lanes per trajectory: continues the slots [*begin, min(*end, cap)) of `in` to their end
+struct SplitSched {
+    unsigned long long* queue;
+    const unsigned long long *begin, *end;
+    Ckpt in;
+};
+
+template <int TRAP, int MINB>
+__global__ void __launch_bounds__(32, MINB)
+integrate_split_kernel(const KParams P, const double* __restrict__ y0, const long long N, const OutPtrs O,
+                       const SplitSched S)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const SplitRole R = make_role(P);
+    const int g = lane / kGroupLanes;
+    const bool leader = !R.ghost && (lane == R.base);
+    const long long first = (long long)*S.begin;
+    const long long last = (long long)((*S.end < (unsigned long long)S.in.cap) ? *S.end : (unsigned long long)S.in.cap);
+    const long long total = last - first;
+    // benign state for lanes without a trajectory (they take part in every shuffle)
+    SplitState Y;
+    Y.xi = 1.0 + R.k;
+    Y.xa = 101.0 + 2.0 * R.k;
+    Y.vi = Y.va = Y.a1i = Y.a1a = 0.0;
+    Core K;
+    K.t = P.t0;
+    K.h = 1.0;
+    K.sprev = 0.0;
+    K.n_acc = 0;
+    K.flags = 0u;
+    ColdRegs C;
+    C.rmin2_ = C.t_first_ = C.t_last_ = 0.0;
+    C.n_rej_ = C.n_turn_ = 0;
+    long long idx = -1;
+    bool live = false;
+    bool dry = (total <= 0);
+
+    for (;;) {
+        const unsigned need = __ballot_sync(FULL, leader && !live);
+        if (need) {
+            if (!dry) {
+                const int cnt = __popc(need);
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(S.queue, (unsigned long long)cnt);
+                base = __shfl_sync(FULL, base, 0);
+                if (!R.ghost && ((need >> R.base) & 1u)) {
+                    const long long cand = (long long)base + __popc(need & ((1u << R.base) - 1u));
+                    if (cand < total) {
+                        const long long slot = first + cand;
+                        const size_t cap = (size_t)S.in.cap;
+                        const double* d = S.in.d + slot;
+                        Y.xi = d[(0 + R.k) * cap];
+                        Y.xa = d[(3 + R.k) * cap];
+                        Y.vi = d[(6 + R.k) * cap];
+                        Y.va = d[(9 + R.k) * cap];
+                        Y.a1i = d[(12 + R.k) * cap];
+                        Y.a1a = d[(15 + R.k) * cap];
+                        K.t = d[18 * cap];
+                        K.h = d[19 * cap];
+                        K.sprev = d[20 * cap];
+                        C.rmin2_ = d[21 * cap];
+                        C.t_first_ = d[22 * cap];
+                        C.t_last_ = d[23 * cap];
+                        const int* q = S.in.i + slot;
+                        K.n_acc = q[0 * cap];
+                        K.flags = (unsigned)q[1 * cap];
+                        C.n_rej_ = q[2 * cap];
+                        C.n_turn_ = q[3 * cap];
+                        idx = S.in.idx[slot];
+                        live = true;
+                    }
+                }
+                if ((long long)base + cnt >= total) dry = true;
+            }
+            if (!__any_sync(FULL, live)) break;
+        }
+        // ---- one attempted step for every group (all lanes together: full-mask shuffles inside)
+        SplitAttempt A;
+        split_attempt<TRAP>(P, R, K, Y, A);
+        int st = -1;
+        if (live) {
+            bool accepted;
+            st = finish_core(P, K, C, A.err, A.t_new, A.r2, A.s, accepted);
+            if (accepted) Y = A.Y;
+        }
+        const unsigned fin = __ballot_sync(FULL, live && st >= 0);
+        if (live && st >= 0) {
+            // a8: lanes e = 0 store component k of the final state, the group's first lane the scalars
+            const double v1[3] = {__shfl_sync(fin, Y.va, R.base), __shfl_sync(fin, Y.va, R.base + 2),
+                                  __shfl_sync(fin, Y.va, R.base + 4)};
+            if (R.e == 0) {
+                O.y_final[(0 + R.k) * N + idx] = Y.xi;
+                O.y_final[(3 + R.k) * N + idx] = Y.vi;
+                O.y_final[(6 + R.k) * N + idx] = Y.xa;
+                O.y_final[(9 + R.k) * N + idx] = Y.va;
+            }
+            if (leader) {
+                const double v0[3] = {__ldg(y0 + 9 * N + idx), __ldg(y0 + 10 * N + idx), __ldg(y0 + 11 * N + idx)};
+                store_scalars(idx, K, C, st, v0, v1, O);
+            }
+            live = false;
+            // back to benign state: the dead group keeps stepping until it is refilled or the warp ends
+            Y.xi = 1.0 + R.k;
+            Y.xa = 101.0 + 2.0 * R.k;
+            Y.vi = Y.va = Y.a1i = Y.a1a = 0.0;
+            K.t = P.t0;
+            K.h = 1.0;
+            K.flags = 0u;
+        }
+        (void)g;
+    }
+}
+
+// ---- work-queue order: trajectories that can reach short range first --------------------------
+// A trajectory can only become long (bound complex, orders of magnitude more steps) if it gets
+// over the centrifugal barrier of the -C4/r^4 tail, i.e. if its impact parameter b is below the
+// Langevin radius b_c = (4 C4/E)^(1/4), E = mu u^2/2 (relative motion at t0).  Those with
+// b < kappa b_c (kappa = 1.25: the moving ion blurs the threshold) are queued first, so that the
+// long ones are found early and continue in the split kernel while the bulk is still running.
+// Polynomial form of b^4 < kappa^4 b_c^4:  |d x u|^4 mu < 8 kappa^4 C4 |u|^2.
+// order[0 .. n_front) = candidates, order[n_front .. N) = the rest; counters[0] = n_front on exit,
+// counters[1] = number placed at the back.  Affects scheduling only, never a result.
+__global__ void __launch_bounds__(256)
+plan_kernel(const double* __restrict__ y0, const long long N, const double mu, const double c4k,
+            long long* __restrict__ order, unsigned long long* __restrict__ counters)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned FULL = 0xffffffffu;
+    bool front = false;
+    if (i < N) {
+        const double d0 = y0[6 * N + i] - y0[0 * N + i], d1 = y0[7 * N + i] - y0[1 * N + i],
+                     d2 = y0[8 * N + i] - y0[2 * N + i];
+        const double u0 = y0[9 * N + i] - y0[3 * N + i], u1 = y0[10 * N + i] - y0[4 * N + i],
+                     u2 = y0[11 * N + i] - y0[5 * N + i];
+        const double c0 = d1 * u2 - d2 * u1, c1 = d2 * u0 - d0 * u2, c2 = d0 * u1 - d1 * u0;
+        const double l2 = c0 * c0 + c1 * c1 + c2 * c2;
+        const double usq = u0 * u0 + u1 * u1 + u2 * u2;
+        front = (l2 * l2 * mu < c4k * usq);
+    }
+    const unsigned in = __ballot_sync(FULL, i < N);
+    const unsigned fr = __ballot_sync(FULL, front);
+    const unsigned bk = in & ~fr;
+    const int lane = threadIdx.x & 31;
+    unsigned long long bf = 0, bb = 0;
+    if (lane == 0) {
+        if (fr) bf = atomicAdd(&counters[0], (unsigned long long)__popc(fr));
+        if (bk) bb = atomicAdd(&counters[1], (unsigned long long)__popc(bk));
+    }
+    bf = __shfl_sync(FULL, bf, 0);
+    bb = __shfl_sync(FULL, bb, 0);
+    if (i < N) {
+        const unsigned below = (1u << lane) - 1u;
+        if (front)
+            order[bf + __popc(fr & below)] = i;
+        else
+            order[N - 1 - (long long)(bb + __popc(bk & below))] = i;
+    }
+}
+
+// counters[dst] = min(counters[src], cap): freezes the number of checkpoint slots written so far
+__global__ void snapshot_kernel(unsigned long long* counters, int dst, int src, unsigned long long cap)
+{
+    const unsigned long long v = counters[src];
+    counters[dst] = v < cap ? v : cap;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -262,18 +419,18 @@ step_once_kernel(const KParams P, const double* __restrict__ y, const double* __
         T.X[3 + k] = y[(6 + k) * N + i];
         T.V[3 + k] = y[(9 + k) * N + i];
     }
-    T.t = t[i];
-    T.h = h[i];
-    T.flags = 0u;
+    T.c.t = t[i];
+    T.c.h = h[i];
+    T.c.flags = 0u;
     double r2;
     Attempt R;
     // RF trap: the branch-free cos where it is valid, libdevice's beyond (the integrator makes
     // this choice once per call on the host, from t0 and t_max)
-    if (TRAP == TRAP_RF && !(fabs(P.omega) * (fabs(T.t) + fabs(T.h)) < 0.99 * kCosMaxArg)) {
-        accel<TRAP_RF_BIG>(P, trap_cos<TRAP_RF_BIG>(P, T.t), T.X, T.A1, r2);
+    if (TRAP == TRAP_RF && !(fabs(P.omega) * (fabs(T.c.t) + fabs(T.c.h)) < 0.99 * kCosMaxArg)) {
+        accel<TRAP_RF_BIG>(P, trap_cos<TRAP_RF_BIG>(P, T.c.t), T.X, T.A1, r2);
         dp45_attempt<TRAP_RF_BIG>(P, T, R);
     } else {
-        accel<TRAP>(P, trap_cos<TRAP>(P, T.t), T.X, T.A1, r2);
+        accel<TRAP>(P, trap_cos<TRAP>(P, T.c.t), T.X, T.A1, r2);
         dp45_attempt<TRAP>(P, T, R);
     }
 #pragma unroll
@@ -472,50 +629,69 @@ KParams make_kparams(const aig_params* p, double t_max, double rtol, double atol
 bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(ptr) % a) == 0; }
 
 // ---- schedule of one aig_integrate call ------------------------------------------------------
-// Stage 0 (fresh): persistent grid of kBlock-thread blocks over the trajectory indices; lanes still
-// running kTailIters iterations after their warp saw the queue empty are suspended into checkpoint
-// buffer 0.  Stages 1..kRounds (resume): one-warp blocks over the slots the previous stage
-// wrote, so the few long-lived trajectories (bound complexes take 10^2..10^3 times the mean number
-// of steps) are packed densely into few warps spread over all SMs instead of idling 31 lanes of
-// many warps that share a sub-partition's FP64 pipe; each round suspends what exceeds its step
-// budget (x4 per round) into the other buffer, the last round has no budget.
-constexpr int kRounds = 6;
-constexpr int kRoundBlock = 32;
-constexpr int kMaxSlots = 65536;  // checkpoint slots per buffer = upper bound on stage-0 lanes
+//   plan      order[] = capture candidates first (plan_kernel), n_front of them
+//   bulk A    per-thread integrator over the candidates; what outlives `budget` accepted steps, or
+//             is still running `tail_iters` iterations after the queue ran dry, is suspended
+//   bulk B    per-thread integrator over the rest (same rules, same slot buffer, appended)
+//   split A   six-lane integrator over the slots bulk A wrote, on a second (high-priority) stream
+//             so that it runs BESIDE bulk B: the longest trajectories (10^2..10^3 x the mean number
+//             of steps, all among the candidates) start their long sequential run early
+//   split B   six-lane integrator over the slots bulk B wrote; then the streams join.
+// No kernel ever waits for another one on the device (no polling): every dependency is a stream
+// order or an event.
+constexpr long long kMinSlots = 65536;
 
 struct SchedConfig {
-    int tail_iters = 256;     // stage 0: iterations a warp keeps stepping after the queue ran dry
-    int budget0 = 1 << 30;    // stage 0: accepted-step budget per trajectory (off)
-    int round_budget = 1024;  // round 1 budget; x4 per round; the last round is unbounded
-    int rounds = kRounds;
+    int tail_iters = 64;      // iterations a warp keeps stepping after the queue ran dry
+    int budget = 2048;        // accepted steps after which the per-thread integrator hands a trajectory over
+    int split_grid_a = 2;     // split A: one-warp blocks per SM (it shares the GPU with bulk B)
+    int split_grid_b = 8;     // split B: one-warp blocks per SM (it has the GPU to itself)
+    int plan = 1;             // 0: natural order, one bulk launch
+    double kappa = 1.25;      // candidates: b < kappa * Langevin radius
 };
 
 const SchedConfig& sched_config()
 {
     static const SchedConfig cfg = [] {
-        SchedConfig c;  // AIG_SCHED="tail_iters,budget0,round_budget,rounds" overrides (tuning aid)
+        SchedConfig c;  // AIG_SCHED="tail_iters,budget,split_grid_a,split_grid_b,plan,kappa" overrides (tuning aid)
         if (const char* e = std::getenv("AIG_SCHED")) {
-            int a = c.tail_iters, b = c.budget0, r = c.round_budget, n = c.rounds;
-            const int got = std::sscanf(e, "%d,%d,%d,%d", &a, &b, &r, &n);
+            int a = c.tail_iters, b = c.budget, ga = c.split_grid_a, gb = c.split_grid_b, pl = c.plan;
+            double kp = c.kappa;
+            const int got = std::sscanf(e, "%d,%d,%d,%d,%d,%lf", &a, &b, &ga, &gb, &pl, &kp);
             if (got >= 1 && a >= 0) c.tail_iters = a;
-            if (got >= 2 && b >= 1) c.budget0 = b;
-            if (got >= 3 && r >= 1) c.round_budget = r;
-            if (got >= 4 && n >= 0 && n <= kRounds) c.rounds = n;
+            if (got >= 2 && b >= 1) c.budget = b;
+            if (got >= 3 && ga >= 1) c.split_grid_a = ga;
+            if (got >= 4 && gb >= 1) c.split_grid_b = gb;
+            if (got >= 5) c.plan = pl;
+            if (got >= 6 && kp >= 0.0) c.kappa = kp;
         }
         return c;
     }();
     return cfg;
 }
 
-int slot_capacity(long long N) { return (int)(N < kMaxSlots ? (N < 1 ? 1 : N) : kMaxSlots); }
+long long slot_capacity(long long N) { return std::min(N < 1 ? 1 : N, std::max(kMinSlots, N / 4)); }
 
 size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// workspace: 64 uint64 counters | checkpoint buffer 0 | checkpoint buffer 1
+// workspace: 64 uint64 counters | order[N] (int64) | checkpoint slots
 constexpr size_t kCounterBytes = 64 * sizeof(unsigned long long);
-size_t ckpt_buffer_bytes(int cap) { return round_up((size_t)cap * kCkptBytesPerSlot, 256); }
+size_t order_bytes(long long N) { return round_up((size_t)(N < 1 ? 1 : N) * sizeof(long long), 256); }
+size_t ckpt_buffer_bytes(long long cap) { return round_up((size_t)cap * kCkptBytesPerSlot, 256); }
 
-Ckpt ckpt_at(unsigned char* base, int cap)
+// counters (uint64 each)
+enum Counter {
+    kCntFront = 0,   // plan: candidates placed (= n_front)
+    kCntBack = 1,    // plan: others placed
+    kCntZero = 2,    // constant 0
+    kCntN = 3,       // constant N
+    kCntQueueA = 4, kCntQueueB = 5, kCntQueueSA = 6, kCntQueueSB = 7,
+    kCntSlots = 8,   // checkpoint slots handed out so far (may overshoot the capacity)
+    kCntSlotsA = 9,  // snapshot after bulk A
+    kCntSlotsB = 10  // snapshot after bulk B
+};
+
+Ckpt ckpt_at(unsigned char* base, long long cap)
 {
     Ckpt c;
     c.d = reinterpret_cast<double*>(base);
@@ -525,75 +701,131 @@ Ckpt ckpt_at(unsigned char* base, int cap)
     return c;
 }
 
-template <int TRAP, int RESUME, int BLOCK, int MINB>
-int stage_capacity(int* blocks_per_sm, int* sm_count)
+template <int TRAP>
+int bulk_capacity(int* blocks_per_sm, int* sm_count)
 {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return AIG_ERR_CUDA;
     if (cudaDeviceGetAttribute(sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
         return AIG_ERR_CUDA;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, integrate_kernel<TRAP, RESUME, BLOCK, MINB>,
-                                                      BLOCK, 0) != cudaSuccess)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, integrate_kernel<TRAP, kBlock, kBlocksPerSM>,
+                                                      kBlock, 0) != cudaSuccess)
         return AIG_ERR_CUDA;
     if (*blocks_per_sm < 1) return AIG_ERR_CUDA;
     return AIG_OK;
 }
 
-constexpr int kRoundMinBlocks = kBlock * kBlocksPerSM / kRoundBlock;  // same register budget as stage 0
+// second stream (high priority) and the fork / join events of the schedule, one set per device
+struct SideStream {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
+    bool ok = false;
+};
+std::mutex g_side_mutex;
+
+SideStream* side_stream()
+{
+    static SideStream side[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(g_side_mutex);
+    SideStream& s = side[dev];
+    if (!s.ok) {
+        int lo = 0, hi = 0;
+        if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return nullptr;
+        if (cudaStreamCreateWithPriority(&s.stream, cudaStreamNonBlocking, hi) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        s.ok = true;
+    }
+    return &s;
+}
+
+constexpr int kSplitMinBlocks = 8;  // register cap of the split kernel: 65536 / (8 x 32) = 256
 
 template <int TRAP>
-int launch_integrate(const KParams& K, const double* y0, long long N, const OutPtrs& O, void* workspace,
-                     cudaStream_t st)
+int launch_integrate(const aig_params* p, const KParams& K, const double* y0, long long N, const OutPtrs& O,
+                     void* workspace, cudaStream_t st)
 {
     const SchedConfig& cfg = sched_config();
-    const int cap = slot_capacity(N);
+    const long long cap = slot_capacity(N);
     unsigned long long* counters = static_cast<unsigned long long*>(workspace);
-    unsigned char* bufs = static_cast<unsigned char*>(workspace) + kCounterBytes;
-    const Ckpt buf[2] = {ckpt_at(bufs, cap), ckpt_at(bufs + ckpt_buffer_bytes(cap), cap)};
+    long long* order = reinterpret_cast<long long*>(static_cast<unsigned char*>(workspace) + kCounterBytes);
+    const Ckpt slots = ckpt_at(static_cast<unsigned char*>(workspace) + kCounterBytes + order_bytes(N), cap);
     if (cudaMemsetAsync(counters, 0, kCounterBytes, st) != cudaSuccess) return AIG_ERR_CUDA;
+    const unsigned long long n64 = (unsigned long long)N;
+    if (cudaMemcpyAsync(counters + kCntN, &n64, sizeof(n64), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return AIG_ERR_CUDA;
 
     int bps = 0, sms = 0;
-    int rc = stage_capacity<TRAP, 0, kBlock, kBlocksPerSM>(&bps, &sms);
+    int rc = bulk_capacity<TRAP>(&bps, &sms);
     if (rc) return rc;
-    // stage 0: counters[0] = queue, counters[8] = slots written to buffer 0
-    long long blocks = (long long)bps * sms;
-    blocks = std::min(blocks, (N + kBlock - 1) / kBlock);
-    blocks = std::min(blocks, (long long)std::max(1, cap / kBlock));  // lanes <= slots
-    const bool single = (cfg.rounds == 0);
-    Sched S;
-    S.queue = counters + 0;
-    S.n_in = nullptr;
-    S.n_out = counters + 8;
-    S.in = buf[1];
-    S.out = buf[0];
-    S.budget = single ? 0x7fffffff : cfg.budget0;
-    S.tail_iters = single ? 0x7fffffff : cfg.tail_iters;
-    integrate_kernel<TRAP, 0, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
-    g_kernel_launches++;
-    if (cudaGetLastError() != cudaSuccess) return AIG_ERR_CUDA;
-    if (single) return AIG_OK;
+    long long blocks = std::min((long long)bps * sms, (N + kBlock - 1) / kBlock);
+    const bool plan = cfg.plan != 0 && p->C4 > 0.0;
+    SideStream* side = plan ? side_stream() : nullptr;
+    if (plan && !side) return AIG_ERR_CUDA;
 
-    // rounds: at most `lanes0` trajectories can be suspended by stage 0, fewer by every later round
-    const long long lanes0 = blocks * kBlock;
-    rc = stage_capacity<TRAP, 1, kRoundBlock, kRoundMinBlocks>(&bps, &sms);
-    if (rc) return rc;
-    long long rblocks = std::min((long long)bps * sms, (std::min(lanes0, N) + kRoundBlock - 1) / kRoundBlock);
-    long long budget = cfg.round_budget;
-    for (int r = 1; r <= cfg.rounds; ++r) {
-        Sched R;
-        R.queue = counters + 16 + r;
-        R.n_in = counters + 8 + (r - 1);
-        R.n_out = counters + 8 + r;
-        R.in = buf[(r - 1) & 1];
-        R.out = buf[r & 1];
-        R.budget = (r == cfg.rounds) ? 0x7fffffff : (int)std::min<long long>(budget, 0x7fffffff);
-        R.tail_iters = 0x7fffffff;
-        integrate_kernel<TRAP, 1, kRoundBlock, kRoundMinBlocks><<<(unsigned)rblocks, kRoundBlock, 0, st>>>(K, y0, N, O, R);
+    Sched S;
+    S.order = nullptr;
+    S.n_out = counters + kCntSlots;
+    S.out = slots;
+    S.budget = cfg.budget;
+    S.tail_iters = cfg.tail_iters;
+    SplitSched T;
+    T.in = slots;
+    const unsigned split_b = (unsigned)std::min<long long>((long long)cfg.split_grid_b * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
+
+    if (!plan) {
+        // natural order: one bulk launch, then the split kernel over everything it suspended
+        S.queue = counters + kCntQueueA;
+        S.begin = counters + kCntZero;
+        S.end = counters + kCntN;
+        integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
         g_kernel_launches++;
-        if (cudaGetLastError() != cudaSuccess) return AIG_ERR_CUDA;
-        budget *= 4;
+        T.queue = counters + kCntQueueSA;
+        T.begin = counters + kCntZero;
+        T.end = counters + kCntSlots;
+        integrate_split_kernel<TRAP, kSplitMinBlocks><<<split_b, 32, 0, st>>>(K, y0, N, O, T);
+        g_kernel_launches++;
+        return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
     }
-    return AIG_OK;
+
+    const double mu = p->m_ion * p->m_atom / (p->m_ion + p->m_atom);
+    const double k2 = cfg.kappa * cfg.kappa;
+    plan_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(y0, N, mu, 8.0 * k2 * k2 * p->C4, order, counters);
+    g_kernel_launches++;
+    // bulk A: order[0, n_front)
+    S.order = order;
+    S.queue = counters + kCntQueueA;
+    S.begin = counters + kCntZero;
+    S.end = counters + kCntFront;
+    integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
+    snapshot_kernel<<<1, 1, 0, st>>>(counters, kCntSlotsA, kCntSlots, (unsigned long long)cap);
+    g_kernel_launches += 2;
+    if (cudaEventRecord(side->fork, st) != cudaSuccess) return AIG_ERR_CUDA;
+    // split A beside bulk B
+    if (cudaStreamWaitEvent(side->stream, side->fork, 0) != cudaSuccess) return AIG_ERR_CUDA;
+    T.queue = counters + kCntQueueSA;
+    T.begin = counters + kCntZero;
+    T.end = counters + kCntSlotsA;
+    const unsigned split_a = (unsigned)std::min<long long>((long long)cfg.split_grid_a * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
+    integrate_split_kernel<TRAP, kSplitMinBlocks><<<split_a, 32, 0, side->stream>>>(K, y0, N, O, T);
+    g_kernel_launches++;
+    if (cudaEventRecord(side->join, side->stream) != cudaSuccess) return AIG_ERR_CUDA;
+    // bulk B: order[n_front, N)
+    S.queue = counters + kCntQueueB;
+    S.begin = counters + kCntFront;
+    S.end = counters + kCntN;
+    integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
+    snapshot_kernel<<<1, 1, 0, st>>>(counters, kCntSlotsB, kCntSlots, (unsigned long long)cap);
+    // split B: slots [slotsA, slotsB)
+    T.queue = counters + kCntQueueSB;
+    T.begin = counters + kCntSlotsA;
+    T.end = counters + kCntSlotsB;
+    integrate_split_kernel<TRAP, kSplitMinBlocks><<<split_b, 32, 0, st>>>(K, y0, N, O, T);
+    g_kernel_launches += 3;
+    if (cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) return AIG_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
 
 }  // namespace
@@ -621,8 +853,8 @@ const char* aig_strerror(int code)
 
 size_t aig_workspace_bytes(int64_t N)
 {
-    // queue / slot counters + two checkpoint buffers of min(N, 65536) suspended trajectories
-    return kCounterBytes + 2 * ckpt_buffer_bytes(slot_capacity(N));
+    // counters + work-queue order (8 B per trajectory) + checkpoint slots for suspended trajectories
+    return kCounterBytes + order_bytes(N) + ckpt_buffer_bytes(slot_capacity(N));
 }
 
 int aig_integrate(const aig_params* p, const double* y0, int64_t N, double t_max, double rtol,
@@ -646,10 +878,10 @@ int aig_integrate(const aig_params* p, const double* y0, int64_t N, double t_max
     OutPtrs O{out->y_final, out->t_final, out->lifetime, out->angle, out->r_min,
               out->n_acc,   out->n_rej,   out->n_turn,   out->status, out->complex_flag};
     switch (trap_mode(p, t_max)) {
-        case TRAP_RF: return launch_integrate<TRAP_RF>(K, y0, N, O, workspace, st);
-        case TRAP_RF_BIG: return launch_integrate<TRAP_RF_BIG>(K, y0, N, O, workspace, st);
-        case TRAP_STATIC: return launch_integrate<TRAP_STATIC>(K, y0, N, O, workspace, st);
-        default: return launch_integrate<TRAP_NONE>(K, y0, N, O, workspace, st);
+        case TRAP_RF: return launch_integrate<TRAP_RF>(p, K, y0, N, O, workspace, st);
+        case TRAP_RF_BIG: return launch_integrate<TRAP_RF_BIG>(p, K, y0, N, O, workspace, st);
+        case TRAP_STATIC: return launch_integrate<TRAP_STATIC>(p, K, y0, N, O, workspace, st);
+        default: return launch_integrate<TRAP_NONE>(p, K, y0, N, O, workspace, st);
     }
 }
 
@@ -876,9 +1108,9 @@ int aig_kernel_info(int* sm_count, int* blocks_per_sm, int* threads_per_block, i
                     int* local_bytes_per_thread)
 {
     cudaFuncAttributes fa;
-    if (cudaFuncGetAttributes(&fa, integrate_kernel<TRAP_RF, 0, kBlock, kBlocksPerSM>) != cudaSuccess) return AIG_ERR_CUDA;
+    if (cudaFuncGetAttributes(&fa, integrate_kernel<TRAP_RF, kBlock, kBlocksPerSM>) != cudaSuccess) return AIG_ERR_CUDA;
     int bps = 0, sms = 0;
-    const int rc = stage_capacity<TRAP_RF, 0, kBlock, kBlocksPerSM>(&bps, &sms);
+    const int rc = bulk_capacity<TRAP_RF>(&bps, &sms);
     if (rc) return rc;
     if (sm_count) *sm_count = sms;
     if (blocks_per_sm) *blocks_per_sm = bps;
