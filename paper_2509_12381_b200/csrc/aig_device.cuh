@@ -39,10 +39,10 @@ enum TrapMode { TRAP_NONE = 0, TRAP_STATIC = 1, TRAP_RF = 2, TRAP_RF_BIG = 3 };
 
 // Derived constants of one call; passed by value as a kernel argument (constant bank).
 struct KParams {
-    double inv_mi, inv_ma;  // 1/m_ion, 1/m_atom
-    double c4x4, c8x8;      // 4*C4, 8*C8
+    double g4i, g8i;        // -4 C4/m_ion, +8 C8/m_ion :  -(dV/dr)/(r m_ion)  = (g4i + g8i/r^4)/r^6
+    double g4a, g8a;        // +4 C4/m_atom, -8 C8/m_atom : +(dV/dr)/(r m_atom) = (g4a + g8a/r^4)/r^6
     double wa[3], wb[3];    // w_k(t) = wa_k + wb_k cos(Omega t): wa = a_k Om^2/4, wb = q_k Om^2/2
-    double omega;
+    double omega, half_omega;
     double t0, t_max, hmax; // hmax = 0.1 (t_max - t0)
     double rtol, inv_rtol, thr;  // thr = atol/rtol
     double rho_scale;       // 1/(0.8 rtol^(1/5)) for the initial step
@@ -50,45 +50,50 @@ struct KParams {
     long long max_steps;
 };
 
-// 1/x for normal x > 0: MUFU.RCP64H seed (20 bits), cubic correction y(1 + e + e^2), one Newton
-// step.  Agrees with the IEEE quotient 1.0/x on every sampled input (measured on B200); no range
-// check: x = 0, inf or NaN give NaN or 0, which the caller's finiteness test turns into a reject.
+// 1/x for normal x > 0: MUFU.RCP64H seed (relative error < 1e-6, measured) + one cubic correction
+// y(1 + e + e^2), e = 1 - x y: error e^3 < 1e-18 plus one rounding.  Differs from the IEEE quotient
+// 1.0/x by 1 ulp on 0.03 % of inputs and never by more (1e9 samples on B200); three dependent FMAs
+// after the seed instead of libdevice's division.  No range check: x = 0, inf or NaN give NaN or 0,
+// which the caller's finiteness test turns into a reject.
 __device__ __forceinline__ double rcp_nr(double x)
 {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double e = fma(-x, y, 1.0);
     const double t = fma(e, e, e);
-    y = fma(y, t, y);
-    const double e1 = fma(-x, y, 1.0);
-    return fma(y, e1, y);
+    return fma(y, t, y);
 }
 
-// cos(x) for |x| < kCosMaxArg, branch-free (gen_trig_constants.py): k = round(x 2/pi),
-// r = x - k pi/2 in three FMA steps, then the cos or sin Taylor kernel in z = r^2 chosen by k mod 2
-// (coefficient table indexed, no select chain) and the sign by (k+1) mod 4 >= 2.
-__device__ __forceinline__ double cos_cw(double x)
+// cos(2 y) for |y| < kCosMaxArg, branch-free and table-free (gen_trig_constants.py): k = round(y 2/pi),
+// u = y - k pi/2 in three FMA steps (|u| <= pi/4), s = sin u by its Taylor kernel in z = u^2 (two
+// interleaved Horner chains in z^2: half the dependent depth), cos(2y) = (-1)^k (1 - 2 s^2).
+// Absolute error < 2e-16 (the force only needs cos to absolute accuracy: it multiplies q_k).
+__device__ __forceinline__ double cos2_cw(double y)
 {
-    const double kd = fma(x, kTwoOverPi, kRoundMagic);
+    const double kd = fma(y, kTwoOverPi, kRoundMagic);
     const int q = __double2loint(kd);
     const double k = kd - kRoundMagic;
-    double r = fma(-k, kPio2_1, x);
-    r = fma(-k, kPio2_2, r);
-    r = fma(-k, kPio2_3, r);
-    const int odd = q & 1;
-    const double z = r * r;
-    double p = kTrig[odd][kTrigTerms - 1];
-#pragma unroll
-    for (int i = kTrigTerms - 2; i >= 0; --i) p = fma(p, z, kTrig[odd][i]);
-    const double base = odd ? r : 1.0;
-    const double res = fma(base * z, p, base);
-    return ((q + 1) & 2) ? -res : res;
+    double u = fma(-k, kPio2_1, y);
+    u = fma(-k, kPio2_2, u);
+    u = fma(-k, kPio2_3, u);
+    const double z = u * u;
+    const double w = z * z;
+    double pe = fma(kSin[6], w, kSin[4]);
+    double po = fma(kSin[7], w, kSin[5]);
+    pe = fma(pe, w, kSin[2]);
+    po = fma(po, w, kSin[3]);
+    pe = fma(pe, w, kSin[0]);
+    po = fma(po, w, kSin[1]);
+    const double p = fma(po, z, pe);
+    const double sn = fma(u * z, p, u);
+    const double res = fma(-2.0 * sn, sn, 1.0);
+    return (q & 1) ? -res : res;
 }
 
 template <int TRAP>
 __device__ __forceinline__ double trap_cos(const KParams& P, double t)
 {
-    if (TRAP == TRAP_RF) return cos_cw(P.omega * t);
+    if (TRAP == TRAP_RF) return cos2_cw(P.half_omega * t);
     if (TRAP == TRAP_RF_BIG) return cos(P.omega * t);
     return 1.0;
 }
@@ -96,15 +101,20 @@ __device__ __forceinline__ double trap_cos(const KParams& P, double t)
 // (a + b) + c: the one order in which every three-component sum is formed (both kernels)
 __device__ __forceinline__ double sum3(double a, double b, double c) { return (a + b) + c; }
 
-// -(dV/dr)/(r m_ion) and +(dV/dr)/(r m_atom) from r^2:  (dV/dr)/r = 4 C4/r^6 - 8 C8/r^10
+// plain compare-and-select maximum / minimum (one DSETP and two selects; fmax / fmin add NaN
+// quieting the callers do not need).  A NaN first operand yields the second operand.
+__device__ __forceinline__ double dmax(double a, double b) { return (a > b) ? a : b; }
+__device__ __forceinline__ double dmin(double a, double b) { return (a < b) ? a : b; }
+
+// gi = -(dV/dr)/(r m_ion) and ga = +(dV/dr)/(r m_atom) from r^2, (dV/dr)/r = 4 C4/r^6 - 8 C8/r^10:
+// the masses are folded into the constants so that both factors are three operations behind 1/r^2
 __device__ __forceinline__ void force_factors(const KParams& P, double r2, double& gi, double& ga)
 {
     const double inv2 = rcp_nr(r2);
     const double inv4 = inv2 * inv2;
     const double inv6 = inv4 * inv2;
-    const double g = inv6 * fma(-P.c8x8, inv4, P.c4x4);
-    ga = g * P.inv_ma;
-    gi = -(g * P.inv_mi);
+    gi = inv6 * fma(P.g8i, inv4, P.g4i);
+    ga = inv6 * fma(P.g8a, inv4, P.g4a);
 }
 
 // trap stiffness of one axis at cos(Omega t) = cs: w = wa + wb cs
@@ -115,7 +125,7 @@ __device__ __forceinline__ double trap_w(double wa, double wb, double cs)
 }
 
 // Accelerations of both particles at positions (xi, xa), cos(Omega t) = cs.
-// eq. (4)-(6): ion  acc_k = -(1/m_i)(dV/dr)(d_k/r) - w_k(t) x_k ;  eq. (8)-(10): atom acc_k = +(1/m_a)(dV/dr)(d_k/r)
+// eq. (4)-(6): ion  acc_k = -(1/m_i)(dV/dr)(d_k/r) - w_k(t) x_k  [the trap product first: it does not wait for 1/r^2];  eq. (8)-(10): atom acc_k = +(1/m_a)(dV/dr)(d_k/r)
 // with d = x_ion - x_atom.  X = (xi, xa), Aout = (Ai, Aa).
 template <int TRAP>
 __device__ __forceinline__ void accel(const KParams& P, double cs, const double (&X)[6], double (&Aout)[6],
@@ -137,7 +147,7 @@ __device__ __forceinline__ void accel(const KParams& P, double cs, const double 
         for (int k = 0; k < 3; ++k) {
             const double w = trap_w<TRAP>(P.wa[k], P.wb[k], cs);
             const double dk = (k == 0) ? d0 : (k == 1 ? d1 : d2);
-            Aout[k] = fma(-w, X[k], gi * dk);
+            Aout[k] = fma(gi, dk, -(w * X[k]));
         }
     }
     r2_out = r2;
@@ -172,8 +182,15 @@ __device__ __forceinline__ double hmin_of(double t)
 // q is clamped to [1e-30, 1e30] (the result is clamped by the caller).
 __device__ __forceinline__ double inv_fifth_root(double q)
 {
-    q = fmin(fmax(q, 1e-30), 1e30);
-    const double z = (double)exp2f(-0.2f * __log2f((float)q));
+    // seed in float: clamp there (two 4-cycle FMNMX instead of two FP64 compare/select pairs on the
+    // controller's dependent chain) and take MUFU.LG2 / MUFU.EX2 directly (the operand and the
+    // result are normal floats after the clamp, no denormal scaling needed)
+    const float qf = fminf(fmaxf((float)q, 1e-30f), 1e30f);
+    float lg, zf;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(qf));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(zf) : "f"(-0.2f * lg));
+    const double z = (double)zf;
+    q = dmin(dmax(q, 1e-30), 1e30);  // off the chain: only the correction needs it
     const double z2 = z * z;
     const double z4 = z2 * z2;
     const double rho = fma(-q, z4 * z, 1.0);
@@ -197,42 +214,52 @@ __device__ __forceinline__ Ratio ratio_max(const Ratio a, const Ratio b)
 
 // Step end of component i (velocity and both error rows), from its seven stage accelerations:
 //   v_new = v + h sum b_l A_l ; e_v = sum E_l A_l ; e_x = h sum Ebar_l A_l  (b_2 = E_2 = Ebar_2 = b_7 = Ebar_7 = 0)
-// returns v_new and the two norm candidates |e_v| / max(|v|,|v_new|,thr), |e_x| / max(|x|,|x_new|,thr).
-__device__ __forceinline__ double step_end_component(const KParams& P, double h, double x, double xn, double v,
-                                                     const double (&A)[7], Ratio& cv, Ratio& cx)
+// in two pieces so that everything that does not need stages 6 and 7 (the last level) can be issued
+// while that level's force evaluation is in flight.
+struct StepEndPart {
+    double sb, ev, ex;  // the three sums over stages 1, 3, 4, 5
+    double mv, mx;      // max(|v|, thr), max(|x|, thr)
+};
+__device__ __forceinline__ void step_end_begin(const KParams& P, double x, double v, const double (&A)[7],
+                                               StepEndPart& S)
 {
     double sb = kB[0] * A[0];
     sb = fma(kB[2], A[2], sb);
     sb = fma(kB[3], A[3], sb);
-    sb = fma(kB[4], A[4], sb);
-    sb = fma(kB[5], A[5], sb);
-    const double vn = fma(h, sb, v);
+    S.sb = fma(kB[4], A[4], sb);
     double ev = kE[0] * A[0];
     ev = fma(kE[2], A[2], ev);
     ev = fma(kE[3], A[3], ev);
-    ev = fma(kE[4], A[4], ev);
-    ev = fma(kE[5], A[5], ev);
-    ev = fma(kE[6], A[6], ev);
+    S.ev = fma(kE[4], A[4], ev);
     double ex = kEbar[0] * A[0];
     ex = fma(kEbar[2], A[2], ex);
     ex = fma(kEbar[3], A[3], ex);
-    ex = fma(kEbar[4], A[4], ex);
-    ex = fma(kEbar[5], A[5], ex);
-    ex = ex * h;
+    S.ex = fma(kEbar[4], A[4], ex);
+    S.mv = dmax(fabs(v), P.thr);
+    S.mx = dmax(fabs(x), P.thr);
+}
+// returns v_new and the two norm candidates |e_v| / max(|v|,|v_new|,thr), |e_x| / max(|x|,|x_new|,thr)
+__device__ __forceinline__ double step_end_finish(const StepEndPart& S, double h, double xn, double v, double A6,
+                                                  double A7, Ratio& cv, Ratio& cx)
+{
+    const double vn = fma(h, fma(kB[5], A6, S.sb), v);
+    const double ev = fma(kE[6], A7, fma(kE[5], A6, S.ev));
+    const double ex = fma(kEbar[5], A6, S.ex) * h;
     cv.n = fabs(ev);
-    cv.d = fmax(fmax(fabs(v), fabs(vn)), P.thr);
+    cv.d = dmax(fabs(vn), S.mv);
     cx.n = fabs(ex);
-    cx.d = fmax(fmax(fabs(x), fabs(xn)), P.thr);
+    cx.d = dmax(fabs(xn), S.mx);
     return vn;
 }
 
-// max over the six candidates of one particle (fixed tree: ((v0,x0),(v1,x1)) , (v2,x2))
-__device__ __forceinline__ Ratio particle_norm(const Ratio (&cv)[3], const Ratio (&cx)[3])
+// Largest of the four ratios of one axis k (velocity and position rows of both particles), found by
+// cross-multiplication in a fixed tree and divided once: max_i |e_i| / max(|y_i|, |ynew_i|, thr)
+// over the four components of that axis.  The error norm is the maximum of the three axis values
+// (an exact maximum: its order does not matter, so the split kernel can gather them in any order).
+__device__ __forceinline__ double axis_quotient(const Ratio cvi, const Ratio cxi, const Ratio cva, const Ratio cxa)
 {
-    const Ratio a = ratio_max(cv[0], cx[0]);
-    const Ratio b = ratio_max(cv[1], cx[1]);
-    const Ratio c = ratio_max(cv[2], cx[2]);
-    return ratio_max(ratio_max(a, b), c);
+    const Ratio m = ratio_max(ratio_max(cvi, cxi), ratio_max(cva, cxa));
+    return m.n * rcp_nr(m.d);
 }
 
 // Controller state of one trajectory: time, step size, radial observable at t, accepted-step
@@ -257,6 +284,7 @@ struct Traj {
 // integrator keeps it in shared memory (ColdShared in aig_kernels.cu: one slot per thread, SoA)
 // to stay within 168 registers at three blocks per SM; ColdRegs is the same thing in registers.
 struct ColdRegs {
+    static constexpr bool kInRegisters = true;
     double rmin2_, t_first_, t_last_;
     int n_rej_, n_turn_;
     __device__ __forceinline__ double& rmin2() { return rmin2_; }
@@ -272,13 +300,13 @@ struct Attempt {
     double t_new, err, r2, s;  // r2, s: |d|^2 and d.u at ynew (observables)
 };
 
-// scaled error estimate from the two particle norms, NaN when the new state is not finite
-__device__ __forceinline__ double error_estimate(double h, const Ratio ion, const Ratio atom, double r2, double s)
+// scaled error estimate from the three axis quotients, NaN when the new state is not finite
+__device__ __forceinline__ double error_estimate(double h, double q0, double q1, double q2, double r2, double s)
 {
-    const Ratio m = ratio_max(ion, atom);
-    double err = h * (m.n * rcp_nr(m.d));
+    double err = h * dmax(dmax(q0, q1), q2);
     // a non-finite state or force makes the estimate NaN (it must reject, like the oracle's NaN)
-    const bool finite_ok = (r2 > 0.0) && (r2 < 1.0e300) && (fabs(s) < 1.0e300);
+    const bool finite_ok = (r2 > 0.0) && (r2 < 1.0e300) && (fabs(s) < 1.0e300) && (q0 == q0) && (q1 == q1) &&
+                           (q2 == q2);
     if (!finite_ok) err = __longlong_as_double(0x7ff8000000000000LL);
     return err;
 }
@@ -339,23 +367,41 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
         R.X[i] = Xs[1][i];
-        R.V[i] = step_end_component(P, h, T.X[i], Xs[1][i], T.V[i], A[i], cv[i], cx[i]);
+        StepEndPart S;
+        step_end_begin(P, T.X[i], T.V[i], A[i], S);
+        R.V[i] = step_end_finish(S, h, Xs[1][i], T.V[i], A[i][5], A[i][6], cv[i], cx[i]);
         R.A7[i] = A[i][6];
     }
-    const Ratio cvi[3] = {cv[0], cv[1], cv[2]}, cxi[3] = {cx[0], cx[1], cx[2]};
-    const Ratio cva[3] = {cv[3], cv[4], cv[5]}, cxa[3] = {cx[3], cx[4], cx[5]};
     R.s = radial_s(R.X, R.V);
     R.r2 = r2[1];
     R.t_new = t_new;
-    R.err = error_estimate(h, particle_norm(cvi, cxi), particle_norm(cva, cxa), R.r2, R.s);
+    R.err = error_estimate(h, axis_quotient(cv[0], cx[0], cv[3], cx[3]), axis_quotient(cv[1], cx[1], cv[4], cx[4]),
+                           axis_quotient(cv[2], cx[2], cv[5], cx[5]), R.r2, R.s);
 }
 
-// O3.3: clamp the step, detect the last step; called at t0 and after every accepted step.
-__device__ __forceinline__ void prepare_step(const KParams& P, Core& K)
+// Times of one attempt that depend on (t, h) only: the split kernel forms them while the stages
+// are in flight, so that the controller's dependent chain after the error estimate is short.
+struct StepTimes {
+    double t_new;     // end of the attempted step (exactly t_max on the last one)
+    double hmin_cur;  // hmin at t (reject path)
+    double hmin_new;  // hmin at t_new
+    double rem_new;   // t_max - t_new
+};
+__device__ __forceinline__ StepTimes step_times(const KParams& P, const Core& K)
 {
-    const double hmin = hmin_of(K.t);
-    double h = fmin(P.hmax, fmax(hmin, K.h));
-    const double rem = P.t_max - K.t;
+    StepTimes S;
+    S.t_new = (K.flags & kLast) ? P.t_max : K.t + K.h;
+    S.hmin_cur = hmin_of(K.t);
+    S.hmin_new = hmin_of(S.t_new);
+    S.rem_new = P.t_max - S.t_new;
+    return S;
+}
+
+// O3.3: clamp the step, detect the last step; called at t0 and after every accepted step
+// (hmin, rem = hmin_of(K.t), t_max - K.t).
+__device__ __forceinline__ void prepare_step(const KParams& P, Core& K, double hmin, double rem)
+{
+    double h = dmin(P.hmax, dmax(hmin, K.h));
     unsigned f = (K.flags & kAnyMin) | kNoFailed;
     if (1.1 * h >= rem) {
         h = rem;
@@ -393,48 +439,84 @@ __device__ __forceinline__ void init_traj(const KParams& P, Traj& T, Cold& C)
     double h = fmin(P.hmax, P.t_max - P.t0);
     if (h * rho > 1.0) h = 1.0 / rho;
     K.h = fmax(h, hmin_of(K.t));
-    prepare_step(P, K);
+    prepare_step(P, K, hmin_of(K.t), P.t_max - K.t);
 }
 
 // Accept / reject logic of one attempt (O3.5-O3.8) on the controller state: err = the scaled
-// error estimate, (t_new, r2, s) = time, |d|^2 and d.u at the attempted step end.  Sets
-// `accepted`; returns the stop status (>= 0) when the trajectory has ended, -1 otherwise.  The
-// caller moves ynew into y when `accepted` (also when the trajectory ends on this step).
+// error estimate, ST = step_times() of this attempt, (r2, s) = |d|^2 and d.u at the attempted step
+// end.  Sets `accepted`; returns the stop status (>= 0) when the trajectory has ended, -1
+// otherwise.  The caller moves ynew into y when `accepted` (also when the trajectory ends on this
+// step).  `live` = false leaves everything untouched and returns -1 (lanes of the split kernel
+// that hold no trajectory).
+// Written without branches: both outcomes are formed and selected, so that the whole attempt is
+// one basic block and the scheduler can hoist what depends on (t, h) only; the step-size chain
+// behind the error estimate is what bounds the latency of a step.
 template <class Cold>
-__device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, double err, double t_new,
-                                           double r2, double s, bool& accepted)
+__device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, double err, const StepTimes& ST,
+                                           double r2, double s, bool live, bool& accepted)
 {
     const double z = inv_fifth_root(err * P.inv_rtol);  // (err/rtol)^(-1/5)
-    accepted = (err <= P.rtol);
-    if (!accepted) {
-        // failed attempt
-        C.n_rej()++;
-        const double hmin = hmin_of(K.t);
-        if (K.h <= hmin) return 3;
-        double fac = 0.5;
-        if (K.flags & kNoFailed) fac = (err == err) ? fmax(0.1, 0.8 * z) : 0.1;
-        K.h = fmax(hmin, K.h * fac);
-        K.flags &= kAnyMin;  // clears kNoFailed and kLast
-        return -1;
-    }
-    K.n_acc++;
-    K.t = t_new;
-    if (r2 < C.rmin2()) C.rmin2() = r2;
-    if (K.sprev < 0.0 && s >= 0.0) {  // radial minimum
-        K.flags |= kAnyMin;
-        if (r2 < P.r_turn2) {
-            const int nt = ++C.n_turn();
-            if (nt == 1) C.t_first() = t_new;
-            C.t_last() = t_new;
+    const bool acc = (err <= P.rtol);                   // NaN rejects
+    const unsigned fl = K.flags;
+    const bool nofailed = (fl & kNoFailed) != 0u;
+    const double h = K.h;
+    // ---- accepted: observables, stop tests, next step size (O3.6-O3.8, O3.3).  What does not
+    //      depend on z is formed first; behind z there is one product, one select, two clamps and
+    //      the last-step test.
+    const double h08 = 0.8 * h;
+    const double h_alt = nofailed ? 5.0 * h : h;  // growth limit 5, or h kept after a failure
+    const bool radial_min = (K.sprev < 0.0) && (s >= 0.0);
+    const unsigned anymin = (fl & kAnyMin) | (radial_min ? kAnyMin : 0u);
+    const bool counted = radial_min && (r2 < P.r_turn2);
+    const int n_acc1 = K.n_acc + 1;
+    const bool stop_exit = (anymin != 0u) && (r2 > P.r_exit2);
+    const bool stop_last = (fl & kLast) != 0u;
+    const bool stop_max = (long long)n_acc1 >= P.max_steps;
+    const int st_acc = stop_exit ? 0 : (stop_last ? 1 : (stop_max ? 2 : -1));
+    // h_cl = min(hmax, max(hmin_new, h_grow)) and last_new = (1.1 h_cl >= rem_new), with the three
+    // comparisons of h_grow side by side instead of one behind the other (exact selects, same values)
+    const double h_grow = (nofailed && z < 6.25) ? h08 * z : h_alt;
+    const bool over = (h_grow > P.hmax) || (ST.hmin_new > P.hmax);
+    const bool under = (h_grow < ST.hmin_new);
+    const bool last_grow = (1.1 * h_grow >= ST.rem_new);
+    const bool last_max = (1.1 * P.hmax >= ST.rem_new), last_min = (1.1 * ST.hmin_new >= ST.rem_new);
+    const double h_cl = over ? P.hmax : (under ? ST.hmin_new : h_grow);
+    const bool last_new = over ? last_max : (under ? last_min : last_grow);
+    const double h_acc = last_new ? ST.rem_new : h_cl;
+    const unsigned fl_acc = anymin | kNoFailed | (last_new ? kLast : 0u);
+    // ---- rejected: shrink (O3.5)
+    const bool underflow = (h <= ST.hmin_cur);
+    const double fac_z = (err == err) ? dmax(0.8 * z, 0.1) : 0.1;
+    const double h_rej = dmax(h * (nofailed ? fac_z : 0.5), ST.hmin_cur);
+    const int st_rej = underflow ? 3 : -1;
+    // ---- commit
+    const bool a = live && acc, r = live && !acc;
+    accepted = a;
+    if (Cold::kInRegisters) {
+        C.rmin2() = (a && r2 < C.rmin2()) ? r2 : C.rmin2();
+        const bool c = a && counted;
+        C.t_first() = (c && C.n_turn() == 0) ? ST.t_new : C.t_first();
+        C.t_last() = c ? ST.t_new : C.t_last();
+        C.n_turn() += c ? 1 : 0;
+        C.n_rej() += r ? 1 : 0;
+    } else {
+        if (a) {
+            if (r2 < C.rmin2()) C.rmin2() = r2;
+            if (counted) {
+                const int nt = ++C.n_turn();
+                if (nt == 1) C.t_first() = ST.t_new;
+                C.t_last() = ST.t_new;
+            }
         }
+        if (r) C.n_rej()++;
     }
-    K.sprev = s;
-    if ((K.flags & kAnyMin) && r2 > P.r_exit2) return 0;
-    if (K.flags & kLast) return 1;
-    if ((long long)K.n_acc >= P.max_steps) return 2;
-    if (K.flags & kNoFailed) K.h = (z < 6.25) ? K.h * (0.8 * z) : 5.0 * K.h;
-    prepare_step(P, K);
-    return -1;
+    K.n_acc = a ? n_acc1 : K.n_acc;
+    K.t = a ? ST.t_new : K.t;
+    K.sprev = a ? s : K.sprev;
+    const bool keep = !live || (r && underflow) || (a && st_acc >= 0);  // ended or idle: h, flags as they are
+    K.h = keep ? h : (a ? h_acc : h_rej);
+    K.flags = keep ? (a ? anymin | (fl & ~kAnyMin) : fl) : (a ? fl_acc : (fl & kAnyMin));
+    return live ? (acc ? st_acc : st_rej) : -1;
 }
 
 // finish_core for the per-thread integrator: on return T holds the state to continue from (or
@@ -443,7 +525,8 @@ template <class Cold>
 __device__ __forceinline__ int finish_attempt(const KParams& P, Traj& T, Cold& C, const Attempt& R)
 {
     bool accepted;
-    const int st = finish_core(P, T.c, C, R.err, R.t_new, R.r2, R.s, accepted);
+    const StepTimes ST = step_times(P, T.c);
+    const int st = finish_core(P, T.c, C, R.err, ST, R.r2, R.s, true, accepted);
     if (accepted) {
 #pragma unroll
         for (int i = 0; i < 6; ++i) {

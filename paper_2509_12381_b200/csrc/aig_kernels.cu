@@ -41,6 +41,24 @@ namespace aig {
 constexpr int kBlock = AIG_BLOCK;             // threads per block of the integrator
 constexpr int kBlocksPerSM = AIG_MIN_BLOCKS;  // resident blocks per SM the register budget is sized for
 
+// Stage timeline (diagnostics): counters[kCntTime + 2 s] = %globaltimer when block 0 of stage s started,
+// counters[kCntTime + 2 s + 1] = latest %globaltimer at which one of its blocks ended (ns).
+constexpr int kCntTime = 32;
+__device__ __forceinline__ unsigned long long global_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void stage_begin(unsigned long long* tl)
+{
+    if (tl && blockIdx.x == 0 && threadIdx.x == 0) tl[0] = global_ns();
+}
+__device__ __forceinline__ void stage_end(unsigned long long* tl)
+{
+    if (tl && (threadIdx.x & 31) == 0) atomicMax(tl + 1, global_ns());
+}
+
 struct OutPtrs {
     double *y_final, *t_final, *lifetime, *angle, *r_min;
     int *n_acc, *n_rej, *n_turn, *status;
@@ -52,6 +70,7 @@ struct OutPtrs {
 // ------------------------------------------------------------------------------------------
 // Cold state of the per-thread integrator: one shared-memory slot per thread, SoA (conflict-free).
 struct ColdShared {
+    static constexpr bool kInRegisters = false;
     __device__ __forceinline__ double& rmin2() { return s_rmin2[threadIdx.x]; }
     __device__ __forceinline__ double& t_first() { return s_tfirst[threadIdx.x]; }
     __device__ __forceinline__ double& t_last() { return s_tlast[threadIdx.x]; }
@@ -165,6 +184,7 @@ struct Sched {
     Ckpt out;
     int budget;
     int tail_iters;
+    unsigned long long* timeline;
 };
 
 template <int TRAP, int BLOCK, int MINB>
@@ -186,6 +206,7 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
     bool live = false;
     bool dry = false;     // warp-uniform: the queue has been seen empty
     bool may_suspend = true;
+    stage_begin(S.timeline);
 
     for (;;) {
         // ---- refill: lanes without a trajectory take the next items of the queue
@@ -231,24 +252,25 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
             }
         }
     }
+    stage_end(S.timeline);
 }
 
 // ---- six lanes per trajectory: continues the slots [*begin, min(*end, cap)) of `in` to their end
 struct SplitSched {
+    unsigned long long* timeline;
     unsigned long long* queue;
     const unsigned long long *begin, *end;
     Ckpt in;
 };
 
-template <int TRAP, int MINB>
-__global__ void __launch_bounds__(32, MINB)
+template <int TRAP, int WARPS, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB)
 integrate_split_kernel(const KParams P, const double* __restrict__ y0, const long long N, const OutPtrs O,
                        const SplitSched S)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const SplitRole R = make_role(P);
-    const int g = lane / kGroupLanes;
     const bool leader = !R.ghost && (lane == R.base);
     const long long first = (long long)*S.begin;
     const long long last = (long long)((*S.end < (unsigned long long)S.in.cap) ? *S.end : (unsigned long long)S.in.cap);
@@ -271,57 +293,69 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
     bool live = false;
     bool dry = (total <= 0);
 
-    for (;;) {
+    // refill: every idle group takes the next slot of the queue (one atomicAdd per warp)
+    auto refill = [&]() {
         const unsigned need = __ballot_sync(FULL, leader && !live);
-        if (need) {
-            if (!dry) {
-                const int cnt = __popc(need);
-                unsigned long long base = 0;
-                if (lane == 0) base = atomicAdd(S.queue, (unsigned long long)cnt);
-                base = __shfl_sync(FULL, base, 0);
-                if (!R.ghost && ((need >> R.base) & 1u)) {
-                    const long long cand = (long long)base + __popc(need & ((1u << R.base) - 1u));
-                    if (cand < total) {
-                        const long long slot = first + cand;
-                        const size_t cap = (size_t)S.in.cap;
-                        const double* d = S.in.d + slot;
-                        Y.xi = d[(0 + R.k) * cap];
-                        Y.xa = d[(3 + R.k) * cap];
-                        Y.vi = d[(6 + R.k) * cap];
-                        Y.va = d[(9 + R.k) * cap];
-                        Y.a1i = d[(12 + R.k) * cap];
-                        Y.a1a = d[(15 + R.k) * cap];
-                        K.t = d[18 * cap];
-                        K.h = d[19 * cap];
-                        K.sprev = d[20 * cap];
-                        C.rmin2_ = d[21 * cap];
-                        C.t_first_ = d[22 * cap];
-                        C.t_last_ = d[23 * cap];
-                        const int* q = S.in.i + slot;
-                        K.n_acc = q[0 * cap];
-                        K.flags = (unsigned)q[1 * cap];
-                        C.n_rej_ = q[2 * cap];
-                        C.n_turn_ = q[3 * cap];
-                        idx = S.in.idx[slot];
-                        live = true;
-                    }
-                }
-                if ((long long)base + cnt >= total) dry = true;
+        if (need == 0u || dry) return;
+        const int cnt = __popc(need);
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(S.queue, (unsigned long long)cnt);
+        base = __shfl_sync(FULL, base, 0);
+        if (!R.ghost && ((need >> R.base) & 1u)) {
+            const long long cand = (long long)base + __popc(need & ((1u << R.base) - 1u));
+            if (cand < total) {
+                const long long slot = first + cand;
+                const size_t cap = (size_t)S.in.cap;
+                const double* d = S.in.d + slot;
+                Y.xi = d[(0 + R.k) * cap];
+                Y.xa = d[(3 + R.k) * cap];
+                Y.vi = d[(6 + R.k) * cap];
+                Y.va = d[(9 + R.k) * cap];
+                Y.a1i = d[(12 + R.k) * cap];
+                Y.a1a = d[(15 + R.k) * cap];
+                K.t = d[18 * cap];
+                K.h = d[19 * cap];
+                K.sprev = d[20 * cap];
+                C.rmin2_ = d[21 * cap];
+                C.t_first_ = d[22 * cap];
+                C.t_last_ = d[23 * cap];
+                const int* q = S.in.i + slot;
+                K.n_acc = q[0 * cap];
+                K.flags = (unsigned)q[1 * cap];
+                C.n_rej_ = q[2 * cap];
+                C.n_turn_ = q[3 * cap];
+                idx = S.in.idx[slot];
+                live = true;
             }
-            if (!__any_sync(FULL, live)) break;
         }
-        // ---- one attempted step for every group (all lanes together: full-mask shuffles inside)
+        if ((long long)base + cnt >= total) dry = true;
+    };
+
+    stage_begin(S.timeline);
+    refill();
+    if (!__any_sync(FULL, live)) {
+        stage_end(S.timeline);
+        return;
+    }
+    for (;;) {
+        // ---- one attempted step for every group (all lanes together: full-mask shuffles inside);
+        //      straight-line code up to the vote below
         SplitAttempt A;
-        split_attempt<TRAP>(P, R, K, Y, A);
-        int st = -1;
-        if (live) {
-            bool accepted;
-            st = finish_core(P, K, C, A.err, A.t_new, A.r2, A.s, accepted);
-            if (accepted) Y = A.Y;
-        }
-        const unsigned fin = __ballot_sync(FULL, live && st >= 0);
-        if (live && st >= 0) {
-            // a8: lanes e = 0 store component k of the final state, the group's first lane the scalars
+        StepTimes ST;
+        split_attempt<TRAP>(P, R, K, Y, A, ST);
+        bool accepted;
+        const int st = finish_core(P, K, C, A.err, ST, A.r2, A.s, live, accepted);
+        Y.xi = accepted ? A.Y.xi : Y.xi;
+        Y.vi = accepted ? A.Y.vi : Y.vi;
+        Y.a1i = accepted ? A.Y.a1i : Y.a1i;
+        Y.xa = accepted ? A.Y.xa : Y.xa;
+        Y.va = accepted ? A.Y.va : Y.va;
+        Y.a1a = accepted ? A.Y.a1a : Y.a1a;
+        const unsigned fin = __ballot_sync(FULL, st >= 0);
+        if (fin == 0u) continue;
+        // ---- a8 (rare): lanes e = 0 store component k of the final state, the group's first lane
+        //      the scalars; then the group takes the next slot
+        if (st >= 0) {
             const double v1[3] = {__shfl_sync(fin, Y.va, R.base), __shfl_sync(fin, Y.va, R.base + 2),
                                   __shfl_sync(fin, Y.va, R.base + 4)};
             if (R.e == 0) {
@@ -335,7 +369,7 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
                 store_scalars(idx, K, C, st, v0, v1, O);
             }
             live = false;
-            // back to benign state: the dead group keeps stepping until it is refilled or the warp ends
+            // benign state again: the idle group keeps stepping (untouched by finish_core) until it is refilled
             Y.xi = 1.0 + R.k;
             Y.xa = 101.0 + 2.0 * R.k;
             Y.vi = Y.va = Y.a1i = Y.a1a = 0.0;
@@ -343,8 +377,10 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
             K.h = 1.0;
             K.flags = 0u;
         }
-        (void)g;
+        refill();
+        if (!__any_sync(FULL, live)) break;
     }
+    stage_end(S.timeline);
 }
 
 // ---- work-queue order: trajectories that can reach short range first --------------------------
@@ -602,16 +638,17 @@ int trap_mode(const aig_params* p, double t_max)
 KParams make_kparams(const aig_params* p, double t_max, double rtol, double atol)
 {
     KParams K;
-    K.inv_mi = 1.0 / p->m_ion;
-    K.inv_ma = 1.0 / p->m_atom;
-    K.c4x4 = 4.0 * p->C4;
-    K.c8x8 = 8.0 * p->C8;
+    K.g4i = -4.0 * p->C4 / p->m_ion;
+    K.g8i = 8.0 * p->C8 / p->m_ion;
+    K.g4a = 4.0 * p->C4 / p->m_atom;
+    K.g8a = -8.0 * p->C8 / p->m_atom;
     const double w2 = p->omega_rf * p->omega_rf;
     for (int k = 0; k < 3; ++k) {
         K.wa[k] = p->a[k] * w2 / 4.0;
         K.wb[k] = p->q[k] * w2 / 2.0;
     }
     K.omega = p->omega_rf;
+    K.half_omega = 0.5 * p->omega_rf;
     K.t0 = p->t0;
     K.t_max = t_max;
     K.hmax = 0.1 * (t_max - p->t0);
@@ -633,18 +670,20 @@ bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(pt
 //   bulk A    per-thread integrator over the candidates; what outlives `budget` accepted steps, or
 //             is still running `tail_iters` iterations after the queue ran dry, is suspended
 //   bulk B    per-thread integrator over the rest (same rules, same slot buffer, appended)
-//   split A   six-lane integrator over the slots bulk A wrote, on a second (high-priority) stream
-//             so that it runs BESIDE bulk B: the longest trajectories (10^2..10^3 x the mean number
-//             of steps, all among the candidates) start their long sequential run early
-//   split B   six-lane integrator over the slots bulk B wrote; then the streams join.
+//   split A   six-lane integrator over the slots bulk A wrote, BESIDE bulk B: the longest trajectories
+//             (10^2..10^3 x the mean number of steps, all among the candidates) start their long
+//             sequential run early.  It takes `split_sms` SMs for itself (one 4-warp block per SM that
+//             asks for the whole shared memory, so that no bulk block can share its FP64 pipes);
+//             bulk B, on a second stream, is sized for the remaining SMs.
+//   split B   six-lane integrator over the slots bulk B wrote (second stream); then the streams join.
 // No kernel ever waits for another one on the device (no polling): every dependency is a stream
 // order or an event.
 constexpr long long kMinSlots = 65536;
 
 struct SchedConfig {
-    int tail_iters = 64;      // iterations a warp keeps stepping after the queue ran dry
+    int tail_iters = 256;     // iterations a warp keeps stepping after the queue ran dry
     int budget = 2048;        // accepted steps after which the per-thread integrator hands a trajectory over
-    int split_grid_a = 2;     // split A: one-warp blocks per SM (it shares the GPU with bulk B)
+    int split_sms = 32;       // SMs that split A takes for itself (one 4-warp block each); bulk B runs on the others
     int split_grid_b = 8;     // split B: one-warp blocks per SM (it has the GPU to itself)
     int plan = 1;             // 0: natural order, one bulk launch
     double kappa = 1.25;      // candidates: b < kappa * Langevin radius
@@ -653,14 +692,14 @@ struct SchedConfig {
 const SchedConfig& sched_config()
 {
     static const SchedConfig cfg = [] {
-        SchedConfig c;  // AIG_SCHED="tail_iters,budget,split_grid_a,split_grid_b,plan,kappa" overrides (tuning aid)
+        SchedConfig c;  // AIG_SCHED="tail_iters,budget,split_sms,split_grid_b,plan,kappa" overrides (tuning aid)
         if (const char* e = std::getenv("AIG_SCHED")) {
-            int a = c.tail_iters, b = c.budget, ga = c.split_grid_a, gb = c.split_grid_b, pl = c.plan;
+            int a = c.tail_iters, b = c.budget, ga = c.split_sms, gb = c.split_grid_b, pl = c.plan;
             double kp = c.kappa;
             const int got = std::sscanf(e, "%d,%d,%d,%d,%d,%lf", &a, &b, &ga, &gb, &pl, &kp);
             if (got >= 1 && a >= 0) c.tail_iters = a;
             if (got >= 2 && b >= 1) c.budget = b;
-            if (got >= 3 && ga >= 1) c.split_grid_a = ga;
+            if (got >= 3 && ga >= 1) c.split_sms = ga;
             if (got >= 4 && gb >= 1) c.split_grid_b = gb;
             if (got >= 5) c.plan = pl;
             if (got >= 6 && kp >= 0.0) c.kappa = kp;
@@ -715,7 +754,7 @@ int bulk_capacity(int* blocks_per_sm, int* sm_count)
     return AIG_OK;
 }
 
-// second stream (high priority) and the fork / join events of the schedule, one set per device
+// second stream and the fork / join events of the schedule, one set per device
 struct SideStream {
     cudaStream_t stream = nullptr;
     cudaEvent_t fork = nullptr, join = nullptr;
@@ -733,7 +772,7 @@ SideStream* side_stream()
     if (!s.ok) {
         int lo = 0, hi = 0;
         if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return nullptr;
-        if (cudaStreamCreateWithPriority(&s.stream, cudaStreamNonBlocking, hi) != cudaSuccess) return nullptr;
+        if (cudaStreamCreateWithPriority(&s.stream, cudaStreamNonBlocking, lo) != cudaSuccess) return nullptr;
         if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
         if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
         s.ok = true;
@@ -742,6 +781,7 @@ SideStream* side_stream()
 }
 
 constexpr int kSplitMinBlocks = 8;  // register cap of the split kernel: 65536 / (8 x 32) = 256
+constexpr int kSplitWarps = 4;      // warps per block of the SM-owning variant: one per scheduler, a warp never waits for another
 
 template <int TRAP>
 int launch_integrate(const aig_params* p, const KParams& K, const double* y0, long long N, const OutPtrs& O,
@@ -771,8 +811,10 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     S.out = slots;
     S.budget = cfg.budget;
     S.tail_iters = cfg.tail_iters;
+    S.timeline = counters + kCntTime + 2;
     SplitSched T;
     T.in = slots;
+    T.timeline = counters + kCntTime + 4;
     const unsigned split_b = (unsigned)std::min<long long>((long long)cfg.split_grid_b * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
 
     if (!plan) {
@@ -785,7 +827,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         T.queue = counters + kCntQueueSA;
         T.begin = counters + kCntZero;
         T.end = counters + kCntSlots;
-        integrate_split_kernel<TRAP, kSplitMinBlocks><<<split_b, 32, 0, st>>>(K, y0, N, O, T);
+        integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_b, 32, 0, st>>>(K, y0, N, O, T);
         g_kernel_launches++;
         return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
     }
@@ -803,27 +845,37 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     snapshot_kernel<<<1, 1, 0, st>>>(counters, kCntSlotsA, kCntSlots, (unsigned long long)cap);
     g_kernel_launches += 2;
     if (cudaEventRecord(side->fork, st) != cudaSuccess) return AIG_ERR_CUDA;
-    // split A beside bulk B
-    if (cudaStreamWaitEvent(side->stream, side->fork, 0) != cudaSuccess) return AIG_ERR_CUDA;
+    // split A on this stream, right behind bulk A: one block per SM it owns (the dynamic shared
+    // memory request leaves no room for a bulk block beside it)
+    int dev = 0, smem_optin = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        return AIG_ERR_CUDA;
+    if (cudaFuncSetAttribute(integrate_split_kernel<TRAP, kSplitWarps, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             smem_optin) != cudaSuccess)
+        return AIG_ERR_CUDA;
+    const long long own = std::max<long long>(1, std::min<long long>(cfg.split_sms, sms / 2));
     T.queue = counters + kCntQueueSA;
     T.begin = counters + kCntZero;
     T.end = counters + kCntSlotsA;
-    const unsigned split_a = (unsigned)std::min<long long>((long long)cfg.split_grid_a * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
-    integrate_split_kernel<TRAP, kSplitMinBlocks><<<split_a, 32, 0, side->stream>>>(K, y0, N, O, T);
+    integrate_split_kernel<TRAP, kSplitWarps, 1><<<(unsigned)own, 32 * kSplitWarps, (size_t)smem_optin, st>>>(K, y0, N, O, T);
     g_kernel_launches++;
-    if (cudaEventRecord(side->join, side->stream) != cudaSuccess) return AIG_ERR_CUDA;
-    // bulk B: order[n_front, N)
+    // second stream: bulk B over order[n_front, N) on the other SMs, then split B over its slots
+    if (cudaStreamWaitEvent(side->stream, side->fork, 0) != cudaSuccess) return AIG_ERR_CUDA;
+    S.timeline = counters + kCntTime + 6;
     S.queue = counters + kCntQueueB;
     S.begin = counters + kCntFront;
     S.end = counters + kCntN;
-    integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
-    snapshot_kernel<<<1, 1, 0, st>>>(counters, kCntSlotsB, kCntSlots, (unsigned long long)cap);
-    // split B: slots [slotsA, slotsB)
+    const long long blocks_b = std::max<long long>(1, std::min<long long>(blocks, (long long)bps * (sms - own)));
+    integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks_b, kBlock, 0, side->stream>>>(K, y0, N, O, S);
+    snapshot_kernel<<<1, 1, 0, side->stream>>>(counters, kCntSlotsB, kCntSlots, (unsigned long long)cap);
+    T.timeline = counters + kCntTime + 8;
     T.queue = counters + kCntQueueSB;
     T.begin = counters + kCntSlotsA;
     T.end = counters + kCntSlotsB;
-    integrate_split_kernel<TRAP, kSplitMinBlocks><<<split_b, 32, 0, st>>>(K, y0, N, O, T);
+    integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_b, 32, 0, side->stream>>>(K, y0, N, O, T);
     g_kernel_launches += 3;
+    if (cudaEventRecord(side->join, side->stream) != cudaSuccess) return AIG_ERR_CUDA;
     if (cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) return AIG_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }

@@ -78,14 +78,20 @@ struct SplitAttempt {
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 __device__ __forceinline__ double shfl_xor_d(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 
-// One level: position of my stage from the accelerations known so far, the force there, and the
-// exchange with the partner lane (k, 1 - e).  NT = number of stage accelerations in the sum.
-template <int TRAP, int LEV>
-__device__ __forceinline__ void split_level(const KParams& P, const SplitRole& R, const SplitState& Y, double h,
-                                            double h2, double mycos, double (&Ai)[7], double (&Aa)[7],
-                                            double& xsi, double& xsa, double& r2)
+// One level in two halves, in the order the dependent chain runs:
+//   level_open : position of my stage from the accelerations known so far, d_k^2, and the three
+//                shuffles that gather |d|^2 over k are issued;
+//   level_close: 1/r^2 -> force factors -> accelerations -> exchange with the partner lane (k, 1 - e).
+// Whatever the caller puts between the two (the cos of this step, the partial step-end sums)
+// runs inside the shuffle latency.
+struct LevelOpen {
+    double xsi, xsa, d;
+    double s0, s1, s2;
+};
+template <int LEV>
+__device__ __forceinline__ void level_open(const SplitRole& R, const SplitState& Y, double h, double h2,
+                                           const double (&Ai)[7], const double (&Aa)[7], LevelOpen& L)
 {
-    const double cs = (TRAP == TRAP_RF || TRAP == TRAP_RF_BIG) ? shfl_d(mycos, R.base + 2 * LEV + R.e) : 1.0;
     const double hc = h * R.cC[LEV];
     const double bi = fma(hc, Y.vi, Y.xi);
     const double ba = fma(hc, Y.va, Y.xa);
@@ -110,66 +116,84 @@ __device__ __forceinline__ void split_level(const KParams& P, const SplitRole& R
             acca = fma(R.cA2[l], Aa[l], acca);
         }
     }
-    xsi = fma(h2, acci, bi);
-    xsa = fma(h2, acca, ba);
-    const double d = xsi - xsa;
-    const double sq = d * d;
+    L.xsi = fma(h2, acci, bi);
+    L.xsa = fma(h2, acca, ba);
+    L.d = L.xsi - L.xsa;
+    const double sq = L.d * L.d;
     const int src = R.base + R.e;
-    r2 = sum3(shfl_d(sq, src), shfl_d(sq, src + 2), shfl_d(sq, src + 4));
+    L.s0 = shfl_d(sq, src);
+    L.s1 = shfl_d(sq, src + 2);
+    L.s2 = shfl_d(sq, src + 4);
+}
+template <int TRAP, int LEV>
+__device__ __forceinline__ double level_close(const KParams& P, const SplitRole& R, const LevelOpen& L,
+                                              double mycos, double (&Ai)[7], double (&Aa)[7])
+{
+    double trap = 0.0;
+    if (TRAP != TRAP_NONE) {
+        const double cs = (TRAP == TRAP_STATIC) ? 1.0 : shfl_d(mycos, R.base + 2 * LEV + R.e);
+        trap = -(trap_w<TRAP>(R.wa, R.wb, cs) * L.xsi);
+    }
+    const double r2 = sum3(L.s0, L.s1, L.s2);
     double gi, ga;
     force_factors(P, r2, gi, ga);
-    const double myAa = ga * d;
-    const double myAi = (TRAP == TRAP_NONE) ? gi * d : fma(-trap_w<TRAP>(R.wa, R.wb, cs), xsi, gi * d);
+    const double myAa = ga * L.d;
+    const double myAi = (TRAP == TRAP_NONE) ? gi * L.d : fma(gi, L.d, trap);
     const double pAi = shfl_xor_d(myAi, 1);
     const double pAa = shfl_xor_d(myAa, 1);
     Ai[2 * LEV + 1] = R.e ? pAi : myAi;
     Ai[2 * LEV + 2] = R.e ? myAi : pAi;
     Aa[2 * LEV + 1] = R.e ? pAa : myAa;
     Aa[2 * LEV + 2] = R.e ? myAa : pAa;
+    return r2;
 }
 
 // One attempted step of size K.h from (K.t, y) for every group of the warp.  All 32 lanes call it
 // together (full-mask shuffles); lanes without a trajectory run it on benign dummy state.
 template <int TRAP>
 __device__ __forceinline__ void split_attempt(const KParams& P, const SplitRole& R, const Core& K,
-                                              const SplitState& Y, SplitAttempt& out)
+                                              const SplitState& Y, SplitAttempt& out, StepTimes& ST)
 {
     const double h = K.h;
     const double h2 = h * h;
-    const double t_new = (K.flags & kLast) ? P.t_max : K.t + h;
-    double mycos = 1.0;
-    if (TRAP == TRAP_RF || TRAP == TRAP_RF_BIG) mycos = trap_cos<TRAP>(P, R.cos_end ? t_new : fma(R.cCos, h, K.t));
+    ST = step_times(P, K);
+    // pin the (t, h)-only quantities here: the compiler would otherwise sink them to their use behind
+    // the error estimate, onto the step's dependent chain
+    asm volatile("" : "+d"(ST.hmin_cur), "+d"(ST.hmin_new), "+d"(ST.rem_new));
     double Ai[7], Aa[7];
     Ai[0] = Y.a1i;
     Aa[0] = Y.a1a;
-    double xsi, xsa, r2;
-    split_level<TRAP, 0>(P, R, Y, h, h2, mycos, Ai, Aa, xsi, xsa, r2);
-    split_level<TRAP, 1>(P, R, Y, h, h2, mycos, Ai, Aa, xsi, xsa, r2);
-    split_level<TRAP, 2>(P, R, Y, h, h2, mycos, Ai, Aa, xsi, xsa, r2);
+    LevelOpen L;
+    level_open<0>(R, Y, h, h2, Ai, Aa, L);
+    // the cos of my stage time, inside the first level's shuffle and reciprocal latency
+    double mycos = 1.0;
+    if (TRAP == TRAP_RF || TRAP == TRAP_RF_BIG) mycos = trap_cos<TRAP>(P, R.cos_end ? ST.t_new : fma(R.cCos, h, K.t));
+    level_close<TRAP, 0>(P, R, L, mycos, Ai, Aa);
+    level_open<1>(R, Y, h, h2, Ai, Aa, L);
+    level_close<TRAP, 1>(P, R, L, mycos, Ai, Aa);
+    level_open<2>(R, Y, h, h2, Ai, Aa, L);
+    // everything of the step end that does not need stages 6 and 7 goes inside the last level
+    StepEndPart Si, Sa;
+    step_end_begin(P, Y.xi, Y.vi, Ai, Si);
+    step_end_begin(P, Y.xa, Y.va, Aa, Sa);
+    const double r2 = level_close<TRAP, 2>(P, R, L, mycos, Ai, Aa);
+    const double xsi = L.xsi, xsa = L.xsa;
     // stage 7 (lanes e = 1) is the 5th-order solution: hand x_new and |d|^2 there to the partner
     const double pxi = shfl_xor_d(xsi, 1), pxa = shfl_xor_d(xsa, 1), pr2 = shfl_xor_d(r2, 1);
     const double xni = R.e ? xsi : pxi, xna = R.e ? xsa : pxa;
     out.r2 = R.e ? r2 : pr2;
     // step end of component k of both particles (replicated on both lanes of the pair)
     Ratio cvi, cxi, cva, cxa;
-    const double vni = step_end_component(P, h, Y.xi, xni, Y.vi, Ai, cvi, cxi);
-    const double vna = step_end_component(P, h, Y.xa, xna, Y.va, Aa, cva, cxa);
-    const Ratio ai = ratio_max(cvi, cxi), aa = ratio_max(cva, cxa);
-    const int src = R.base + R.e;
-    Ratio gi3[3], ga3[3];
-#pragma unroll
-    for (int m = 0; m < 3; ++m) {
-        gi3[m].n = shfl_d(ai.n, src + 2 * m);
-        gi3[m].d = shfl_d(ai.d, src + 2 * m);
-        ga3[m].n = shfl_d(aa.n, src + 2 * m);
-        ga3[m].d = shfl_d(aa.d, src + 2 * m);
-    }
-    const Ratio ion = ratio_max(ratio_max(gi3[0], gi3[1]), gi3[2]);
-    const Ratio atom = ratio_max(ratio_max(ga3[0], ga3[1]), ga3[2]);
+    const double vni = step_end_finish(Si, h, xni, Y.vi, Ai[5], Ai[6], cvi, cxi);
+    const double vna = step_end_finish(Sa, h, xna, Y.va, Aa[5], Aa[6], cva, cxa);
+    const double q = axis_quotient(cvi, cxi, cva, cxa);
     const double p = (xna - xni) * (vna - vni);
-    out.s = sum3(shfl_d(p, src), shfl_d(p, src + 2), shfl_d(p, src + 4));
-    out.t_new = t_new;
-    out.err = error_estimate(h, ion, atom, out.r2, out.s);
+    const int src = R.base + R.e;
+    const double q0 = shfl_d(q, src), q1 = shfl_d(q, src + 2), q2 = shfl_d(q, src + 4);
+    const double p0 = shfl_d(p, src), p1 = shfl_d(p, src + 2), p2 = shfl_d(p, src + 4);
+    out.s = sum3(p0, p1, p2);
+    out.t_new = ST.t_new;
+    out.err = error_estimate(h, q0, q1, q2, out.r2, out.s);
     out.Y.xi = xni;
     out.Y.vi = vni;
     out.Y.a1i = Ai[6];
