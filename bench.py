@@ -233,6 +233,13 @@ def run_ours(args) -> int:
     ms_total = max_over_ranks(e_begin.elapsed_time(e_end))
     ms_int = max_over_ranks(float(np.mean([a.elapsed_time(b) for a, b in kev])))
 
+    # stage timeline of the last aig_integrate call (ns %globaltimer stamps the kernels leave in the workspace)
+    tl = ws[:512].view(torch.int64)[32:42].cpu().numpy().astype(np.float64)
+    t_first = min((x for x in tl if x > 0), default=0.0)
+    stages_ms = {name: [round((tl[2 * i] - t_first) / 1e6, 3), round((tl[2 * i + 1] - t_first) / 1e6, 3)]
+                 for i, name in enumerate(("plan", "bulk_candidates", "split_beside_bulk", "bulk_rest", "split_rest"))
+                 if tl[2 * i] > 0}
+
     n_acc = int(out["n_acc"].sum(dtype=torch.int64).item())
     n_rej = int(out["n_rej"].sum(dtype=torch.int64).item())
     totals = aig.hist_to_numpy(hist)["totals"] if world == 1 else None
@@ -327,7 +334,9 @@ def run_ours(args) -> int:
             "ms_integrate_kernel": ms_int,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL / 1e12, "unit": "TFLOP/s",
                          "frac": achieved * 1e12 / FP64_PEAK_NOMINAL, "traffic": INTEGRATE_DRAM_TRAFFIC_BYTES,
-                         "kernel": "integrate_kernel<TRAP_RF>",
+                         "kernel": "aig_integrate: plan_kernel + integrate_kernel<TRAP_RF> x2 + integrate_split_kernel<TRAP_RF> x2 "
+                                   "(overlapped on two streams), timed as one region on the launching stream",
+                         "stages_ms": stages_ms,
                          "flops_per_attempted_step": FLOPS_PER_ATTEMPT,
                          "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md)",
                          "peak_measured_dfma": peak_meas / 1e12,

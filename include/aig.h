@@ -102,7 +102,9 @@ typedef struct aig_hist {
     uint64_t *angle, *lifetime, *n_turn, *status, *totals;
 } aig_hist;
 
-/* Bytes of DEVICE scratch aig_integrate needs for N trajectories (work-queue counter). */
+/* Bytes of DEVICE scratch aig_integrate needs for N trajectories: 64 uint64 counters (work
+ * queues, slot counts, a stage timeline), the work-queue order (one int64 per trajectory) and
+ * min(N, max(65536, N/4)) checkpoint slots of 216 B for suspended trajectories. */
 size_t aig_workspace_bytes(int64_t N);
 
 /* Integrate N trajectories from t0 to the first stop (exit radius, t_max, max_steps).
@@ -111,8 +113,12 @@ size_t aig_workspace_bytes(int64_t N);
  *   t_max     end of the time span (> p->t0);  rtol > 0, atol >= 0: ode45 tolerances
  *   out       HOST struct of DEVICE pointers
  *   workspace DEVICE scratch of >= aig_workspace_bytes(N) bytes, 8-byte aligned
- * One persistent kernel: each thread integrates one trajectory at a time and refills from
- * a global work queue when it finishes (PAPER.md:186-202 runs one array element per thread). */
+ * Persistent kernels: each thread integrates one trajectory at a time and refills from a
+ * global work queue when it finishes (PAPER.md:186-202 runs one array element per thread);
+ * trajectories that outlive a step budget (long-lived complexes) are continued by a second
+ * kernel that spreads one trajectory over six lanes, on SMs of its own beside the bulk (an
+ * internal second stream, joined to `cuda_stream` before the call's work is complete from the
+ * caller's point of view).  Every result is bit-identical whichever kernel produced it. */
 int aig_integrate(const aig_params *p, const double *y0, int64_t N, double t_max, double rtol,
                   double atol, const aig_out *out, void *workspace, void *cuda_stream);
 
@@ -155,6 +161,20 @@ int aig_kernel_info(int *sm_count, int *blocks_per_sm, int *threads_per_block,
  * step-once kernels; the FP64 probe is not counted).  bench.py reports the difference over its
  * timed region as "gpu_launches". */
 uint64_t aig_kernel_launches(void);
+
+/* Test / tuning hook: the schedule aig_integrate uses from now on in this process.
+ *   tail_iters  iterations a warp of the per-thread integrator keeps stepping after its work
+ *               queue ran dry before it hands its trajectories over (default 256)
+ *   budget      accepted steps after which a trajectory is handed to the six-lane integrator
+ *               (default 2048)
+ *   split_sms   SMs the six-lane integrator owns while the second part of the bulk runs (32)
+ *   split_grid  one-warp blocks per SM of the final six-lane pass (8)
+ *   plan        0: natural order, one bulk pass; 1: capture candidates first (default)
+ *   kappa       candidates are trajectories with impact parameter < kappa Langevin radii (1.25)
+ * Scheduling never changes a result (tests/test_gpu_parity.py::test_schedule_invariance).
+ * Returns AIG_ERR_PARAM for out-of-range values.  Not thread-safe against concurrent
+ * aig_integrate calls that should see the old schedule. */
+int aig_set_schedule(int tail_iters, int budget, int split_sms, int split_grid, int plan, double kappa);
 
 const char *aig_strerror(int code);
 int aig_version(void);

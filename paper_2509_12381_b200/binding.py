@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libaig.so")
 _lib = None
 
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
-           "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_strerror", "aig_version"]
+           "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_set_schedule", "aig_strerror",
+           "aig_version"]
 
 
 class AigError(RuntimeError):
@@ -237,6 +238,15 @@ def kernel_info() -> dict:
     _check(lib().aig_kernel_info(*[C.byref(x) for x in v]), "aig_kernel_info")
     keys = ("sm_count", "blocks_per_sm", "threads_per_block", "regs_per_thread", "local_bytes_per_thread")
     return dict(zip(keys, [x.value for x in v]))
+
+
+def set_schedule(tail_iters=256, budget=2048, split_sms=32, split_grid=8, plan=1, kappa=1.25) -> None:
+    """Test / tuning hook (include/aig.h: aig_set_schedule); never changes a result."""
+    L = lib()
+    L.aig_set_schedule.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double]
+    L.aig_set_schedule.restype = C.c_int
+    _check(L.aig_set_schedule(int(tail_iters), int(budget), int(split_sms), int(split_grid), int(plan), float(kappa)),
+           "aig_set_schedule")
 
 
 def kernel_launches() -> int:

@@ -305,8 +305,7 @@ __device__ __forceinline__ double error_estimate(double h, double q0, double q1,
 {
     double err = h * dmax(dmax(q0, q1), q2);
     // a non-finite state or force makes the estimate NaN (it must reject, like the oracle's NaN)
-    const bool finite_ok = (r2 > 0.0) && (r2 < 1.0e300) && (fabs(s) < 1.0e300) && (q0 == q0) && (q1 == q1) &&
-                           (q2 == q2);
+    const bool finite_ok = (r2 > 0.0) & (r2 < 1.0e300) & (fabs(s) < 1.0e300) & (q0 == q0) & (q1 == q1) & (q2 == q2);
     if (!finite_ok) err = __longlong_as_double(0x7ff8000000000000LL);
     return err;
 }
@@ -465,18 +464,18 @@ __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, d
     //      the last-step test.
     const double h08 = 0.8 * h;
     const double h_alt = nofailed ? 5.0 * h : h;  // growth limit 5, or h kept after a failure
-    const bool radial_min = (K.sprev < 0.0) && (s >= 0.0);
+    const bool radial_min = (K.sprev < 0.0) & (s >= 0.0);
     const unsigned anymin = (fl & kAnyMin) | (radial_min ? kAnyMin : 0u);
-    const bool counted = radial_min && (r2 < P.r_turn2);
+    const bool counted = radial_min & (r2 < P.r_turn2);
     const int n_acc1 = K.n_acc + 1;
-    const bool stop_exit = (anymin != 0u) && (r2 > P.r_exit2);
+    const bool stop_exit = (anymin != 0u) & (r2 > P.r_exit2);
     const bool stop_last = (fl & kLast) != 0u;
     const bool stop_max = (long long)n_acc1 >= P.max_steps;
     const int st_acc = stop_exit ? 0 : (stop_last ? 1 : (stop_max ? 2 : -1));
     // h_cl = min(hmax, max(hmin_new, h_grow)) and last_new = (1.1 h_cl >= rem_new), with the three
     // comparisons of h_grow side by side instead of one behind the other (exact selects, same values)
-    const double h_grow = (nofailed && z < 6.25) ? h08 * z : h_alt;
-    const bool over = (h_grow > P.hmax) || (ST.hmin_new > P.hmax);
+    const double h_grow = (nofailed & (z < 6.25)) ? h08 * z : h_alt;
+    const bool over = (h_grow > P.hmax) | (ST.hmin_new > P.hmax);
     const bool under = (h_grow < ST.hmin_new);
     const bool last_grow = (1.1 * h_grow >= ST.rem_new);
     const bool last_max = (1.1 * P.hmax >= ST.rem_new), last_min = (1.1 * ST.hmin_new >= ST.rem_new);
@@ -490,12 +489,12 @@ __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, d
     const double h_rej = dmax(h * (nofailed ? fac_z : 0.5), ST.hmin_cur);
     const int st_rej = underflow ? 3 : -1;
     // ---- commit
-    const bool a = live && acc, r = live && !acc;
+    const bool a = live & acc, r = live & !acc;
     accepted = a;
     if (Cold::kInRegisters) {
-        C.rmin2() = (a && r2 < C.rmin2()) ? r2 : C.rmin2();
-        const bool c = a && counted;
-        C.t_first() = (c && C.n_turn() == 0) ? ST.t_new : C.t_first();
+        C.rmin2() = (a & (r2 < C.rmin2())) ? r2 : C.rmin2();
+        const bool c = a & counted;
+        C.t_first() = (c & (C.n_turn() == 0)) ? ST.t_new : C.t_first();
         C.t_last() = c ? ST.t_new : C.t_last();
         C.n_turn() += c ? 1 : 0;
         C.n_rej() += r ? 1 : 0;
@@ -513,7 +512,7 @@ __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, d
     K.n_acc = a ? n_acc1 : K.n_acc;
     K.t = a ? ST.t_new : K.t;
     K.sprev = a ? s : K.sprev;
-    const bool keep = !live || (r && underflow) || (a && st_acc >= 0);  // ended or idle: h, flags as they are
+    const bool keep = !live | (r & underflow) | (a & (st_acc >= 0));  // ended or idle: h, flags as they are
     K.h = keep ? h : (a ? h_acc : h_rej);
     K.flags = keep ? (a ? anymin | (fl & ~kAnyMin) : fl) : (a ? fl_acc : (fl & kAnyMin));
     return live ? (acc ? st_acc : st_rej) : -1;

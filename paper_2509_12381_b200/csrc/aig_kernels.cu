@@ -689,10 +689,17 @@ struct SchedConfig {
     double kappa = 1.25;      // candidates: b < kappa * Langevin radius
 };
 
-const SchedConfig& sched_config()
+std::mutex g_sched_mutex;
+SchedConfig g_sched;          // guarded by g_sched_mutex
+bool g_sched_init = false;
+
+// the schedule in force: defaults, overridden once by AIG_SCHED="tail_iters,budget,split_sms,
+// split_grid_b,plan,kappa" (tuning aid) and at any time by aig_set_schedule()
+SchedConfig sched_config()
 {
-    static const SchedConfig cfg = [] {
-        SchedConfig c;  // AIG_SCHED="tail_iters,budget,split_sms,split_grid_b,plan,kappa" overrides (tuning aid)
+    std::lock_guard<std::mutex> lock(g_sched_mutex);
+    if (!g_sched_init) {
+        SchedConfig c;
         if (const char* e = std::getenv("AIG_SCHED")) {
             int a = c.tail_iters, b = c.budget, ga = c.split_sms, gb = c.split_grid_b, pl = c.plan;
             double kp = c.kappa;
@@ -704,9 +711,10 @@ const SchedConfig& sched_config()
             if (got >= 5) c.plan = pl;
             if (got >= 6 && kp >= 0.0) c.kappa = kp;
         }
-        return c;
-    }();
-    return cfg;
+        g_sched = c;
+        g_sched_init = true;
+    }
+    return g_sched;
 }
 
 long long slot_capacity(long long N) { return std::min(N < 1 ? 1 : N, std::max(kMinSlots, N / 4)); }
@@ -787,7 +795,7 @@ template <int TRAP>
 int launch_integrate(const aig_params* p, const KParams& K, const double* y0, long long N, const OutPtrs& O,
                      void* workspace, cudaStream_t st)
 {
-    const SchedConfig& cfg = sched_config();
+    const SchedConfig cfg = sched_config();
     const long long cap = slot_capacity(N);
     unsigned long long* counters = static_cast<unsigned long long*>(workspace);
     long long* order = reinterpret_cast<long long*>(static_cast<unsigned char*>(workspace) + kCounterBytes);
@@ -887,6 +895,20 @@ extern "C" {
 int aig_version(void) { return AIG_VERSION; }
 
 uint64_t aig_kernel_launches(void) { return g_kernel_launches.load(); }
+
+int aig_set_schedule(int tail_iters, int budget, int split_sms, int split_grid, int plan, double kappa)
+{
+    if (tail_iters < 0 || budget < 1 || split_sms < 1 || split_grid < 1 || !(kappa >= 0.0)) return AIG_ERR_PARAM;
+    (void)sched_config();  // settle the defaults / environment first
+    std::lock_guard<std::mutex> lock(g_sched_mutex);
+    g_sched.tail_iters = tail_iters;
+    g_sched.budget = budget;
+    g_sched.split_sms = split_sms;
+    g_sched.split_grid_b = split_grid;
+    g_sched.plan = plan;
+    g_sched.kappa = kappa;
+    return AIG_OK;
+}
 
 const char* aig_strerror(int code)
 {

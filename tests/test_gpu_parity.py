@@ -199,6 +199,35 @@ def test_config0_trajectories(aig):
     assert abs(int(g["complex_flag"].sum()) - int(o["complex_flag"].sum())) <= 3
 
 
+def test_schedule_invariance(aig):
+    """Where a trajectory is integrated (per-thread kernel, six-lane kernel, before or after a
+    suspension, queued first or last) never changes its result: every output array is bit-identical
+    under very different schedules (include/aig.h: aig_set_schedule)."""
+    w = inputs.config(2).replace(N=8192 + 37)   # several blocks of both kernels and a ragged tail
+    y0 = inputs.generate_y0(w)
+    schedules = [dict(),                                              # defaults
+                 dict(plan=0, budget=10 ** 9, tail_iters=10 ** 9),    # everything in the per-thread kernel
+                 dict(plan=0, budget=1, tail_iters=0),                # everything handed to the six-lane kernel
+                 dict(plan=1, budget=40, tail_iters=3, split_sms=5, split_grid=2, kappa=2.0),
+                 dict(plan=1, budget=300, tail_iters=50, split_sms=70, split_grid=1, kappa=0.5)]
+    ref = None
+    try:
+        for kw in schedules:
+            aig.set_schedule(**kw)
+            g = run_gpu(aig, w, y0)
+            assert np.all(g["status"] <= 1)
+            if ref is None:
+                ref = g
+                assert int((g["n_acc"] > 300).sum()) > 50   # the budgets above do hand trajectories over
+                continue
+            for k in ref:
+                assert np.array_equal(ref[k].view(np.uint8), g[k].view(np.uint8)), (kw, k)
+    finally:
+        aig.set_schedule()
+    with pytest.raises(Exception):
+        aig.set_schedule(budget=0)
+
+
 def test_config1_two_body_physics(aig):
     """Trap off, N = 65,536: parity on a prefix + physics at full size."""
     w = inputs.config(1)
