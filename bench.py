@@ -363,7 +363,7 @@ def main() -> int:
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--cpu-sample", type=int, default=65536)
+    ap.add_argument("--cpu-sample", type=int, default=2097152)
     ap.add_argument("--ref-sample", type=int, default=16384)
     args = ap.parse_args()
     if args.impl == "reference":

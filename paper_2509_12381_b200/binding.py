@@ -240,7 +240,7 @@ def kernel_info() -> dict:
     return dict(zip(keys, [x.value for x in v]))
 
 
-def set_schedule(tail_iters=256, budget=2048, split_sms=32, split_grid=8, plan=1, kappa=1.25) -> None:
+def set_schedule(tail_iters=256, budget=2048, split_sms=32, split_grid=8, plan=1, kappa=1.5) -> None:
     """Test / tuning hook (include/aig.h: aig_set_schedule); never changes a result."""
     L = lib()
     L.aig_set_schedule.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double]

@@ -173,14 +173,19 @@ __device__ __forceinline__ void ckpt_store(const Ckpt& K, long long slot, long l
 // Scheduling arguments of one launch of the per-thread integrator.  Work items are the entries
 // [*begin, *end) of `order` (trajectory indices; order == nullptr: the indices themselves).  A lane
 // whose trajectory has not ended is suspended (state written to slot atomicAdd(*n_out, 1) of
-// `out`) when it has taken `budget` accepted steps, or `tail_iters` iterations after its warp
-// has seen the queue empty; when the slots are exhausted it simply keeps stepping.  Suspension
-// never changes a trajectory's arithmetic, only where it continues.
+// `out`) when it has taken `budget` accepted steps -- as long as this stage has handed over fewer
+// than `soft_cap` trajectories (the six-lane integrator has half the throughput per FP64
+// operation: it is for the few, not for the many; a trajectory that is kept is asked again one
+// budget later) -- or `tail_iters` iterations after its warp has seen the queue empty; when the
+// slots are exhausted it simply keeps stepping.  Suspension never changes a trajectory's
+// arithmetic, only where it continues.
 struct Sched {
     unsigned long long* queue;
     const long long* order;
     const unsigned long long *begin, *end;
     unsigned long long* n_out;
+    const unsigned long long* soft_base;  // slots handed out before this stage
+    long long soft_cap;
     Ckpt out;
     int budget;
     int tail_iters;
@@ -199,6 +204,7 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
     const int lane = threadIdx.x & 31;
     const long long first = (long long)*S.begin;
     const long long total = (long long)*S.end - first;
+    const long long soft_first = (long long)*S.soft_base;
     Traj T;
     long long idx = -1;
     int stop_at = 0;      // suspend when n_acc reaches this
@@ -242,12 +248,20 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
                 store_traj(y0, N, idx, T, C, st, O);
                 live = false;
             } else if (may_suspend && (T.c.n_acc >= stop_at || since_dry > S.tail_iters)) {
-                const long long slot = (long long)atomicAdd(S.n_out, 1ULL);
-                if (slot < S.out.cap) {
-                    ckpt_store(S.out, slot, idx, T, C);
-                    live = false;
-                } else {
-                    may_suspend = false;  // no slot left: finish it here
+                bool room = true;
+                if (since_dry <= S.tail_iters) {  // budget hand-over: only while the six-lane queue is short
+                    const long long used = (long long)(*(volatile unsigned long long*)S.n_out) - soft_first;
+                    room = used < S.soft_cap;
+                    if (!room) stop_at += S.budget;
+                }
+                if (room) {
+                    const long long slot = (long long)atomicAdd(S.n_out, 1ULL);
+                    if (slot < S.out.cap) {
+                        ckpt_store(S.out, slot, idx, T, C);
+                        live = false;
+                    } else {
+                        may_suspend = false;  // no slot left: finish it here
+                    }
                 }
             }
         }
@@ -387,7 +401,7 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
 // A trajectory can only become long (bound complex, orders of magnitude more steps) if it gets
 // over the centrifugal barrier of the -C4/r^4 tail, i.e. if its impact parameter b is below the
 // Langevin radius b_c = (4 C4/E)^(1/4), E = mu u^2/2 (relative motion at t0).  Those with
-// b < kappa b_c (kappa = 1.25: the moving ion blurs the threshold) are queued first, so that the
+// b < kappa b_c (kappa = 1.5: the moving ion and its micromotion blur the threshold) are queued first, so that the
 // long ones are found early and continue in the split kernel while the bulk is still running.
 // Polynomial form of b^4 < kappa^4 b_c^4:  |d x u|^4 mu < 8 kappa^4 C4 |u|^2.
 // order[0 .. n_front) = candidates, order[n_front .. N) = the rest; counters[0] = n_front on exit,
@@ -685,8 +699,9 @@ struct SchedConfig {
     int budget = 2048;        // accepted steps after which the per-thread integrator hands a trajectory over
     int split_sms = 32;       // SMs that split A takes for itself (one 4-warp block each); bulk B runs on the others
     int split_grid_b = 8;     // split B: one-warp blocks per SM (it has the GPU to itself)
+    int soft_cap = 16384;     // budget hand-overs per bulk stage (drain hand-overs come on top)
     int plan = 1;             // 0: natural order, one bulk launch
-    double kappa = 1.25;      // candidates: b < kappa * Langevin radius
+    double kappa = 1.5;       // candidates: b < kappa * Langevin radius
 };
 
 std::mutex g_sched_mutex;
@@ -819,6 +834,8 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     S.out = slots;
     S.budget = cfg.budget;
     S.tail_iters = cfg.tail_iters;
+    S.soft_base = counters + kCntZero;
+    S.soft_cap = cfg.soft_cap;
     S.timeline = counters + kCntTime + 2;
     SplitSched T;
     T.in = slots;
@@ -869,6 +886,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     integrate_split_kernel<TRAP, kSplitWarps, 1><<<(unsigned)own, 32 * kSplitWarps, (size_t)smem_optin, st>>>(K, y0, N, O, T);
     g_kernel_launches++;
     // second stream: bulk B over order[n_front, N) on the other SMs, then split B over its slots
+    S.soft_base = counters + kCntSlotsA;
     if (cudaStreamWaitEvent(side->stream, side->fork, 0) != cudaSuccess) return AIG_ERR_CUDA;
     S.timeline = counters + kCntTime + 6;
     S.queue = counters + kCntQueueB;
