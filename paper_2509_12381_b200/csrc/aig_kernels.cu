@@ -38,6 +38,10 @@ namespace aig {
 #ifndef AIG_MIN_BLOCKS
 #define AIG_MIN_BLOCKS 2
 #endif
+#ifndef AIG_SPLIT_UNROLL
+#define AIG_SPLIT_UNROLL 2
+#endif
+constexpr int kSplitUnroll = AIG_SPLIT_UNROLL;  // steps per basic block of the six-lane integrator
 constexpr int kBlock = AIG_BLOCK;             // threads per block of the integrator
 constexpr int kBlocksPerSM = AIG_MIN_BLOCKS;  // resident blocks per SM the register budget is sized for
 
@@ -352,19 +356,28 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
         return;
     }
     for (;;) {
-        // ---- one attempted step for every group (all lanes together: full-mask shuffles inside);
-        //      straight-line code up to the vote below
-        SplitAttempt A;
-        StepTimes ST;
-        split_attempt<TRAP>(P, R, K, Y, A, ST);
-        bool accepted;
-        const int st = finish_core(P, K, C, A.err, ST, A.r2, A.s, live, accepted);
-        Y.xi = accepted ? A.Y.xi : Y.xi;
-        Y.vi = accepted ? A.Y.vi : Y.vi;
-        Y.a1i = accepted ? A.Y.a1i : Y.a1i;
-        Y.xa = accepted ? A.Y.xa : Y.xa;
-        Y.va = accepted ? A.Y.va : Y.va;
-        Y.a1a = accepted ? A.Y.a1a : Y.a1a;
+        // ---- kSplitUnroll attempted steps for every group (all lanes together: full-mask shuffles
+        //      inside), straight-line code up to the vote below.  Several steps per basic block
+        //      because the step-size chain of one step continues into the next: the instruction
+        //      scheduler then sees it as the long path and orders a step's bookkeeping (state
+        //      selects, observables, stop tests) behind it instead of in front of it.  A group whose
+        //      trajectory ends inside the block idles for the rest of it (st keeps the status).
+        int st = -1;
+#pragma unroll
+        for (int u = 0; u < kSplitUnroll; ++u) {
+            SplitAttempt A;
+            StepTimes ST;
+            split_attempt<TRAP>(P, R, K, Y, A, ST);
+            bool accepted;
+            const int s1 = finish_core(P, K, C, A.err, ST, A.r2, A.s, live & (st < 0), accepted);
+            Y.xi = accepted ? A.Y.xi : Y.xi;
+            Y.vi = accepted ? A.Y.vi : Y.vi;
+            Y.a1i = accepted ? A.Y.a1i : Y.a1i;
+            Y.xa = accepted ? A.Y.xa : Y.xa;
+            Y.va = accepted ? A.Y.va : Y.va;
+            Y.a1a = accepted ? A.Y.a1a : Y.a1a;
+            st = (st < 0) ? s1 : st;
+        }
         const unsigned fin = __ballot_sync(FULL, st >= 0);
         if (fin == 0u) continue;
         // ---- a8 (rare): lanes e = 0 store component k of the final state, the group's first lane
