@@ -121,7 +121,7 @@ __device__ __forceinline__ void store_scalars(long long idx, const Core& K, Cold
 }
 
 template <class Cold>
-__device__ __forceinline__ void store_traj(const double* __restrict__ y0, long long N, long long idx,
+__device__ __forceinline__ void store_traj(const double (&v0)[3], long long N, long long idx,
                                            const Traj& T, Cold& C, int status, const OutPtrs& O)
 {
 #pragma unroll
@@ -131,7 +131,6 @@ __device__ __forceinline__ void store_traj(const double* __restrict__ y0, long l
         O.y_final[(6 + k) * N + idx] = T.X[3 + k];
         O.y_final[(9 + k) * N + idx] = T.V[3 + k];
     }
-    const double v0[3] = {__ldg(y0 + 9 * N + idx), __ldg(y0 + 10 * N + idx), __ldg(y0 + 11 * N + idx)};
     const double v1[3] = {T.V[3], T.V[4], T.V[5]};
     store_scalars(idx, T.c, C, status, v0, v1, O);
 }
@@ -193,6 +192,7 @@ struct Sched {
     Ckpt out;
     int budget;
     int tail_iters;
+    int refill_batch, refill_wait;
     unsigned long long* timeline;
 };
 
@@ -202,6 +202,7 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
                  const Sched S)
 {
     __shared__ double s_rmin2[BLOCK], s_tfirst[BLOCK], s_tlast[BLOCK];
+    __shared__ double s_v0[3][BLOCK];  // initial atom velocity (for the scattering angle at the end)
     __shared__ int s_nrej[BLOCK], s_nturn[BLOCK];
     ColdShared C{s_rmin2, s_tfirst, s_tlast, s_nrej, s_nturn};
     const unsigned FULL = 0xffffffffu;
@@ -216,12 +217,24 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
     bool live = false;
     bool dry = false;     // warp-uniform: the queue has been seen empty
     bool may_suspend = true;
+    int pending = -1;     // stop status of a finished trajectory whose results are not stored yet
+    int waited = 0;       // warp-uniform: iterations since a lane of this warp went idle
     stage_begin(S.timeline);
 
     for (;;) {
-        // ---- refill: lanes without a trajectory take the next items of the queue
+        // ---- service: lanes without a trajectory store what they finished and take the next items
+        //      of the queue.  The whole warp walks through this code (atan2 / sqrt of the end, global
+        //      loads and the twelve divisions of the start) whenever one lane needs it, so idle lanes
+        //      are served in batches: when refill_batch of them wait, or one has waited refill_wait
+        //      iterations, or the queue is empty.
         const unsigned need = __ballot_sync(FULL, !live);
-        if (need) {
+        if (need && (__popc(need) >= S.refill_batch || waited >= S.refill_wait || dry)) {
+            waited = 0;
+            if (pending >= 0) {
+                const double v0[3] = {s_v0[0][threadIdx.x], s_v0[1][threadIdx.x], s_v0[2][threadIdx.x]};
+                store_traj(v0, N, idx, T, C, pending, O);
+                pending = -1;
+            }
             if (!dry) {
                 const int cnt = __popc(need);
                 const int leader = __ffs(need) - 1;
@@ -233,6 +246,8 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
                     if (cand < total) {
                         idx = S.order ? S.order[first + cand] : first + cand;
                         load_traj<TRAP>(P, y0, N, idx, T, C);
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) s_v0[k][threadIdx.x] = T.V[3 + k];
                         stop_at = S.budget;
                         may_suspend = true;
                         live = true;
@@ -241,6 +256,8 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
                 if ((long long)base + cnt >= total) dry = true;
             }
             if (!__any_sync(FULL, live)) break;
+        } else if (need) {
+            ++waited;
         }
         if (dry) ++since_dry;
         // ---- one attempted step for every live lane
@@ -249,7 +266,7 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
             dp45_attempt<TRAP>(P, T, R);
             const int st = finish_attempt(P, T, C, R);
             if (st >= 0) {
-                store_traj(y0, N, idx, T, C, st, O);
+                pending = st;
                 live = false;
             } else if (may_suspend && (T.c.n_acc >= stop_at || since_dry > S.tail_iters)) {
                 bool room = true;
@@ -699,7 +716,7 @@ bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(pt
 //   bulk B    per-thread integrator over the rest (same rules, same slot buffer, appended)
 //   split A   six-lane integrator over the slots bulk A wrote, BESIDE bulk B: the longest trajectories
 //             (10^2..10^3 x the mean number of steps, all among the candidates) start their long
-//             sequential run early.  It takes `split_sms` SMs for itself (one 4-warp block per SM that
+//             sequential run early.  It takes `split_sms` SMs for itself (one 8-warp block per SM that
 //             asks for the whole shared memory, so that no bulk block can share its FP64 pipes);
 //             bulk B, on a second stream, is sized for the remaining SMs.
 //   split B   six-lane integrator over the slots bulk B wrote (second stream); then the streams join.
@@ -710,9 +727,11 @@ constexpr long long kMinSlots = 65536;
 struct SchedConfig {
     int tail_iters = 256;     // iterations a warp keeps stepping after the queue ran dry
     int budget = 2048;        // accepted steps after which the per-thread integrator hands a trajectory over
-    int split_sms = 32;       // SMs that split A takes for itself (one 4-warp block each); bulk B runs on the others
+    int split_sms = 32;       // SMs that split A takes for itself (one 8-warp block each); bulk B runs on the others
     int split_grid_b = 8;     // split B: one-warp blocks per SM (it has the GPU to itself)
     int soft_cap = 16384;     // budget hand-overs per bulk stage (drain hand-overs come on top)
+    int refill_batch = 8;     // idle lanes of a warp that trigger its refill ...
+    int refill_wait = 16;     // ... or iterations one of them has waited
     int plan = 1;             // 0: natural order, one bulk launch
     double kappa = 1.5;       // candidates: b < kappa * Langevin radius
 };
@@ -738,6 +757,12 @@ SchedConfig sched_config()
             if (got >= 4 && gb >= 1) c.split_grid_b = gb;
             if (got >= 5) c.plan = pl;
             if (got >= 6 && kp >= 0.0) c.kappa = kp;
+        }
+        if (const char* e = std::getenv("AIG_REFILL")) {  // "batch,wait" (tuning aid)
+            int b = c.refill_batch, w = c.refill_wait;
+            const int got = std::sscanf(e, "%d,%d", &b, &w);
+            if (got >= 1 && b >= 1) c.refill_batch = b;
+            if (got >= 2 && w >= 0) c.refill_wait = w;
         }
         g_sched = c;
         g_sched_init = true;
@@ -817,7 +842,11 @@ SideStream* side_stream()
 }
 
 constexpr int kSplitMinBlocks = 8;  // register cap of the split kernel: 65536 / (8 x 32) = 256
-constexpr int kSplitWarps = 4;      // warps per block of the SM-owning variant: one per scheduler, a warp never waits for another
+#ifndef AIG_SPLIT_WARPS
+#define AIG_SPLIT_WARPS 8
+#endif
+constexpr int kSplitWarps = AIG_SPLIT_WARPS;  // warps per block of the SM-owning variant: two per scheduler (a warp issues 30 % of the
+                                              // time, so two barely slow each other while the queue is long; at the end each is alone)
 
 template <int TRAP>
 int launch_integrate(const aig_params* p, const KParams& K, const double* y0, long long N, const OutPtrs& O,
@@ -849,6 +878,8 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     S.tail_iters = cfg.tail_iters;
     S.soft_base = counters + kCntZero;
     S.soft_cap = cfg.soft_cap;
+    S.refill_batch = cfg.refill_batch;
+    S.refill_wait = cfg.refill_wait;
     S.timeline = counters + kCntTime + 2;
     SplitSched T;
     T.in = slots;
