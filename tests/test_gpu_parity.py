@@ -308,6 +308,47 @@ def test_config3_prefix_heavy_light(aig):
     assert g["n_acc"].max() > 20 * np.median(g["n_acc"])   # the imbalance the refill queue is for
 
 
+@pytest.mark.parametrize("cfg,kw", [(4, {}), (3, {})])
+def test_full_size_sampled_outputs(aig, cfg, kw):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (configs[4]: N = 4,194,304,
+    default schedule; configs[3]: N = 1,048,576): outputs of a seeded sample of trajectories are compared
+    with the oracle one by one, the rest through properties that hold at any size."""
+    import torch
+    w = inputs.config(cfg, **kw)
+    y0 = inputs.generate_y0(w)
+    p = aig.make_params(**w.params())
+    out = aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol)
+    ae, le = inputs.histogram_edges()
+    hist = aig.aig_histogram(out, _dev(ae), _dev(le), 64)
+    g = _host(out)
+    H = aig.hist_to_numpy(hist)
+    # properties at any size
+    assert np.all((g["status"] == 0) | (g["status"] == 1))           # exit radius or t_max, nothing failed
+    assert np.array_equal(g["complex_flag"], (g["n_turn"] >= 2).astype(np.uint8))
+    assert np.all(g["lifetime"][g["n_turn"] < 2] == 0) and np.all(g["lifetime"] >= 0)
+    assert np.all(g["n_acc"] >= 1) and np.all(g["n_rej"] >= 0)
+    assert np.all(np.isfinite(g["y_final"])) and np.all((g["angle"] >= 0) & (g["angle"] <= math.pi))
+    tmax_hit = g["status"] == 1
+    assert np.all(g["t_final"][tmax_hit] == w.t_max) and np.all(g["t_final"][~tmax_hit] <= w.t_max)
+    r_fin = np.linalg.norm(g["y_final"][6:9] - g["y_final"][0:3], axis=0)
+    assert np.all(r_fin[~tmax_hit] > w.params()["r_exit"])          # stopped beyond the exit radius
+    assert np.all(g["r_min"] <= r_fin * (1 + 1e-12))
+    ref = orc.histogram(g, ae, le, 64)                                # the device reduction is integer-exact
+    for k in ref:
+        assert np.array_equal(H[k], ref[k]), k
+    assert int(H["totals"][3]) == w.N and int(H["totals"][0]) == int(g["n_acc"].astype(np.int64).sum())
+    # a seeded sample, one by one against the oracle
+    rng = np.random.Generator(np.random.PCG64(12345 + cfg))
+    idx = np.sort(rng.choice(w.N, size=3000, replace=False))
+    ys = np.ascontiguousarray(y0[:, idx])
+    o = run_orc(w, ys)
+    gs = {k: np.ascontiguousarray(v[..., idx]) for k, v in g.items()}
+    _compare_direct(w, ys, gs, o)
+    _ensemble_checks(gs, o, len(idx), len(idx))
+    del out, hist
+    torch.cuda.empty_cache()
+
+
 def test_degenerate_inputs(aig):
     import torch
     w = inputs.config(0)
