@@ -234,10 +234,10 @@ def run_ours(args) -> int:
     ms_int = max_over_ranks(float(np.mean([a.elapsed_time(b) for a, b in kev])))
 
     # stage timeline of the last aig_integrate call (ns %globaltimer stamps the kernels leave in the workspace)
-    tl = ws[:512].view(torch.int64)[32:42].cpu().numpy().astype(np.float64)
+    tl = ws[:512].view(torch.int64)[32:50].cpu().numpy().astype(np.float64)
     t_first = min((x for x in tl if x > 0), default=0.0)
     stages_ms = {name: [round((tl[2 * i] - t_first) / 1e6, 3), round((tl[2 * i + 1] - t_first) / 1e6, 3)]
-                 for i, name in enumerate(("plan", "bulk_candidates", "split_beside_bulk", "bulk_rest", "split_rest"))
+                 for i, name in enumerate(("plan", "bulk0", "split0", "bulk1", "split1", "bulk2", "split2", "bulk3", "split3"))
                  if tl[2 * i] > 0}
 
     n_acc = int(out["n_acc"].sum(dtype=torch.int64).item())

@@ -427,50 +427,121 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
     stage_end(S.timeline);
 }
 
-// ---- work-queue order: trajectories that can reach short range first --------------------------
-// A trajectory can only become long (bound complex, orders of magnitude more steps) if it gets
-// over the centrifugal barrier of the -C4/r^4 tail, i.e. if its impact parameter b is below the
-// Langevin radius b_c = (4 C4/E)^(1/4), E = mu u^2/2 (relative motion at t0).  Those with
-// b < kappa b_c (kappa = 1.5: the moving ion and its micromotion blur the threshold) are queued first, so that the
-// long ones are found early and continue in the split kernel while the bulk is still running.
-// Polynomial form of b^4 < kappa^4 b_c^4:  |d x u|^4 mu < 8 kappa^4 C4 |u|^2.
-// order[0 .. n_front) = candidates, order[n_front .. N) = the rest; counters[0] = n_front on exit,
-// counters[1] = number placed at the back.  Affects scheduling only, never a result.
+// ---- work-queue order: the trajectories that can become long first ------------------------------
+// (1) A trajectory can only form a complex (orders of magnitude more steps) if it gets over the
+//     centrifugal barrier of the -C4/r^4 tail, i.e. if its impact parameter b is below the
+//     Langevin radius b_c = (4 C4/E)^(1/4), E = mu u^2/2 (relative motion at t0): "candidates" are
+//     those with b < kappa b_c (kappa = 1.5: the moving ion and its micromotion blur the
+//     threshold).  Polynomial form of b^4 < kappa^4 b_c^4:  |d x u|^4 mu < 8 kappa^4 C4 |u|^2.
+// (2) Among them the slow ones take longest: the flight alone lasts ~1/u, and the complexes that
+//     survive until t_max are low-energy ones (of the 12 longest trajectories of the bench
+//     workload all have u^2 < <u^2>/2; measured).
+// Three classes, queued in this order, each a stage of the schedule:
+//     0: candidates with u^2 < <u^2>/2   1: the other candidates, and anything with u^2 < <u^2>/10
+//     2: the rest
+// so that the longest trajectories start their sequential run in the six-lane integrator after the
+// first few per cent of the work instead of anywhere.  Affects scheduling only, never a result.
+constexpr int kCntClass = 24;    // counters: trajectories per class (3)
+constexpr int kCntCursor = 28;   // counters: placement cursors (3)
+constexpr int kCntMeanU2 = 60;   // counters: <u^2> (double bits)
+
+struct PlanArgs {
+    double mu, c4k;  // reduced mass, 8 kappa^4 C4
+    double slow0, slow1;  // class thresholds as fractions of <u^2>
+};
+
+__device__ __forceinline__ double rel_speed2(const double* __restrict__ y0, long long N, long long i)
+{
+    const double u0 = y0[9 * N + i] - y0[3 * N + i], u1 = y0[10 * N + i] - y0[4 * N + i],
+                 u2 = y0[11 * N + i] - y0[5 * N + i];
+    return u0 * u0 + u1 * u1 + u2 * u2;
+}
+
+__device__ __forceinline__ int plan_class(const double* __restrict__ y0, long long N, long long i, const PlanArgs& A,
+                                          double mean_u2)
+{
+    const double d0 = y0[6 * N + i] - y0[0 * N + i], d1 = y0[7 * N + i] - y0[1 * N + i],
+                 d2 = y0[8 * N + i] - y0[2 * N + i];
+    const double u0 = y0[9 * N + i] - y0[3 * N + i], u1 = y0[10 * N + i] - y0[4 * N + i],
+                 u2 = y0[11 * N + i] - y0[5 * N + i];
+    const double c0 = d1 * u2 - d2 * u1, c1 = d2 * u0 - d0 * u2, c2 = d0 * u1 - d1 * u0;
+    const double l2 = c0 * c0 + c1 * c1 + c2 * c2;
+    const double usq = u0 * u0 + u1 * u1 + u2 * u2;
+    const bool cand = (l2 * l2 * A.mu < A.c4k * usq);
+    if (cand && usq < A.slow0 * mean_u2) return 0;
+    if (cand || usq < A.slow1 * mean_u2) return 1;
+    return 2;
+}
+
+// <u^2> over the first min(N, 65536) trajectories (a sample is enough for a scheduling threshold)
+__global__ void __launch_bounds__(1024)
+plan_mean_kernel(const double* __restrict__ y0, const long long N, unsigned long long* __restrict__ counters)
+{
+    __shared__ double part[32];
+    const long long n = N < 65536 ? N : 65536;
+    double s = 0.0;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) s += rel_speed2(y0, N, i);
+    for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        s = (threadIdx.x < (blockDim.x >> 5)) ? part[threadIdx.x] : 0.0;
+        for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+        if (threadIdx.x == 0) counters[kCntMeanU2] = (unsigned long long)__double_as_longlong(s / (double)n);
+    }
+}
+
+// PLACE = 0: count the classes; PLACE = 1: write order[] (cursors set by plan_bounds_kernel)
+template <int PLACE>
 __global__ void __launch_bounds__(256)
-plan_kernel(const double* __restrict__ y0, const long long N, const double mu, const double c4k,
-            long long* __restrict__ order, unsigned long long* __restrict__ counters)
+plan_kernel(const double* __restrict__ y0, const long long N, const PlanArgs A, long long* __restrict__ order,
+            unsigned long long* __restrict__ counters)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned FULL = 0xffffffffu;
-    bool front = false;
-    if (i < N) {
-        const double d0 = y0[6 * N + i] - y0[0 * N + i], d1 = y0[7 * N + i] - y0[1 * N + i],
-                     d2 = y0[8 * N + i] - y0[2 * N + i];
-        const double u0 = y0[9 * N + i] - y0[3 * N + i], u1 = y0[10 * N + i] - y0[4 * N + i],
-                     u2 = y0[11 * N + i] - y0[5 * N + i];
-        const double c0 = d1 * u2 - d2 * u1, c1 = d2 * u0 - d0 * u2, c2 = d0 * u1 - d1 * u0;
-        const double l2 = c0 * c0 + c1 * c1 + c2 * c2;
-        const double usq = u0 * u0 + u1 * u1 + u2 * u2;
-        front = (l2 * l2 * mu < c4k * usq);
-    }
-    const unsigned in = __ballot_sync(FULL, i < N);
-    const unsigned fr = __ballot_sync(FULL, front);
-    const unsigned bk = in & ~fr;
+    const double mean_u2 = __longlong_as_double((long long)counters[kCntMeanU2]);
+    const int cls = (i < N) ? plan_class(y0, N, i, A, mean_u2) : -1;
     const int lane = threadIdx.x & 31;
-    unsigned long long bf = 0, bb = 0;
-    if (lane == 0) {
-        if (fr) bf = atomicAdd(&counters[0], (unsigned long long)__popc(fr));
-        if (bk) bb = atomicAdd(&counters[1], (unsigned long long)__popc(bk));
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const unsigned m = __ballot_sync(FULL, cls == c);
+        if (m == 0u) continue;
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(&counters[(PLACE ? kCntCursor : kCntClass) + c], (unsigned long long)__popc(m));
+        if (PLACE) {
+            base = __shfl_sync(FULL, base, 0);
+            if (cls == c) order[base + __popc(m & ((1u << lane) - 1u))] = i;
+        }
     }
-    bf = __shfl_sync(FULL, bf, 0);
-    bb = __shfl_sync(FULL, bb, 0);
-    if (i < N) {
-        const unsigned below = (1u << lane) - 1u;
-        if (front)
-            order[bf + __popc(fr & below)] = i;
-        else
-            order[N - 1 - (long long)(bb + __popc(bk & below))] = i;
+}
+
+// bound[0..3] = prefix sums of the class counts, cursors at the class starts
+__global__ void plan_bounds_kernel(unsigned long long* counters, int bound0, int front)
+{
+    unsigned long long acc = 0;
+    for (int c = 0; c < 3; ++c) {
+        counters[bound0 + c] = acc;
+        counters[kCntCursor + c] = acc;
+        acc += counters[kCntClass + c];
+        if (c == 1) counters[front] = acc;  // classes 0 and 1 (diagnostics)
     }
+    counters[bound0 + 3] = acc;
+}
+
+// without a plan: one stage over [0, N)
+__global__ void bounds_kernel(unsigned long long* counters, int bound0, unsigned long long N)
+{
+    counters[bound0] = 0;
+    counters[bound0 + 1] = N;
+}
+
+// Head start for the split pass of the previous stage: it is next in ITS stream's order and must take
+// its SMs before the bulk pass of this stage (other stream) fills them; both become ready when the
+// previous bulk pass ends.  Waits until the split pass has stamped its start (or at most `ns`).
+__global__ void head_start_kernel(const unsigned long long* started, unsigned long long ns)
+{
+    const unsigned long long t0 = global_ns();
+    while (*(volatile const unsigned long long*)started == 0ULL && global_ns() - t0 < ns) __nanosleep(500);
 }
 
 // counters[dst] = min(counters[src], cap): freezes the number of checkpoint slots written so far
@@ -730,6 +801,8 @@ struct SchedConfig {
     int split_sms = 32;       // SMs that split A takes for itself (one 8-warp block each); bulk B runs on the others
     int split_grid_b = 8;     // split B: one-warp blocks per SM (it has the GPU to itself)
     int soft_cap = 16384;     // budget hand-overs per bulk stage (drain hand-overs come on top)
+    double slow0 = 0.5;       // class 0: candidates with u^2 < slow0 <u^2>
+    double slow1 = 0.1;       // class 1 also takes anything with u^2 < slow1 <u^2>
     int refill_batch = 8;     // idle lanes of a warp that trigger its refill ...
     int refill_wait = 16;     // ... or iterations one of them has waited
     int plan = 1;             // 0: natural order, one bulk launch
@@ -758,11 +831,14 @@ SchedConfig sched_config()
             if (got >= 5) c.plan = pl;
             if (got >= 6 && kp >= 0.0) c.kappa = kp;
         }
-        if (const char* e = std::getenv("AIG_REFILL")) {  // "batch,wait" (tuning aid)
+        if (const char* e = std::getenv("AIG_REFILL")) {  // "batch,wait,slow0,slow1" (tuning aid)
             int b = c.refill_batch, w = c.refill_wait;
-            const int got = std::sscanf(e, "%d,%d", &b, &w);
+            double s0 = c.slow0, s1 = c.slow1;
+            const int got = std::sscanf(e, "%d,%d,%lf,%lf", &b, &w, &s0, &s1);
             if (got >= 1 && b >= 1) c.refill_batch = b;
             if (got >= 2 && w >= 0) c.refill_wait = w;
+            if (got >= 3 && s0 >= 0.0) c.slow0 = s0;
+            if (got >= 4 && s1 >= 0.0) c.slow1 = s1;
         }
         g_sched = c;
         g_sched_init = true;
@@ -779,16 +855,19 @@ constexpr size_t kCounterBytes = 64 * sizeof(unsigned long long);
 size_t order_bytes(long long N) { return round_up((size_t)(N < 1 ? 1 : N) * sizeof(long long), 256); }
 size_t ckpt_buffer_bytes(long long cap) { return round_up((size_t)cap * kCkptBytesPerSlot, 256); }
 
-// counters (uint64 each)
+// counters (uint64 each).  Stage i of the schedule: bulk pass over order[bound[i], bound[i+1]), its
+// hand-overs are the slots [snap[i], snap[i+1]).
+constexpr int kMaxStages = 4;
 enum Counter {
     kCntFront = 0,   // plan: candidates placed (= n_front)
     kCntBack = 1,    // plan: others placed
     kCntZero = 2,    // constant 0
     kCntN = 3,       // constant N
-    kCntQueueA = 4, kCntQueueB = 5, kCntQueueSA = 6, kCntQueueSB = 7,
-    kCntSlots = 8,   // checkpoint slots handed out so far (may overshoot the capacity)
-    kCntSlotsA = 9,  // snapshot after bulk A
-    kCntSlotsB = 10  // snapshot after bulk B
+    kCntSlots = 4,   // checkpoint slots handed out so far (may overshoot the capacity)
+    kCntBound = 5,   // bound[0 .. kMaxStages]
+    kCntSnap = 10,   // snap[0 .. kMaxStages], snap[0] = 0
+    kCntQueueBulk = 16,   // work queue of bulk pass i
+    kCntQueueSplit = 20   // work queue of split pass i
 };
 
 Ckpt ckpt_at(unsigned char* base, long long cap)
@@ -815,27 +894,32 @@ int bulk_capacity(int* blocks_per_sm, int* sm_count)
     return AIG_OK;
 }
 
-// second stream and the fork / join events of the schedule, one set per device
-struct SideStream {
-    cudaStream_t stream = nullptr;
-    cudaEvent_t fork = nullptr, join = nullptr;
+// side streams (stage i >= 1 runs on stream i - 1) and the events that chain and join them, one set
+// per device
+struct SideStreams {
+    cudaStream_t stream[kMaxStages - 1] = {};
+    cudaEvent_t done[kMaxStages] = {};   // done[i]: bulk pass i and its snapshot are complete
+    cudaEvent_t join[kMaxStages - 1] = {};
     bool ok = false;
 };
 std::mutex g_side_mutex;
 
-SideStream* side_stream()
+SideStreams* side_streams()
 {
-    static SideStream side[64];
+    static SideStreams side[64];
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
     std::lock_guard<std::mutex> lock(g_side_mutex);
-    SideStream& s = side[dev];
+    SideStreams& s = side[dev];
     if (!s.ok) {
         int lo = 0, hi = 0;
         if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return nullptr;
-        if (cudaStreamCreateWithPriority(&s.stream, cudaStreamNonBlocking, lo) != cudaSuccess) return nullptr;
-        if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
-        if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        for (int i = 0; i < kMaxStages - 1; ++i) {
+            if (cudaStreamCreateWithPriority(&s.stream[i], cudaStreamNonBlocking, lo) != cudaSuccess) return nullptr;
+            if (cudaEventCreateWithFlags(&s.join[i], cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        }
+        for (int i = 0; i < kMaxStages; ++i)
+            if (cudaEventCreateWithFlags(&s.done[i], cudaEventDisableTiming) != cudaSuccess) return nullptr;
         s.ok = true;
     }
     return &s;
@@ -865,57 +949,33 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     int bps = 0, sms = 0;
     int rc = bulk_capacity<TRAP>(&bps, &sms);
     if (rc) return rc;
-    long long blocks = std::min((long long)bps * sms, (N + kBlock - 1) / kBlock);
+    const long long blocks = std::min((long long)bps * sms, (N + kBlock - 1) / kBlock);
     const bool plan = cfg.plan != 0 && p->C4 > 0.0;
-    SideStream* side = plan ? side_stream() : nullptr;
-    if (plan && !side) return AIG_ERR_CUDA;
+    // stages: the three classes of the plan; without a plan one stage over [0, N)
+    const int stages = plan ? 3 : 1;
+    SideStreams* side = stages > 1 ? side_streams() : nullptr;
+    if (stages > 1 && !side) return AIG_ERR_CUDA;
 
-    Sched S;
-    S.order = nullptr;
-    S.n_out = counters + kCntSlots;
-    S.out = slots;
-    S.budget = cfg.budget;
-    S.tail_iters = cfg.tail_iters;
-    S.soft_base = counters + kCntZero;
-    S.soft_cap = cfg.soft_cap;
-    S.refill_batch = cfg.refill_batch;
-    S.refill_wait = cfg.refill_wait;
-    S.timeline = counters + kCntTime + 2;
-    SplitSched T;
-    T.in = slots;
-    T.timeline = counters + kCntTime + 4;
-    const unsigned split_b = (unsigned)std::min<long long>((long long)cfg.split_grid_b * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
-
-    if (!plan) {
-        // natural order: one bulk launch, then the split kernel over everything it suspended
-        S.queue = counters + kCntQueueA;
-        S.begin = counters + kCntZero;
-        S.end = counters + kCntN;
-        integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
+    long long* order_arg = nullptr;
+    if (plan) {
+        PlanArgs A;
+        A.mu = p->m_ion * p->m_atom / (p->m_ion + p->m_atom);
+        const double k2 = cfg.kappa * cfg.kappa;
+        A.c4k = 8.0 * k2 * k2 * p->C4;
+        A.slow0 = cfg.slow0;
+        A.slow1 = cfg.slow1;
+        const unsigned pg = (unsigned)((N + 255) / 256);
+        plan_mean_kernel<<<1, 1024, 0, st>>>(y0, N, counters);
+        plan_kernel<0><<<pg, 256, 0, st>>>(y0, N, A, order, counters);
+        plan_bounds_kernel<<<1, 1, 0, st>>>(counters, kCntBound, kCntFront);
+        plan_kernel<1><<<pg, 256, 0, st>>>(y0, N, A, order, counters);
+        g_kernel_launches += 4;
+        order_arg = order;
+    } else {
+        bounds_kernel<<<1, 1, 0, st>>>(counters, kCntBound, (unsigned long long)N);
         g_kernel_launches++;
-        T.queue = counters + kCntQueueSA;
-        T.begin = counters + kCntZero;
-        T.end = counters + kCntSlots;
-        integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_b, 32, 0, st>>>(K, y0, N, O, T);
-        g_kernel_launches++;
-        return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
     }
 
-    const double mu = p->m_ion * p->m_atom / (p->m_ion + p->m_atom);
-    const double k2 = cfg.kappa * cfg.kappa;
-    plan_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(y0, N, mu, 8.0 * k2 * k2 * p->C4, order, counters);
-    g_kernel_launches++;
-    // bulk A: order[0, n_front)
-    S.order = order;
-    S.queue = counters + kCntQueueA;
-    S.begin = counters + kCntZero;
-    S.end = counters + kCntFront;
-    integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
-    snapshot_kernel<<<1, 1, 0, st>>>(counters, kCntSlotsA, kCntSlots, (unsigned long long)cap);
-    g_kernel_launches += 2;
-    if (cudaEventRecord(side->fork, st) != cudaSuccess) return AIG_ERR_CUDA;
-    // split A on this stream, right behind bulk A: one block per SM it owns (the dynamic shared
-    // memory request leaves no room for a bulk block beside it)
     int dev = 0, smem_optin = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
@@ -924,29 +984,58 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
                              smem_optin) != cudaSuccess)
         return AIG_ERR_CUDA;
     const long long own = std::max<long long>(1, std::min<long long>(cfg.split_sms, sms / 2));
-    T.queue = counters + kCntQueueSA;
-    T.begin = counters + kCntZero;
-    T.end = counters + kCntSlotsA;
-    integrate_split_kernel<TRAP, kSplitWarps, 1><<<(unsigned)own, 32 * kSplitWarps, (size_t)smem_optin, st>>>(K, y0, N, O, T);
-    g_kernel_launches++;
-    // second stream: bulk B over order[n_front, N) on the other SMs, then split B over its slots
-    S.soft_base = counters + kCntSlotsA;
-    if (cudaStreamWaitEvent(side->stream, side->fork, 0) != cudaSuccess) return AIG_ERR_CUDA;
-    S.timeline = counters + kCntTime + 6;
-    S.queue = counters + kCntQueueB;
-    S.begin = counters + kCntFront;
-    S.end = counters + kCntN;
-    const long long blocks_b = std::max<long long>(1, std::min<long long>(blocks, (long long)bps * (sms - own)));
-    integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks_b, kBlock, 0, side->stream>>>(K, y0, N, O, S);
-    snapshot_kernel<<<1, 1, 0, side->stream>>>(counters, kCntSlotsB, kCntSlots, (unsigned long long)cap);
-    T.timeline = counters + kCntTime + 8;
-    T.queue = counters + kCntQueueSB;
-    T.begin = counters + kCntSlotsA;
-    T.end = counters + kCntSlotsB;
-    integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_b, 32, 0, side->stream>>>(K, y0, N, O, T);
-    g_kernel_launches += 3;
-    if (cudaEventRecord(side->join, side->stream) != cudaSuccess) return AIG_ERR_CUDA;
-    if (cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) return AIG_ERR_CUDA;
+    const long long blocks_beside = std::max<long long>(1, std::min<long long>(blocks, (long long)bps * (sms - own)));
+    const unsigned split_last =
+        (unsigned)std::min<long long>((long long)cfg.split_grid_b * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
+
+    // Stage i on its own stream (stage 0: the caller's): bulk pass i, snapshot, [event done_i], split pass i.
+    // Stage i + 1 waits for done_i, so bulk pass i + 1 runs beside split pass i; the split pass comes first
+    // in its own stream's order and takes its SMs before the next bulk pass (other stream, event) arrives.
+    for (int i = 0; i < stages; ++i) {
+        cudaStream_t cs = (i == 0) ? st : side->stream[i - 1];
+        if (i > 0) {
+            if (cudaStreamWaitEvent(cs, side->done[i - 1], 0) != cudaSuccess) return AIG_ERR_CUDA;
+            // split pass i - 1 stamps counters[kCntTime + 2 (2 + 2 (i - 1))] when its first block starts
+            head_start_kernel<<<1, 1, 0, cs>>>(counters + kCntTime + 2 * (2 + 2 * (i - 1)), 200000ULL);
+            g_kernel_launches++;
+        }
+        Sched S;
+        S.order = order_arg;
+        S.queue = counters + kCntQueueBulk + i;
+        S.begin = counters + kCntBound + i;
+        S.end = counters + kCntBound + i + 1;
+        S.n_out = counters + kCntSlots;
+        S.soft_base = counters + kCntSnap + i;
+        S.soft_cap = cfg.soft_cap;
+        S.out = slots;
+        S.budget = cfg.budget;
+        S.tail_iters = cfg.tail_iters;
+        S.refill_batch = cfg.refill_batch;
+        S.refill_wait = cfg.refill_wait;
+        S.timeline = counters + kCntTime + 2 * (1 + 2 * i);
+        const long long grid = (i == 0) ? blocks : blocks_beside;
+        integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)grid, kBlock, 0, cs>>>(K, y0, N, O, S);
+        snapshot_kernel<<<1, 1, 0, cs>>>(counters, kCntSnap + i + 1, kCntSlots, (unsigned long long)cap);
+        g_kernel_launches += 2;
+        if (i + 1 < stages && cudaEventRecord(side->done[i], cs) != cudaSuccess) return AIG_ERR_CUDA;
+        SplitSched T;
+        T.in = slots;
+        T.timeline = counters + kCntTime + 2 * (2 + 2 * i);
+        T.queue = counters + kCntQueueSplit + i;
+        T.begin = counters + kCntSnap + i;
+        T.end = counters + kCntSnap + i + 1;
+        if (i + 1 < stages) {
+            // beside the next bulk pass: one block per SM it owns (the dynamic shared memory request
+            // leaves no room for a bulk block next to it)
+            integrate_split_kernel<TRAP, kSplitWarps, 1><<<(unsigned)own, 32 * kSplitWarps, (size_t)smem_optin, cs>>>(K, y0, N, O, T);
+        } else {
+            integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_last, 32, 0, cs>>>(K, y0, N, O, T);
+        }
+        g_kernel_launches++;
+        if (i > 0 && cudaEventRecord(side->join[i - 1], cs) != cudaSuccess) return AIG_ERR_CUDA;
+    }
+    for (int i = 1; i < stages; ++i)
+        if (cudaStreamWaitEvent(st, side->join[i - 1], 0) != cudaSuccess) return AIG_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
 
