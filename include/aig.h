@@ -167,9 +167,9 @@ uint64_t aig_kernel_launches(void);
  *               queue ran dry before it hands its trajectories over (default 256)
  *   budget      accepted steps after which a trajectory is handed to the six-lane integrator
  *               (default 2048)
- *   split_sms   SMs the six-lane integrator owns while the second part of the bulk runs (32)
+ *   split_sms   SMs a six-lane pass owns while the next bulk pass runs beside it (32)
  *   split_grid  one-warp blocks per SM of the final six-lane pass (8)
- *   plan        0: natural order, one bulk pass; 1: capture candidates first (default)
+ *   plan        0: natural order, one bulk pass; 1: three classes, slow capture candidates first (default)
  *   kappa       candidates are trajectories with impact parameter < kappa Langevin radii (1.5)
  * Scheduling never changes a result (tests/test_gpu_parity.py::test_schedule_invariance).
  * Returns AIG_ERR_PARAM for out-of-range values.  Not thread-safe against concurrent

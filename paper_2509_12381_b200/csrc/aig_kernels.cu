@@ -1,9 +1,10 @@
 // aig_kernels.cu -- kernels and C ABI of libaig (include/aig.h).  sm_100a only.
 //
 // Kernels
-//   plan_kernel              : orders the work queue: trajectories whose impact parameter is inside
-//                              ~1.25 Langevin radii (the only ones that can reach short range and
-//                              form a long-lived complex) go first.  Scheduling only.
+//   plan_*_kernel            : order the work queue in three classes: slow capture candidates (impact
+//                              parameter inside 1.5 Langevin radii: the only ones that can form a
+//                              long-lived complex; the slow ones last longest), the other candidates,
+//                              the rest.  Scheduling only.
 //   integrate_kernel<TRAP>   : persistent threads, one trajectory per lane, registers only;
 //                              finished lanes refill from a global atomic work queue
 //                              (warp-aggregated: one atomicAdd per warp per refill event); a
@@ -781,25 +782,28 @@ KParams make_kparams(const aig_params* p, double t_max, double rtol, double atol
 bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(ptr) % a) == 0; }
 
 // ---- schedule of one aig_integrate call ------------------------------------------------------
-//   plan      order[] = capture candidates first (plan_kernel), n_front of them
-//   bulk A    per-thread integrator over the candidates; what outlives `budget` accepted steps, or
-//             is still running `tail_iters` iterations after the queue ran dry, is suspended
-//   bulk B    per-thread integrator over the rest (same rules, same slot buffer, appended)
-//   split A   six-lane integrator over the slots bulk A wrote, BESIDE bulk B: the longest trajectories
-//             (10^2..10^3 x the mean number of steps, all among the candidates) start their long
-//             sequential run early.  It takes `split_sms` SMs for itself (one 8-warp block per SM that
-//             asks for the whole shared memory, so that no bulk block can share its FP64 pipes);
-//             bulk B, on a second stream, is sized for the remaining SMs.
-//   split B   six-lane integrator over the slots bulk B wrote (second stream); then the streams join.
-// No kernel ever waits for another one on the device (no polling): every dependency is a stream
-// order or an event.
+//   plan        order[] in three classes (plan_*_kernel), bound[] = where each class starts
+//   stage i     (i = 0, 1, 2 = class; each on its own stream, stage 0 on the caller's):
+//     bulk i    per-thread integrator over class i; what outlives `budget` accepted steps, or is
+//               still running `tail_iters` iterations after the queue ran dry, is suspended into
+//               the next free checkpoint slots
+//     split i   six-lane integrator over the slots bulk i wrote.  Stage i + 1 starts when bulk i is
+//               complete (event), so split i runs BESIDE bulk i + 1: the longest trajectories
+//               (10^2..10^3 x the mean number of steps, nearly all in class 0) start their long
+//               sequential run after a few per cent of the work.  Beside a bulk pass it takes
+//               `split_sms` SMs for itself (one 8-warp block per SM that asks for the whole shared
+//               memory, so that no bulk block can share its FP64 pipes); that bulk pass is sized
+//               for the remaining SMs and lets the split pass take its SMs first (head_start_kernel).
+//   join        the caller's stream waits for the side streams.
+// No kernel waits for another one's progress (no polling for work): every dependency is a stream
+// order or an event; head_start_kernel only delays a launch, by at most 200 us.
 constexpr long long kMinSlots = 65536;
 
 struct SchedConfig {
     int tail_iters = 256;     // iterations a warp keeps stepping after the queue ran dry
     int budget = 2048;        // accepted steps after which the per-thread integrator hands a trajectory over
-    int split_sms = 32;       // SMs that split A takes for itself (one 8-warp block each); bulk B runs on the others
-    int split_grid_b = 8;     // split B: one-warp blocks per SM (it has the GPU to itself)
+    int split_sms = 32;       // SMs a six-lane pass takes for itself beside a bulk pass (one 8-warp block each)
+    int split_grid_b = 8;     // last six-lane pass: one-warp blocks per SM (it has the GPU to itself)
     int soft_cap = 16384;     // budget hand-overs per bulk stage (drain hand-overs come on top)
     double slow0 = 0.5;       // class 0: candidates with u^2 < slow0 <u^2>
     double slow1 = 0.1;       // class 1 also takes anything with u^2 < slow1 <u^2>
