@@ -797,7 +797,9 @@ bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(pt
 //   join        the caller's stream waits for the side streams.
 // No kernel waits for another one's progress (no polling for work): every dependency is a stream
 // order or an event; head_start_kernel only delays a launch, by at most 200 us.
-constexpr long long kMinSlots = 65536;
+// Checkpoint slots: min(N, max(2^20, N/4)).  Hand-overs are bounded by 3 stages x (soft_cap + resident lanes)
+// ~ 1.6e5, so the capacity test in the kernel is a safety net, not a working regime.
+constexpr long long kMinSlots = 1 << 20;
 
 struct SchedConfig {
     int tail_iters = 256;     // iterations a warp keeps stepping after the queue ran dry
@@ -864,7 +866,6 @@ size_t ckpt_buffer_bytes(long long cap) { return round_up((size_t)cap * kCkptByt
 constexpr int kMaxStages = 4;
 enum Counter {
     kCntFront = 0,   // plan: candidates placed (= n_front)
-    kCntBack = 1,    // plan: others placed
     kCntZero = 2,    // constant 0
     kCntN = 3,       // constant N
     kCntSlots = 4,   // checkpoint slots handed out so far (may overshoot the capacity)

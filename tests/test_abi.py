@@ -42,7 +42,7 @@ def test_version_strerror_workspace(lib):
     assert lib.aig_workspace_bytes(0) >= 8 and lib.aig_workspace_bytes(1 << 22) >= 8
     assert lib.aig_kernel_launches() == 0       # nothing launched by loading
     # workspace: counters + 8 B per trajectory (queue order) + checkpoint slots, monotone in N
-    assert lib.aig_workspace_bytes(1 << 22) >= 512 + 8 * (1 << 22) + 65536 * 216
+    assert lib.aig_workspace_bytes(1 << 22) >= 512 + 8 * (1 << 22) + (1 << 20) * 216
     assert lib.aig_workspace_bytes(1 << 22) > lib.aig_workspace_bytes(1 << 20) > lib.aig_workspace_bytes(256)
     # the schedule hook validates its arguments on the host (no device needed)
     lib.aig_set_schedule.argtypes = [C.c_int] * 5 + [C.c_double]
