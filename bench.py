@@ -364,7 +364,7 @@ def main() -> int:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=2097152)
-    ap.add_argument("--ref-sample", type=int, default=16384)
+    ap.add_argument("--ref-sample", type=int, default=262144)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

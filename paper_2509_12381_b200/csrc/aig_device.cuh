@@ -101,10 +101,22 @@ __device__ __forceinline__ double trap_cos(const KParams& P, double t)
 // (a + b) + c: the one order in which every three-component sum is formed (both kernels)
 __device__ __forceinline__ double sum3(double a, double b, double c) { return (a + b) + c; }
 
-// plain compare-and-select maximum / minimum (one DSETP and two selects; fmax / fmin add NaN
-// quieting the callers do not need).  A NaN first operand yields the second operand.
-__device__ __forceinline__ double dmax(double a, double b) { return (a > b) ? a : b; }
-__device__ __forceinline__ double dmin(double a, double b) { return (a < b) ? a : b; }
+// plain compare-and-select maximum / minimum: one DSETP and two selects.  Written in PTX because
+// the compiler turns (a > b) ? a : b into max.f64, whose SASS expansion (DSETP.MAX, FSEL, SEL, a
+// predicated LOP3 that quiets NaNs) is longer and deeper; the callers do not need NaN quieting.
+// A NaN first operand yields the second operand.
+__device__ __forceinline__ double dmax(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.gt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
+__device__ __forceinline__ double dmin(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
 
 // gi = -(dV/dr)/(r m_ion) and ga = +(dV/dr)/(r m_atom) from r^2, (dV/dr)/r = 4 C4/r^6 - 8 C8/r^10:
 // the masses are folded into the constants so that both factors are three operations behind 1/r^2
