@@ -264,3 +264,46 @@ def histogram(obs: dict, angle_edges, life_edges, n_turn_bins: int = 64) -> dict
                          np.asarray(obs["n_rej"]).astype(np.int64).sum(),
                          int(cf.sum()), N], dtype=np.uint64),
     )
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: the paper's remaining per-trajectory observables and its "outliers"
+# ---------------------------------------------------------------------------------------------
+OUTLIER_KEYS = ("angle", "n_turn", "lifetime", "transfer", "dist", "n_acc", "KE")
+
+
+def observables(p: OrcParams, y0, y_final) -> dict:
+    """The observables of PAPER.md:495-497 that follow from the initial and final states alone,
+    written as their definitions (float64, one trajectory per column):
+      dist     final atom-ion distance                     |x_atom - x_ion| at the end
+      KE       final kinetic energy of the ion             m_ion |v_ion|^2 / 2
+      transfer momentum transferred by the atom            m_atom |v_atom(end) - v_atom(t0)|
+    (the paper names them without formulas; readings S24-S26 of DESIGN.md)."""
+    y0 = np.asarray(y0, dtype=np.float64)
+    yf = np.asarray(y_final, dtype=np.float64)
+    d = yf[6:9] - yf[0:3]
+    dv = yf[9:12] - y0[9:12]
+    return {"dist": np.sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]),
+            "KE": 0.5 * p.m_ion * (yf[3] * yf[3] + yf[4] * yf[4] + yf[5] * yf[5]),
+            "transfer": p.m_atom * np.sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2])}
+
+
+def outliers(obs: dict) -> dict:
+    """PAPER.md:521 ("outliers.txt stores the initial conditions for the trajectories with the highest
+    and lowest value of each observable"): for each observable of OUTLIER_KEYS the index of its
+    smallest and of its largest value; the first index wins a tie; NaNs are skipped (an observable
+    that is NaN everywhere, or N = 0, gives -1).  Plain loops over the definition."""
+    out = {}
+    for k in OUTLIER_KEYS:
+        v = np.asarray(obs[k])
+        lo = hi = -1
+        for i in range(v.shape[0]):
+            x = v[i]
+            if x != x:
+                continue
+            if lo < 0 or x < v[lo]:
+                lo = i
+            if hi < 0 or x > v[hi]:
+                hi = i
+        out[k] = (lo, hi)
+    return out

@@ -532,3 +532,67 @@ def test_histogram_definition_bruteforce():
     assert np.array_equal(H["status"], [np.sum(obs["status"] == s) for s in range(4)])
     assert list(H["totals"]) == [obs["n_acc"].sum(), obs["n_rej"].sum(), obs["complex_flag"].sum(), n]
     assert H["angle"].sum() == n and H["angle"][-1] == (obs["angle"] >= math.pi).sum() + 1
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: remaining observables and outliers (:521)
+# ---------------------------------------------------------------------------------------------
+
+def test_observables_two_body_closed_forms():
+    """Trap off, centre-of-mass frame (config 1): total momentum is zero, so
+    m_ion v_ion = -m_atom v_atom at all times, and far from the ion the atom's speed is its initial
+    one, so the momentum it transfers is the chord  2 m_atom |v_atom| sin(angle / 2)  of its
+    deflection; the final distance lies just beyond the exit radius."""
+    w = inputs.config(1).replace(N=400)
+    y0 = inputs.generate_y0(w)
+    p = orc.make_params(**w.params())
+    o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=4)
+    ob = orc.observables(p, y0, o["y_final"])
+    va = np.linalg.norm(o["y_final"][9:12], axis=0)
+    # KE_ion = (m_atom / m_ion) KE_atom  (zero total momentum)
+    ke_from_atom = 0.5 * p.m_atom ** 2 / p.m_ion * va ** 2
+    assert np.max(np.abs(ob["KE"] / ke_from_atom - 1)) < 1e-9
+    # chord formula, with the measured initial and final speeds (they differ by V(R)/E ~ 1e-4)
+    v0 = np.linalg.norm(y0[9:12], axis=0)
+    chord = p.m_atom * np.sqrt(v0 ** 2 + va ** 2 - 2 * v0 * va * np.cos(o["angle"]))
+    assert np.max(np.abs(ob["transfer"] - chord)) <= 1e-9 * np.max(chord)
+    ex = o["status"] == 0   # a complex still bound at t_max has not recovered its asymptotic speed
+    simple = 2 * p.m_atom * v0 * np.sin(o["angle"] / 2)
+    assert ex.sum() > 350 and np.max(np.abs(ob["transfer"] - simple)[ex]) <= 2e-3 * np.max(simple)
+    r_exit = w.params()["r_exit"]
+    assert np.all(ob["dist"][ex] > r_exit) and np.all(ob["dist"][ex] < 1.2 * r_exit)
+    assert np.allclose(ob["dist"], np.linalg.norm(o["y_final"][6:9] - o["y_final"][0:3], axis=0), rtol=1e-15)
+
+
+def test_observables_free_motion_exact():
+    """No potential, no trap: nothing is transferred, the ion keeps its kinetic energy, and the final
+    distance is |d0 + u t_final| of the straight line."""
+    w = inputs.config(0).replace(N=64)
+    y0 = inputs.generate_y0(w)
+    kw = w.params()
+    kw.update(C4=0.0, C8=0.0, omega_rf=0.0)
+    p = orc.make_params(**kw)
+    o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=2)
+    ob = orc.observables(p, y0, o["y_final"])
+    assert np.max(ob["transfer"]) <= 1e-12 * p.m_atom * np.max(np.linalg.norm(y0[9:12], axis=0))
+    assert np.allclose(ob["KE"], 0.5 * p.m_ion * np.sum(y0[3:6] ** 2, axis=0), rtol=1e-12)
+    d_lin = (y0[6:9] - y0[0:3]) + (y0[9:12] - y0[3:6]) * o["t_final"]
+    assert np.allclose(ob["dist"], np.linalg.norm(d_lin, axis=0), rtol=1e-10)
+
+
+def test_outliers_definition():
+    rng = np.random.Generator(np.random.PCG64(7))
+    n = 500
+    obs = {k: rng.standard_normal(n) for k in orc.OUTLIER_KEYS}
+    obs["n_turn"] = rng.integers(0, 5, n).astype(np.int32)       # many ties: the first index wins
+    obs["n_acc"] = rng.integers(10, 1000, n).astype(np.int32)
+    obs["lifetime"][::7] = np.nan                                  # NaNs are skipped
+    out = orc.outliers(obs)
+    for k in orc.OUTLIER_KEYS:
+        v = np.asarray(obs[k], dtype=np.float64)
+        assert out[k] == (int(np.nanargmin(v)), int(np.nanargmax(v))), k
+    assert out["n_turn"][0] == int(np.flatnonzero(obs["n_turn"] == obs["n_turn"].min())[0])
+    allnan = {k: np.full(4, np.nan) for k in orc.OUTLIER_KEYS}
+    assert all(v == (-1, -1) for v in orc.outliers(allnan).values())
+    empty = {k: np.empty(0) for k in orc.OUTLIER_KEYS}
+    assert all(v == (-1, -1) for v in orc.outliers(empty).values())
