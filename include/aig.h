@@ -130,6 +130,33 @@ int aig_integrate(const aig_params *p, const double *y0, int64_t N, double t_max
 int aig_histogram(const aig_out *obs, int64_t N, const aig_hist_spec *spec, const aig_hist *out,
                   void *cuda_stream);
 
+/* ---- NEXT-1: the paper's remaining observables and its outliers ------------------ */
+
+/* Observables of PAPER.md:495-497 that follow from the initial and final states alone: DEVICE
+ * arrays of length N, written by aig_observables.  The paper names them without formulas; the
+ * readings are DESIGN.md S24-S26:
+ *   dist      "the final atom-ion distance"          |x_atom - x_ion| at the end
+ *   KE        "the final kinetic energy of the ion"  m_ion |v_ion|^2 / 2
+ *   transfer  "the momentum transfered by the atom"  m_atom |v_atom(end) - v_atom(t0)|          */
+typedef struct aig_obs_extra {
+    double *dist, *KE, *transfer;
+} aig_obs_extra;
+
+/* dist, KE, transfer of N trajectories from y0 (DEVICE [12][N]) and out->y_final as written by
+ * aig_integrate (only y_final of `out` is read).  One HBM-bound kernel on `cuda_stream`. */
+int aig_observables(const aig_params *p, const double *y0, const aig_out *out, int64_t N,
+                    const aig_obs_extra *extra, void *cuda_stream);
+
+/* "outliers" (the trajectories with the highest and lowest value of each
+ * observable): result (DEVICE int64 [7][2]) receives, for the observables
+ *   0 angle, 1 n_turn ("bounces"), 2 lifetime, 3 transfer, 4 dist, 5 n_acc ("nsteps"), 6 KE
+ * the index of the smallest ([k][0]) and of the largest ([k][1]) value; the smallest index wins a
+ * tie, NaNs are skipped, -1 when nothing qualifies (N = 0).  One pass over the seven arrays.
+ * workspace: DEVICE scratch of aig_outliers_workspace_bytes() bytes, 16-byte aligned. */
+size_t aig_outliers_workspace_bytes(void);
+int aig_outliers(const aig_out *out, const aig_obs_extra *extra, int64_t N, int64_t *result,
+                 void *workspace, void *cuda_stream);
+
 /* Test hook: ONE attempted DP5(4) step of size h[i] from (t[i], y[:, i]) for each of N
  * states.  DEVICE: y [12][N], t [N], h [N], ynew [12][N] (5th-order solution), err [N]
  * (ode45's scaled error estimate; the step would be accepted iff err <= rtol). */

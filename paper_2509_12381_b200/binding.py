@@ -18,7 +18,7 @@ _lib = None
 
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
            "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_set_schedule", "aig_strerror",
-           "aig_version"]
+           "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes"]
 
 
 class AigError(RuntimeError):
@@ -178,6 +178,48 @@ def aig_histogram(obs, angle_edges, life_edges, n_turn_bins: int = 64, hist=None
     rc = lib().aig_histogram(C.byref(o), N, C.byref(spec), C.byref(h), _stream_ptr(stream))
     _check(rc, "aig_histogram")
     return hist
+
+
+class ObsExtra(C.Structure):
+    _fields_ = [("dist", C.c_void_p), ("KE", C.c_void_p), ("transfer", C.c_void_p)]
+
+
+OUTLIER_KEYS = ("angle", "n_turn", "lifetime", "transfer", "dist", "n_acc", "KE")   # order of aig_outliers' result rows
+
+
+def aig_observables(params: Params, y0, obs, extra=None, stream=None):
+    """dist, KE, transfer (include/aig.h) of the trajectories in ``obs`` (dict from aig_integrate)."""
+    torch = _torch()
+    N = y0.shape[1]
+    assert y0.is_cuda and y0.dtype == torch.float64 and y0.shape[0] == 12 and y0.is_contiguous()
+    if extra is None:
+        extra = {k: torch.empty(N, dtype=torch.float64, device=y0.device) for k in ("dist", "KE", "transfer")}
+    e = ObsExtra(*[extra[k].data_ptr() for k in ("dist", "KE", "transfer")])
+    o = _out_struct(obs)
+    L = lib()
+    L.aig_observables.restype = C.c_int
+    L.aig_observables.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    _check(L.aig_observables(C.byref(params), y0.data_ptr(), C.byref(o), N, C.byref(e), _stream_ptr(stream)),
+           "aig_observables")
+    return extra
+
+
+def aig_outliers(obs, extra, stream=None):
+    """int64 CUDA tensor [7, 2]: index of the smallest / largest value of each OUTLIER_KEYS observable."""
+    torch = _torch()
+    N = obs["angle"].numel()
+    dev = obs["angle"].device
+    L = lib()
+    L.aig_outliers_workspace_bytes.restype = C.c_size_t
+    L.aig_outliers.restype = C.c_int
+    L.aig_outliers.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+    ws = torch.empty(int(L.aig_outliers_workspace_bytes()), dtype=torch.uint8, device=dev)
+    res = torch.empty((len(OUTLIER_KEYS), 2), dtype=torch.int64, device=dev)
+    e = ObsExtra(*[extra[k].data_ptr() for k in ("dist", "KE", "transfer")])
+    o = _out_struct(obs)
+    _check(L.aig_outliers(C.byref(o), C.byref(e), N, res.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "aig_outliers")
+    res._ws = ws  # keep the scratch alive until the stream has run
+    return res
 
 
 def aig_step_once(params: Params, y, t, h, rtol, atol, stream=None):

@@ -687,6 +687,129 @@ histogram_kernel(const HistArgs a, const long long N)
 }
 
 // ------------------------------------------------------------------------------------------
+// NEXT-1: the paper's remaining observables and its outliers (:521)
+// ------------------------------------------------------------------------------------------
+// HBM-bound: reads the final state (96 B) and the initial atom velocity (24 B), writes 24 B.
+__global__ void __launch_bounds__(256)
+observables_kernel(const double* __restrict__ y0, const double* __restrict__ yf, const long long N,
+                   const double m_ion, const double m_atom, double* __restrict__ dist, double* __restrict__ ke,
+                   double* __restrict__ transfer)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+        const double d0 = yf[6 * N + i] - yf[0 * N + i], d1 = yf[7 * N + i] - yf[1 * N + i],
+                     d2 = yf[8 * N + i] - yf[2 * N + i];
+        const double v0 = yf[3 * N + i], v1 = yf[4 * N + i], v2 = yf[5 * N + i];
+        const double w0 = yf[9 * N + i] - y0[9 * N + i], w1 = yf[10 * N + i] - y0[10 * N + i],
+                     w2 = yf[11 * N + i] - y0[11 * N + i];
+        dist[i] = sqrt(sum3(d0 * d0, d1 * d1, d2 * d2));
+        ke[i] = (0.5 * m_ion) * sum3(v0 * v0, v1 * v1, v2 * v2);
+        transfer[i] = m_atom * sqrt(sum3(w0 * w0, w1 * w1, w2 * w2));
+    }
+}
+
+// arg-min / arg-max of seven observables in one pass: (value, index) pairs, the smaller index wins
+// a tie, NaNs are skipped, index -1 = nothing seen.
+constexpr int kOutlierObs = 7;  // angle, n_turn, lifetime, transfer, dist, n_acc, KE
+struct Extreme {
+    double v;
+    long long i;
+};
+__device__ __forceinline__ Extreme pick_min(const Extreme a, const Extreme b)
+{
+    const bool tb = (b.i >= 0) && ((a.i < 0) || (b.v < a.v) || ((b.v == a.v) && (b.i < a.i)));
+    return tb ? b : a;
+}
+__device__ __forceinline__ Extreme pick_max(const Extreme a, const Extreme b)
+{
+    const bool tb = (b.i >= 0) && ((a.i < 0) || (b.v > a.v) || ((b.v == a.v) && (b.i < a.i)));
+    return tb ? b : a;
+}
+__device__ __forceinline__ Extreme shfl_extreme(const Extreme e, int off)
+{
+    Extreme r;
+    r.v = __shfl_down_sync(0xffffffffu, e.v, off);
+    r.i = __shfl_down_sync(0xffffffffu, e.i, off);
+    return r;
+}
+
+struct OutlierArgs {
+    const double *angle, *lifetime, *transfer, *dist, *ke;
+    const int *n_turn, *n_acc;
+    Extreme* partial;              // [gridDim.x][kOutlierObs][2]
+    unsigned int* ticket;          // blocks that have finished
+    long long* result;             // [kOutlierObs][2]: index of the minimum, of the maximum
+};
+
+__global__ void __launch_bounds__(256)
+outliers_kernel(const OutlierArgs a, const long long N)
+{
+    __shared__ Extreme s_part[8][kOutlierObs][2];
+    __shared__ bool s_last;
+    Extreme lo[kOutlierObs], hi[kOutlierObs];
+#pragma unroll
+    for (int k = 0; k < kOutlierObs; ++k) {
+        lo[k].v = hi[k].v = 0.0;
+        lo[k].i = hi[k].i = -1;
+    }
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+        const double x[kOutlierObs] = {a.angle[i],    (double)a.n_turn[i], a.lifetime[i], a.transfer[i],
+                                       a.dist[i],     (double)a.n_acc[i],  a.ke[i]};
+#pragma unroll
+        for (int k = 0; k < kOutlierObs; ++k) {
+            if (x[k] == x[k]) {
+                const Extreme e{x[k], i};
+                lo[k] = pick_min(lo[k], e);
+                hi[k] = pick_max(hi[k], e);
+            }
+        }
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < kOutlierObs; ++k) {
+        for (int off = 16; off > 0; off >>= 1) {
+            lo[k] = pick_min(lo[k], shfl_extreme(lo[k], off));
+            hi[k] = pick_max(hi[k], shfl_extreme(hi[k], off));
+        }
+        if (lane == 0) {
+            s_part[warp][k][0] = lo[k];
+            s_part[warp][k][1] = hi[k];
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < kOutlierObs * 2) {
+        const int k = threadIdx.x >> 1, m = threadIdx.x & 1;
+        Extreme e = s_part[0][k][m];
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) e = m ? pick_max(e, s_part[w][k][m]) : pick_min(e, s_part[w][k][m]);
+        a.partial[((size_t)blockIdx.x * kOutlierObs + k) * 2 + m] = e;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (s_last) {
+        // the last block to finish folds the partials: 16 threads per (observable, min | max); the order
+        // of the fold does not matter ((value, index) pairs are totally ordered)
+        __threadfence();
+        const int c = threadIdx.x >> 4, sub = threadIdx.x & 15;
+        const bool act = c < kOutlierObs * 2;
+        const int k = act ? (c >> 1) : 0, m = c & 1;
+        Extreme e{0.0, -1};
+        if (act)
+            for (unsigned b = sub; b < gridDim.x; b += 16) {
+                const Extreme f = a.partial[((size_t)b * kOutlierObs + k) * 2 + m];
+                e = m ? pick_max(e, f) : pick_min(e, f);
+            }
+        for (int off = 8; off > 0; off >>= 1) {
+            const Extreme f = shfl_extreme(e, off);
+            e = m ? pick_max(e, f) : pick_min(e, f);
+        }
+        if (act && sub == 0) a.result[k * 2 + m] = e.i;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // FP64 roofline probe: ILP independent FMA chains per thread, all in registers
 // ------------------------------------------------------------------------------------------
 template <int ILP>
@@ -1185,6 +1308,68 @@ int aig_histogram(const aig_out* obs, int64_t N, const aig_hist_spec* spec, cons
     const long long cap = (long long)sms * 8;
     if (blocks > cap) blocks = cap;
     histogram_kernel<<<(unsigned)blocks, 256, smem, st>>>(a, N);
+    g_kernel_launches++;
+    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
+}
+
+int aig_observables(const aig_params* p, const double* y0, const aig_out* out, int64_t N,
+                    const aig_obs_extra* extra, void* cuda_stream)
+{
+    if (!p || !extra) return AIG_ERR_NULL;
+    if (!(p->m_ion > 0.0) || !(p->m_atom > 0.0) || !std::isfinite(p->m_ion) || !std::isfinite(p->m_atom))
+        return AIG_ERR_PARAM;
+    if (N < 0 || N > (1LL << 40)) return AIG_ERR_SIZE;
+    if (N == 0) return AIG_OK;
+    if (!y0 || !out || !out->y_final || !extra->dist || !extra->KE || !extra->transfer) return AIG_ERR_NULL;
+    if (!aligned(y0, 8) || !aligned(out->y_final, 8) || !aligned(extra->dist, 8) || !aligned(extra->KE, 8) ||
+        !aligned(extra->transfer, 8))
+        return AIG_ERR_ALIGN;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AIG_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return AIG_ERR_CUDA;
+    const long long blocks = std::min<long long>((N + 255) / 256, (long long)sms * 8);
+    observables_kernel<<<(unsigned)blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        y0, out->y_final, N, p->m_ion, p->m_atom, extra->dist, extra->KE, extra->transfer);
+    g_kernel_launches++;
+    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
+}
+
+constexpr int kOutlierBlocksMax = 1024;
+
+size_t aig_outliers_workspace_bytes(void)
+{
+    return 256 + (size_t)kOutlierBlocksMax * kOutlierObs * 2 * sizeof(Extreme);
+}
+
+int aig_outliers(const aig_out* out, const aig_obs_extra* extra, int64_t N, int64_t* result, void* workspace,
+                 void* cuda_stream)
+{
+    if (!result || !workspace) return AIG_ERR_NULL;
+    if (N < 0 || N > (1LL << 40)) return AIG_ERR_SIZE;
+    if (!aligned(result, 8) || !aligned(workspace, 16)) return AIG_ERR_ALIGN;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (N > 0) {
+        if (!out || !extra) return AIG_ERR_NULL;
+        if (!out->angle || !out->lifetime || !out->n_turn || !out->n_acc || !extra->dist || !extra->KE || !extra->transfer)
+            return AIG_ERR_NULL;
+    }
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AIG_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return AIG_ERR_CUDA;
+    if (cudaMemsetAsync(workspace, 0, 256, st) != cudaSuccess) return AIG_ERR_CUDA;
+    OutlierArgs a;
+    a.angle = N ? out->angle : nullptr;
+    a.lifetime = N ? out->lifetime : nullptr;
+    a.n_turn = N ? out->n_turn : nullptr;
+    a.n_acc = N ? out->n_acc : nullptr;
+    a.transfer = N ? extra->transfer : nullptr;
+    a.dist = N ? extra->dist : nullptr;
+    a.ke = N ? extra->KE : nullptr;
+    a.ticket = static_cast<unsigned int*>(workspace);
+    a.partial = reinterpret_cast<Extreme*>(static_cast<unsigned char*>(workspace) + 256);
+    a.result = reinterpret_cast<long long*>(result);
+    long long blocks = std::min<long long>(std::max<long long>(1, (N + 255) / 256), std::min<long long>((long long)sms * 4, kOutlierBlocksMax));
+    outliers_kernel<<<(unsigned)blocks, 256, 0, st>>>(a, N);
     g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }

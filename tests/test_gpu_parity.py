@@ -349,6 +349,45 @@ def test_full_size_sampled_outputs(aig, cfg, kw):
     torch.cuda.empty_cache()
 
 
+def test_observables_and_outliers(aig):
+    """NEXT-1: dist, KE, transfer against their definitions on the same arrays (rounding only), the
+    outliers index for index (integer work: exact), on several blocks and a ragged tail, with ties
+    and NaNs, and for N = 0."""
+    import torch
+    w = inputs.config(2).replace(N=20000 + 13)
+    y0 = inputs.generate_y0(w)
+    p = aig.make_params(**w.params())
+    y0d = _dev(y0)
+    out = aig.aig_integrate(p, y0d, w.t_max, w.rtol, w.atol)
+    extra = aig.aig_observables(p, y0d, out)
+    res = aig.aig_outliers(out, extra)
+    g = _host(out)
+    e = {k: v.cpu().numpy() for k, v in extra.items()}
+    ref = orc.observables(orc.make_params(**w.params()), y0, g["y_final"])
+    for k in ("dist", "KE", "transfer"):
+        assert np.max(np.abs(e[k] - ref[k]) / np.maximum(np.abs(ref[k]), 1e-300)) <= 4e-16 * 4, k
+    allobs = dict(g)
+    allobs.update(e)
+    want = orc.outliers(allobs)
+    got = res.cpu().numpy()
+    for r, k in enumerate(aig.OUTLIER_KEYS):
+        assert (int(got[r, 0]), int(got[r, 1])) == want[k], (k, got[r], want[k])
+    # NaNs and ties: poison some lifetimes, flatten the angles
+    out["lifetime"][::3] = float("nan")
+    out["angle"][:] = 1.0
+    got = aig.aig_outliers(out, extra).cpu().numpy()
+    allobs["lifetime"] = out["lifetime"].cpu().numpy()
+    allobs["angle"] = out["angle"].cpu().numpy()
+    want = orc.outliers(allobs)
+    for r, k in enumerate(aig.OUTLIER_KEYS):
+        assert (int(got[r, 0]), int(got[r, 1])) == want[k], k
+    assert tuple(got[0]) == (0, 0)                         # all equal: the first index
+    # N = 0
+    empty = aig.alloc_out(0, torch.device("cuda"))
+    ex0 = {k: torch.empty(0, dtype=torch.float64, device="cuda") for k in ("dist", "KE", "transfer")}
+    assert np.all(aig.aig_outliers(empty, ex0).cpu().numpy() == -1)
+
+
 def test_degenerate_inputs(aig):
     import torch
     w = inputs.config(0)
