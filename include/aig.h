@@ -157,6 +157,18 @@ size_t aig_outliers_workspace_bytes(void);
 int aig_outliers(const aig_out *out, const aig_obs_extra *extra, int64_t N, int64_t *result,
                  void *workspace, void *cuda_stream);
 
+/* ---- NEXT-3: replay of one trajectory, every accepted step recorded ---------------
+ * the paper simulates its longest-lived (or a custom) trajectory again "with
+ * the same exact initial conditions" to display it.  y0: DEVICE [12], one state in the paper's
+ * component order.  Row j (j < cap) of the record is the state after accepted step j + 1:
+ * t_out[j], y_out[k * cap + j] (SoA like y_final).  The integration always runs to its stop;
+ * steps beyond `cap` are not recorded.  n_out: DEVICE int64 [4] = accepted steps, status
+ * (AIG_STATUS_*), failed attempts, counted turning points.  One thread, the arithmetic of
+ * aig_integrate: the last recorded row equals that call's y_final for the same y0 bit for bit.
+ * Data only: no plotting (out of scope). */
+int aig_trace(const aig_params *p, const double *y0, double t_max, double rtol, double atol,
+              int64_t cap, double *t_out, double *y_out, int64_t *n_out, void *cuda_stream);
+
 /* Test hook: ONE attempted DP5(4) step of size h[i] from (t[i], y[:, i]) for each of N
  * states.  DEVICE: y [12][N], t [N], h [N], ynew [12][N] (5th-order solution), err [N]
  * (ode45's scaled error estimate; the step would be accepted iff err <= rtol). */

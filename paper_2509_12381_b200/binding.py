@@ -18,7 +18,7 @@ _lib = None
 
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
            "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_set_schedule", "aig_strerror",
-           "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes"]
+           "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes", "aig_trace"]
 
 
 class AigError(RuntimeError):
@@ -220,6 +220,23 @@ def aig_outliers(obs, extra, stream=None):
     _check(L.aig_outliers(C.byref(o), C.byref(e), N, res.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "aig_outliers")
     res._ws = ws  # keep the scratch alive until the stream has run
     return res
+
+
+def aig_trace(params: Params, y0, t_max, rtol, atol, cap: int = 1 << 20, stream=None):
+    """Replay one trajectory (y0: CUDA float64 [12]); returns (t [cap], y [12, cap], n [4]) CUDA tensors,
+    n = (accepted steps, status, failed attempts, turning points); rows beyond min(n[0], cap) are unset."""
+    torch = _torch()
+    assert y0.is_cuda and y0.dtype == torch.float64 and y0.numel() == 12 and y0.is_contiguous()
+    t = torch.empty(cap, dtype=torch.float64, device=y0.device)
+    y = torch.empty((12, cap), dtype=torch.float64, device=y0.device)
+    n = torch.zeros(4, dtype=torch.int64, device=y0.device)
+    L = lib()
+    L.aig_trace.restype = C.c_int
+    L.aig_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_int64, C.c_void_p,
+                            C.c_void_p, C.c_void_p, C.c_void_p]
+    _check(L.aig_trace(C.byref(params), y0.data_ptr(), t_max, rtol, atol, cap, t.data_ptr(), y.data_ptr(),
+                       n.data_ptr(), _stream_ptr(stream)), "aig_trace")
+    return t, y, n
 
 
 def aig_step_once(params: Params, y, t, h, rtol, atol, stream=None):

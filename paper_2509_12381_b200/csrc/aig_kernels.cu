@@ -687,6 +687,54 @@ histogram_kernel(const HistArgs a, const long long N)
 }
 
 // ------------------------------------------------------------------------------------------
+// NEXT-3: replay of one trajectory with every accepted step recorded
+// ------------------------------------------------------------------------------------------
+// One thread, the same functions as integrate_kernel: the replay is bit-identical to what
+// aig_integrate computed for these initial conditions (the paper recomputes its longest-lived
+// trajectory "with the same exact initial conditions" and gets different bounces, :509).
+template <int TRAP>
+__global__ void __launch_bounds__(32)
+trace_kernel(const KParams P, const double* __restrict__ y0, const long long cap, double* __restrict__ t_out,
+             double* __restrict__ y_out, long long* __restrict__ n_out)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    Traj T;
+    ColdRegs C;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        T.X[k] = y0[0 + k];
+        T.V[k] = y0[3 + k];
+        T.X[3 + k] = y0[6 + k];
+        T.V[3 + k] = y0[9 + k];
+    }
+    init_traj<TRAP>(P, T, C);
+    int st = -1;
+    while (st < 0) {
+        const int before = T.c.n_acc;
+        Attempt R;
+        dp45_attempt<TRAP>(P, T, R);
+        st = finish_attempt(P, T, C, R);
+        if (T.c.n_acc != before) {
+            const long long j = (long long)before;
+            if (j < cap) {
+                t_out[j] = T.c.t;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    y_out[(0 + k) * cap + j] = T.X[k];
+                    y_out[(3 + k) * cap + j] = T.V[k];
+                    y_out[(6 + k) * cap + j] = T.X[3 + k];
+                    y_out[(9 + k) * cap + j] = T.V[3 + k];
+                }
+            }
+        }
+    }
+    n_out[0] = T.c.n_acc;
+    n_out[1] = st;
+    n_out[2] = C.n_rej();
+    n_out[3] = C.n_turn();
+}
+
+// ------------------------------------------------------------------------------------------
 // NEXT-1: the paper's remaining observables and its outliers (:521)
 // ------------------------------------------------------------------------------------------
 // HBM-bound: reads the final state (96 B) and the initial atom velocity (24 B), writes 24 B.
@@ -1308,6 +1356,27 @@ int aig_histogram(const aig_out* obs, int64_t N, const aig_hist_spec* spec, cons
     const long long cap = (long long)sms * 8;
     if (blocks > cap) blocks = cap;
     histogram_kernel<<<(unsigned)blocks, 256, smem, st>>>(a, N);
+    g_kernel_launches++;
+    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
+}
+
+int aig_trace(const aig_params* p, const double* y0, double t_max, double rtol, double atol, int64_t cap,
+              double* t_out, double* y_out, int64_t* n_out, void* cuda_stream)
+{
+    int rc = check_params(p, t_max, rtol, atol);
+    if (rc) return rc;
+    if (cap < 0 || cap > (1LL << 40)) return AIG_ERR_SIZE;
+    if (!y0 || !n_out || (cap > 0 && (!t_out || !y_out))) return AIG_ERR_NULL;
+    if (!aligned(y0, 8) || !aligned(n_out, 8) || !aligned(t_out, 8) || !aligned(y_out, 8)) return AIG_ERR_ALIGN;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const KParams K = make_kparams(p, t_max, rtol, atol);
+    long long* n = reinterpret_cast<long long*>(n_out);
+    switch (trap_mode(p, t_max)) {
+        case TRAP_RF: trace_kernel<TRAP_RF><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        case TRAP_RF_BIG: trace_kernel<TRAP_RF_BIG><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        case TRAP_STATIC: trace_kernel<TRAP_STATIC><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        default: trace_kernel<TRAP_NONE><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+    }
     g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }

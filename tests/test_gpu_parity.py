@@ -388,6 +388,44 @@ def test_observables_and_outliers(aig):
     assert np.all(aig.aig_outliers(empty, ex0).cpu().numpy() == -1)
 
 
+def test_trace_replay(aig):
+    """NEXT-3: the replay of one trajectory (every accepted step recorded) is the trajectory
+    aig_integrate computed -- last row, step counts and status bit for bit, also for the longest-lived
+    one -- and follows the oracle's record step by step on a direct trajectory."""
+    import torch
+    w = inputs.config(2).replace(N=4096)
+    y0 = inputs.generate_y0(w)
+    p = aig.make_params(**w.params())
+    out = aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol)
+    g = _host(out)
+    longest = int(np.argmax(g["lifetime"]))
+    direct = int(np.flatnonzero((g["n_turn"] <= 1) & (g["r_min"] > SHORT_RANGE) & (g["status"] == 0))[0])
+    for i in (longest, direct, 0):
+        t, y, n = aig.aig_trace(p, _dev(y0[:, i].copy()), w.t_max, w.rtol, w.atol, cap=1 << 17)
+        torch.cuda.synchronize()
+        n = n.cpu().numpy()
+        na = int(n[0])
+        assert (na, int(n[1]), int(n[2]), int(n[3])) == (int(g["n_acc"][i]), int(g["status"][i]), int(g["n_rej"][i]),
+                                                         int(g["n_turn"][i]))
+        assert na <= 1 << 17
+        tt, yy = t[:na].cpu().numpy(), y[:, :na].cpu().numpy()
+        assert np.array_equal(yy[:, -1].view(np.uint64), g["y_final"][:, i].view(np.uint64))
+        assert tt[-1] == g["t_final"][i] and np.all(np.diff(tt) > 0)
+    # step by step against the oracle's record on the direct trajectory
+    po = orc.make_params(**w.params())
+    to, yo, st = orc.integrate_trace(po, y0[:, direct], w.t_max, w.rtol, w.atol)
+    t, y, n = aig.aig_trace(p, _dev(y0[:, direct].copy()), w.t_max, w.rtol, w.atol, cap=8192)
+    na = int(n[0].item())
+    assert abs(na - len(to)) <= 2 and st == int(n[1].item())
+    m = min(na, len(to)) - 3                       # the two records share their steps up to rounding
+    tg, yg = t[:m].cpu().numpy(), y[:, :m].cpu().numpy()
+    assert np.max(np.abs(tg / to[:m] - 1)) <= 1e-6
+    assert block_rel(yg, yo[:m].T).max() <= 1e-6
+    # cap smaller than the trajectory: the integration still runs to its stop
+    t, y, n = aig.aig_trace(p, _dev(y0[:, longest].copy()), w.t_max, w.rtol, w.atol, cap=10)
+    assert int(n[0].item()) == int(g["n_acc"][longest])
+
+
 def test_degenerate_inputs(aig):
     import torch
     w = inputs.config(0)
