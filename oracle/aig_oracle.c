@@ -45,6 +45,8 @@ typedef struct orc_params {
     double r_exit;        /* stop when r > r_exit after the first radial minimum; <= 0 disables */
     double r_turn;        /* a radial minimum is a counted turning point only if r < r_turn */
     int64_t max_steps;    /* accepted-step cap */
+    int32_t n_att, n_rep; /* NEXT-1: V(r) = -C_n/r^n + C_m/r^m with n = n_att, C_n = C4,
+                             m = n_rep, C_m = C8; 0, 0 = the benchmark potential n = 4, m = 8 */
 } orc_params;
 
 typedef void (*orc_rhs_fn)(double t, const double *y, double *f, int n, const void *ctx);
@@ -85,7 +87,12 @@ void orc_rhs_atomion(double t, const double *y, double *f, int n, const void *ct
     const double r = sqrt(dx * dx + dy * dy + dz * dz); /* PAPER.md:90 */
     const double r2 = r * r, r4 = r2 * r2;
     const double r5 = r4 * r, r9 = r4 * r4 * r;
-    const double dVdr = 4.0 * p->C4 / r5 - 8.0 * p->C8 / r9; /* PAPER.md:90 */
+    double dVdr = 4.0 * p->C4 / r5 - 8.0 * p->C8 / r9; /* PAPER.md:90 */
+    if (p->n_att != 0 || p->n_rep != 0) {
+        /* general exponents (PAPER.md:51, :428): dV/dr = n C_n / r^(n+1) - m C_m / r^(m+1) */
+        const double n = (double)p->n_att, m = (double)p->n_rep;
+        dVdr = n * p->C4 / pow(r, n + 1.0) - m * p->C8 / pow(r, m + 1.0);
+    }
     const double W2 = p->omega_rf * p->omega_rf / 4.0;
     const double cwt = cos(p->omega_rf * t);
     f[0] = y[3]; /* eq. (3) */

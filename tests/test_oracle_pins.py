@@ -596,3 +596,81 @@ def test_outliers_definition():
     assert all(v == (-1, -1) for v in orc.outliers(allnan).values())
     empty = {k: np.empty(0) for k in orc.OUTLIER_KEYS}
     assert all(v == (-1, -1) for v in orc.outliers(empty).values())
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: general exponents V(r) = -C_n/r^n + C_m/r^m
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("n,m", [(4, 8), (6, 12), (3, 9), (4, 6), (1, 2)])
+def test_general_potential_force_is_minus_grad_V(n, m):
+    """The oracle's force with exponents (n, m) against central finite differences of the V(r) the
+    paper prints, in extended precision; odd exponents included (they need the square root)."""
+    ld = np.longdouble
+    rng = np.random.default_rng(11 + n)
+    Cn, Cm = 37.5, 1.25e3 * 9.0 ** (m - n - 4)
+    p = orc.make_params(3.0, 5.0, Cn, Cm, (0, 0, 0), (0, 0, 0), 0.0, n_att=n, n_rep=m)
+
+    def V(xi, xa):
+        r = np.sqrt(((xi.astype(ld) - xa.astype(ld)) ** 2).sum())
+        return -ld(Cn) / r ** n + ld(Cm) / r ** m
+
+    for trial in range(5):
+        xi = rng.normal(0, 5.0, 3)
+        xa = xi + rng.normal(0, 1.0, 3) * [6.0, 12.0, 40.0][trial % 3]
+        y = np.concatenate([xi, np.zeros(3), xa, np.zeros(3)])
+        f = orc.rhs(p, 0.0, y.reshape(12, 1))[:, 0]
+        d = 1e-4
+        for k in range(3):
+            e = np.zeros(3)
+            e[k] = d
+            gi = float((V(xi + e, xa) - V(xi - e, xa)) / (2 * d))
+            ga = float((V(xi, xa + e) - V(xi, xa - e)) / (2 * d))
+            scale = max(abs(gi), 1e-30)
+            assert abs(f[3 + k] - (-gi / 3.0)) <= 1e-6 * scale / 3.0 + 1e-12 * scale
+            assert abs(f[9 + k] - (-ga / 5.0)) <= 1e-6 * scale / 5.0 + 1e-12 * scale
+
+
+def test_general_potential_reduces_to_the_benchmark_one():
+    """(n, m) = (4, 8) through the general formula equals the printed r^5, r^9 form to rounding, step by
+    step along whole trajectories."""
+    w = inputs.config(1).replace(N=16)
+    y0 = inputs.generate_y0(w)
+    pa = orc.make_params(**w.params())
+    pb = orc.make_params(**w.params(), n_att=4, n_rep=8)
+    a = orc.integrate(pa, y0, w.t_max, w.rtol, w.atol)
+    b = orc.integrate(pb, y0, w.t_max, w.rtol, w.atol)
+    direct = (a["n_turn"] <= 1) & (a["r_min"] > 50)
+    assert direct.sum() >= 4
+    assert np.max(np.abs(a["n_acc"][direct] - b["n_acc"][direct])) <= 1
+    assert np.allclose(a["angle"][direct], b["angle"][direct], rtol=0, atol=1e-9)
+
+
+def test_lennard_jones_6_12_conserves_energy_and_angular_momentum():
+    """(n, m) = (6, 12), trap off: total energy with THAT potential and angular momentum are conserved,
+    and the force vanishes at the textbook minimum r_e = (2 C12 / C6)^(1/6)."""
+    w = inputs.config(1).replace(N=64)
+    y0 = inputs.generate_y0(w)
+    kw = w.params()
+    C6, re = 2.0e4, 12.0
+    C12 = C6 * re ** 6 / 2.0
+    kw.update(C4=C6, C8=C12)
+    p = orc.make_params(**kw, n_att=6, n_rep=12)
+    y = np.zeros((12, 1))
+    y[6, 0] = re
+    assert abs(orc.rhs(p, 0.0, y)[9, 0]) <= 1e-12 * 6 * C6 / re ** 7 / p.m_atom
+    o = orc.integrate(p, y0, w.t_max, 1e-10, 1e-14, threads=4)
+
+    def invariants(y):
+        d = y[6:9] - y[0:3]
+        r = np.linalg.norm(d, axis=0)
+        E = 0.5 * p.m_ion * (y[3:6] ** 2).sum(0) + 0.5 * p.m_atom * (y[9:12] ** 2).sum(0) - C6 / r ** 6 + C12 / r ** 12
+        L = p.m_ion * np.cross(y[0:3].T, y[3:6].T).T + p.m_atom * np.cross(y[6:9].T, y[9:12].T).T
+        return E, L
+
+    E0, L0 = invariants(y0)
+    E1, L1 = invariants(o["y_final"])
+    De = C6 ** 2 / (4 * C12)
+    assert np.max(np.abs(E1 - E0)) <= 1e-7 * De
+    assert np.max(np.abs(L1 - L0)) <= 1e-8 * np.max(np.abs(L0))
+    assert np.all(o["status"] <= 1) and o["n_turn"].max() >= 1
