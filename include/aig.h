@@ -66,6 +66,11 @@ typedef struct aig_params {
     double r_turn;        /* a radial minimum counts as a turning point only if r < r_turn;
                              +inf counts all of them */
     int64_t max_steps;    /* accepted-step cap, paper default 1,000,000 */
+    int32_t n_att, n_rep; /* NEXT-1: general exponents V(r) = -C_n/r^n + C_m/r^m with
+                             n = n_att, C_n = C4, m = n_rep, C_m = C8, 1 <= n < m <= 32; 0, 0 = the
+                             benchmark potential n = 4, m = 8.  Other pairs take a general force
+                             routine (integer powers by repeated squaring, a square root when an
+                             exponent is odd) and the natural work-queue order unless n = 4. */
 } aig_params;
 
 /* Per-trajectory outputs: caller-allocated DEVICE buffers, each of length N

@@ -29,7 +29,7 @@ class Params(C.Structure):
     _fields_ = [("m_ion", C.c_double), ("m_atom", C.c_double), ("C4", C.c_double), ("C8", C.c_double),
                 ("a", C.c_double * 3), ("q", C.c_double * 3), ("omega_rf", C.c_double),
                 ("t0", C.c_double), ("r_exit", C.c_double), ("r_turn", C.c_double),
-                ("max_steps", C.c_int64)]
+                ("max_steps", C.c_int64), ("n_att", C.c_int32), ("n_rep", C.c_int32)]
 
 
 class Out(C.Structure):
@@ -93,8 +93,10 @@ def _check(rc: int, what: str):
 
 
 def make_params(m_ion, m_atom, C4, C8, a, q, omega_rf, t0=0.0, r_exit=0.0, r_turn=math.inf,
-                max_steps=1_000_000) -> Params:
+                max_steps=1_000_000, n_att=0, n_rep=0) -> Params:
+    """n_att, n_rep: exponents of V = -C_n/r^n + C_m/r^m with C_n = C4, C_m = C8 (0, 0 = the 4-8 benchmark potential)."""
     p = Params()
+    p.n_att, p.n_rep = int(n_att), int(n_rep)
     p.m_ion, p.m_atom, p.C4, p.C8 = m_ion, m_atom, C4, C8
     for k in range(3):
         p.a[k] = a[k]

@@ -36,11 +36,20 @@ namespace aig {
 // TRAP_RF_BIG: RF trap with |Omega t| >= kCosMaxArg somewhere in the time span: libdevice cos
 // (Payne-Hanek slow path available); chosen on the host, never needed by BASELINE.json's configs.
 enum TrapMode { TRAP_NONE = 0, TRAP_STATIC = 1, TRAP_RF = 2, TRAP_RF_BIG = 3 };
+// The kernels' template argument `TRAP` is a MODE: trap mode + 4 x potential kind.
+//   potential kind 0: the benchmark potential V = C8/r^8 - C4/r^4, even powers of r only;
+//   potential kind 1: V = C_m/r^m - C_n/r^n with integer exponents (NEXT-1).
+enum PotKind { POT_4_8 = 0, POT_GENERAL = 1 };
+__host__ __device__ constexpr int trap_of(int mode) { return mode & 3; }
+__host__ __device__ constexpr int pot_of(int mode) { return mode >> 2; }
 
 // Derived constants of one call; passed by value as a kernel argument (constant bank).
 struct KParams {
     double g4i, g8i;        // -4 C4/m_ion, +8 C8/m_ion :  -(dV/dr)/(r m_ion)  = (g4i + g8i/r^4)/r^6
     double g4a, g8a;        // +4 C4/m_atom, -8 C8/m_atom : +(dV/dr)/(r m_atom) = (g4a + g8a/r^4)/r^6
+                            // general potential: g4 = -/+ n C_n/m, g8 = +/- m C_m/m
+    int pot_e_att, pot_e_rep;  // general potential: (dV/dr)/r = n C_n b^e_att - m C_m b^e_rep with b = 1/r^2
+    int pot_sqrt;              //   (exponents (n+2)/2, (m+2)/2), or b = 1/r (exponents n+2, m+2) if n or m is odd
     double wa[3], wb[3];    // w_k(t) = wa_k + wb_k cos(Omega t): wa = a_k Om^2/4, wb = q_k Om^2/2
     double omega, half_omega;
     double t0, t_max, hmax; // hmax = 0.1 (t_max - t0)
@@ -93,8 +102,8 @@ __device__ __forceinline__ double cos2_cw(double y)
 template <int TRAP>
 __device__ __forceinline__ double trap_cos(const KParams& P, double t)
 {
-    if (TRAP == TRAP_RF) return cos2_cw(P.half_omega * t);
-    if (TRAP == TRAP_RF_BIG) return cos(P.omega * t);
+    if (trap_of(TRAP) == TRAP_RF) return cos2_cw(P.half_omega * t);
+    if (trap_of(TRAP) == TRAP_RF_BIG) return cos(P.omega * t);
     return 1.0;
 }
 
@@ -120,20 +129,42 @@ __device__ __forceinline__ double dmin(double a, double b)
 
 // gi = -(dV/dr)/(r m_ion) and ga = +(dV/dr)/(r m_atom) from r^2, (dV/dr)/r = 4 C4/r^6 - 8 C8/r^10:
 // the masses are folded into the constants so that both factors are three operations behind 1/r^2
+// x^e for an integer e >= 1 by repeated squaring; the order of the products is fixed by e alone
+__device__ __forceinline__ double ipow(double x, int e)
+{
+    double r = 1.0, b = x;
+    for (;;) {
+        if (e & 1) r *= b;
+        e >>= 1;
+        if (e == 0) break;
+        b *= b;
+    }
+    return r;
+}
+template <int MODE>
 __device__ __forceinline__ void force_factors(const KParams& P, double r2, double& gi, double& ga)
 {
     const double inv2 = rcp_nr(r2);
-    const double inv4 = inv2 * inv2;
-    const double inv6 = inv4 * inv2;
-    gi = inv6 * fma(P.g8i, inv4, P.g4i);
-    ga = inv6 * fma(P.g8a, inv4, P.g4a);
+    if (pot_of(MODE) == POT_4_8) {
+        const double inv4 = inv2 * inv2;
+        const double inv6 = inv4 * inv2;
+        gi = inv6 * fma(P.g8i, inv4, P.g4i);
+        ga = inv6 * fma(P.g8a, inv4, P.g4a);
+    } else {
+        // V = C_m/r^m - C_n/r^n: (dV/dr)/r = n C_n/r^(n+2) - m C_m/r^(m+2), powers of 1/r^2 (or of 1/r
+        // when an exponent is odd: one square root)
+        const double b = P.pot_sqrt ? sqrt(inv2) : inv2;
+        const double pa = ipow(b, P.pot_e_att), pr = ipow(b, P.pot_e_rep);
+        gi = fma(P.g8i, pr, P.g4i * pa);
+        ga = fma(P.g8a, pr, P.g4a * pa);
+    }
 }
 
 // trap stiffness of one axis at cos(Omega t) = cs: w = wa + wb cs
 template <int TRAP>
 __device__ __forceinline__ double trap_w(double wa, double wb, double cs)
 {
-    return (TRAP == TRAP_STATIC) ? wa : fma(wb, cs, wa);
+    return (trap_of(TRAP) == TRAP_STATIC) ? wa : fma(wb, cs, wa);
 }
 
 // Accelerations of both particles at positions (xi, xa), cos(Omega t) = cs.
@@ -146,11 +177,11 @@ __device__ __forceinline__ void accel(const KParams& P, double cs, const double 
     const double d0 = X[0] - X[3], d1 = X[1] - X[4], d2 = X[2] - X[5];
     const double r2 = sum3(d0 * d0, d1 * d1, d2 * d2);
     double gi, ga;
-    force_factors(P, r2, gi, ga);
+    force_factors<TRAP>(P, r2, gi, ga);
     Aout[3] = ga * d0;
     Aout[4] = ga * d1;
     Aout[5] = ga * d2;
-    if (TRAP == TRAP_NONE) {
+    if (trap_of(TRAP) == TRAP_NONE) {
         Aout[0] = gi * d0;
         Aout[1] = gi * d1;
         Aout[2] = gi * d2;

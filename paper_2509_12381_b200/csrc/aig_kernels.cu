@@ -578,9 +578,10 @@ step_once_kernel(const KParams P, const double* __restrict__ y, const double* __
     Attempt R;
     // RF trap: the branch-free cos where it is valid, libdevice's beyond (the integrator makes
     // this choice once per call on the host, from t0 and t_max)
-    if (TRAP == TRAP_RF && !(fabs(P.omega) * (fabs(T.c.t) + fabs(T.c.h)) < 0.99 * kCosMaxArg)) {
-        accel<TRAP_RF_BIG>(P, trap_cos<TRAP_RF_BIG>(P, T.c.t), T.X, T.A1, r2);
-        dp45_attempt<TRAP_RF_BIG>(P, T, R);
+    if (trap_of(TRAP) == TRAP_RF && !(fabs(P.omega) * (fabs(T.c.t) + fabs(T.c.h)) < 0.99 * kCosMaxArg)) {
+        constexpr int BIG = TRAP_RF_BIG + 4 * pot_of(TRAP);
+        accel<BIG>(P, trap_cos<BIG>(P, T.c.t), T.X, T.A1, r2);
+        dp45_attempt<BIG>(P, T, R);
     } else {
         accel<TRAP>(P, trap_cos<TRAP>(P, T.c.t), T.X, T.A1, r2);
         dp45_attempt<TRAP>(P, T, R);
@@ -904,6 +905,7 @@ int check_params(const aig_params* p, double t_max, double rtol, double atol)
     for (int k = 0; k < 3; ++k)
         if (!finite(p->a[k]) || !finite(p->q[k])) return AIG_ERR_PARAM;
     if (p->max_steps < 1) return AIG_ERR_PARAM;
+    if (!(p->n_att == 0 && p->n_rep == 0) && !(p->n_att >= 1 && p->n_att < p->n_rep && p->n_rep <= 32)) return AIG_ERR_PARAM;
     if (std::isnan(p->r_exit) || std::isnan(p->r_turn)) return AIG_ERR_PARAM;
     return AIG_OK;
 }
@@ -922,13 +924,23 @@ int trap_mode(const aig_params* p, double t_max)
     return (phase < 0.99 * kCosMaxArg) ? TRAP_RF : TRAP_RF_BIG;
 }
 
+// potential kind: 0, 0 (or 4, 8) = the benchmark potential's fast path, anything else the general one
+bool general_potential(const aig_params* p)
+{
+    return !((p->n_att == 0 && p->n_rep == 0) || (p->n_att == 4 && p->n_rep == 8));
+}
+
 KParams make_kparams(const aig_params* p, double t_max, double rtol, double atol)
 {
     KParams K;
-    K.g4i = -4.0 * p->C4 / p->m_ion;
-    K.g8i = 8.0 * p->C8 / p->m_ion;
-    K.g4a = 4.0 * p->C4 / p->m_atom;
-    K.g8a = -8.0 * p->C8 / p->m_atom;
+    const int n = p->n_att ? p->n_att : 4, m = p->n_rep ? p->n_rep : 8;
+    K.g4i = -(double)n * p->C4 / p->m_ion;
+    K.g8i = (double)m * p->C8 / p->m_ion;
+    K.g4a = (double)n * p->C4 / p->m_atom;
+    K.g8a = -(double)m * p->C8 / p->m_atom;
+    K.pot_sqrt = ((n | m) & 1) ? 1 : 0;
+    K.pot_e_att = K.pot_sqrt ? n + 2 : (n + 2) / 2;
+    K.pot_e_rep = K.pot_sqrt ? m + 2 : (m + 2) / 2;
     const double w2 = p->omega_rf * p->omega_rf;
     for (int k = 0; k < 3; ++k) {
         K.wa[k] = p->a[k] * w2 / 4.0;
@@ -1126,7 +1138,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     int rc = bulk_capacity<TRAP>(&bps, &sms);
     if (rc) return rc;
     const long long blocks = std::min((long long)bps * sms, (N + kBlock - 1) / kBlock);
-    const bool plan = cfg.plan != 0 && p->C4 > 0.0;
+    const bool plan = cfg.plan != 0 && p->C4 > 0.0 && (p->n_att == 0 || p->n_att == 4);  // the Langevin test is the r^-4 tail's
     // stages: the three classes of the plan; without a plan one stage over [0, N)
     const int stages = plan ? 3 : 1;
     SideStreams* side = stages > 1 ? side_streams() : nullptr;
@@ -1278,11 +1290,15 @@ int aig_integrate(const aig_params* p, const double* y0, int64_t N, double t_max
     const KParams K = make_kparams(p, t_max, rtol, atol);
     OutPtrs O{out->y_final, out->t_final, out->lifetime, out->angle, out->r_min,
               out->n_acc,   out->n_rej,   out->n_turn,   out->status, out->complex_flag};
-    switch (trap_mode(p, t_max)) {
+    switch (trap_mode(p, t_max) + 4 * (general_potential(p) ? POT_GENERAL : POT_4_8)) {
         case TRAP_RF: return launch_integrate<TRAP_RF>(p, K, y0, N, O, workspace, st);
         case TRAP_RF_BIG: return launch_integrate<TRAP_RF_BIG>(p, K, y0, N, O, workspace, st);
         case TRAP_STATIC: return launch_integrate<TRAP_STATIC>(p, K, y0, N, O, workspace, st);
-        default: return launch_integrate<TRAP_NONE>(p, K, y0, N, O, workspace, st);
+        case TRAP_NONE: return launch_integrate<TRAP_NONE>(p, K, y0, N, O, workspace, st);
+        case 4 + TRAP_RF: return launch_integrate<4 + TRAP_RF>(p, K, y0, N, O, workspace, st);
+        case 4 + TRAP_RF_BIG: return launch_integrate<4 + TRAP_RF_BIG>(p, K, y0, N, O, workspace, st);
+        case 4 + TRAP_STATIC: return launch_integrate<4 + TRAP_STATIC>(p, K, y0, N, O, workspace, st);
+        default: return launch_integrate<4 + TRAP_NONE>(p, K, y0, N, O, workspace, st);
     }
 }
 
@@ -1301,11 +1317,15 @@ int aig_step_once(const aig_params* p, const double* y, const double* t, const d
     KParams K = make_kparams(p, p->t0 + 1.0, rtol, atol);
     K.t_max = INFINITY;
     const unsigned blocks = (unsigned)((N + kBlock - 1) / kBlock);
-    switch (trap_mode(p, p->t0 + 1.0)) {
+    switch (trap_mode(p, p->t0 + 1.0) + 4 * (general_potential(p) ? POT_GENERAL : POT_4_8)) {
         case TRAP_RF_BIG:
         case TRAP_RF: step_once_kernel<TRAP_RF><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
         case TRAP_STATIC: step_once_kernel<TRAP_STATIC><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
-        default: step_once_kernel<TRAP_NONE><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
+        case TRAP_NONE: step_once_kernel<TRAP_NONE><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
+        case 4 + TRAP_RF_BIG:
+        case 4 + TRAP_RF: step_once_kernel<4 + TRAP_RF><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
+        case 4 + TRAP_STATIC: step_once_kernel<4 + TRAP_STATIC><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
+        default: step_once_kernel<4 + TRAP_NONE><<<blocks, kBlock, 0, st>>>(K, y, t, h, N, ynew, err); break;
     }
     g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
@@ -1371,11 +1391,15 @@ int aig_trace(const aig_params* p, const double* y0, double t_max, double rtol, 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const KParams K = make_kparams(p, t_max, rtol, atol);
     long long* n = reinterpret_cast<long long*>(n_out);
-    switch (trap_mode(p, t_max)) {
+    switch (trap_mode(p, t_max) + 4 * (general_potential(p) ? POT_GENERAL : POT_4_8)) {
         case TRAP_RF: trace_kernel<TRAP_RF><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
         case TRAP_RF_BIG: trace_kernel<TRAP_RF_BIG><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
         case TRAP_STATIC: trace_kernel<TRAP_STATIC><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
-        default: trace_kernel<TRAP_NONE><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        case TRAP_NONE: trace_kernel<TRAP_NONE><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        case 4 + TRAP_RF: trace_kernel<4 + TRAP_RF><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        case 4 + TRAP_RF_BIG: trace_kernel<4 + TRAP_RF_BIG><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        case 4 + TRAP_STATIC: trace_kernel<4 + TRAP_STATIC><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
+        default: trace_kernel<4 + TRAP_NONE><<<1, 32, 0, st>>>(K, y0, cap, t_out, y_out, n); break;
     }
     g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;

@@ -130,15 +130,15 @@ __device__ __forceinline__ double level_close(const KParams& P, const SplitRole&
                                               double mycos, double (&Ai)[7], double (&Aa)[7])
 {
     double trap = 0.0;
-    if (TRAP != TRAP_NONE) {
-        const double cs = (TRAP == TRAP_STATIC) ? 1.0 : shfl_d(mycos, R.base + 2 * LEV + R.e);
+    if (trap_of(TRAP) != TRAP_NONE) {
+        const double cs = (trap_of(TRAP) == TRAP_STATIC) ? 1.0 : shfl_d(mycos, R.base + 2 * LEV + R.e);
         trap = -(trap_w<TRAP>(R.wa, R.wb, cs) * L.xsi);
     }
     const double r2 = sum3(L.s0, L.s1, L.s2);
     double gi, ga;
-    force_factors(P, r2, gi, ga);
+    force_factors<TRAP>(P, r2, gi, ga);
     const double myAa = ga * L.d;
-    const double myAi = (TRAP == TRAP_NONE) ? gi * L.d : fma(gi, L.d, trap);
+    const double myAi = (trap_of(TRAP) == TRAP_NONE) ? gi * L.d : fma(gi, L.d, trap);
     const double pAi = shfl_xor_d(myAi, 1);
     const double pAa = shfl_xor_d(myAa, 1);
     Ai[2 * LEV + 1] = R.e ? pAi : myAi;
@@ -167,7 +167,7 @@ __device__ __forceinline__ void split_attempt(const KParams& P, const SplitRole&
     level_open<0>(R, Y, h, h2, Ai, Aa, L);
     // the cos of my stage time, inside the first level's shuffle and reciprocal latency
     double mycos = 1.0;
-    if (TRAP == TRAP_RF || TRAP == TRAP_RF_BIG) mycos = trap_cos<TRAP>(P, R.cos_end ? ST.t_new : fma(R.cCos, h, K.t));
+    if (trap_of(TRAP) == TRAP_RF || trap_of(TRAP) == TRAP_RF_BIG) mycos = trap_cos<TRAP>(P, R.cos_end ? ST.t_new : fma(R.cCos, h, K.t));
     level_close<TRAP, 0>(P, R, L, mycos, Ai, Aa);
     level_open<1>(R, Y, h, h2, Ai, Aa, L);
     level_close<TRAP, 1>(P, R, L, mycos, Ai, Aa);

@@ -49,11 +49,16 @@ def test_version_strerror_workspace(lib):
     assert lib.aig_set_schedule(256, 2048, 32, 8, 1, 1.25) == 0
     assert lib.aig_set_schedule(256, 0, 32, 8, 1, 1.25) == -5
     assert lib.aig_set_schedule(-1, 2048, 32, 8, 1, 1.25) == -5
+    # potential exponents: 0, 0 (the benchmark 4-8) or 1 <= n < m <= 32
+    for n, m, rc in ((0, 0, -1), (6, 12, -1), (3, 9, -1), (8, 4, -5), (4, 4, -5), (0, 8, -5), (4, 40, -5)):
+        p = binding.make_params(1.0, 1.0, 1.0, 1.0, (0, 0, 0), (0, 0, 0), 0.0, n_att=n, n_rep=m)
+        assert lib.aig_integrate(C.byref(p), None, 4, 1.0, 1e-6, 1e-9, None, None, None) == rc, (n, m)
 
 
 def test_struct_layouts_match_header():
     # aig_params: 13 doubles + int64 ; aig_out: 10 pointers ; aig_hist_spec: ptr,i32,ptr,i32,i32
-    assert C.sizeof(binding.Params) == 15 * 8 + 8 - 8  # 14 doubles (2+2+3+3+1+1+1+1) + int64
+    assert C.sizeof(binding.Params) == 14 * 8 + 8 + 8  # 14 doubles (2+2+3+3+1+1+1+1) + int64 + 2 int32
+    assert binding.Params.n_att.offset == 15 * 8 and binding.Params.n_rep.offset == 15 * 8 + 4
     assert binding.Params.max_steps.offset == 14 * 8
     assert C.sizeof(binding.Out) == 10 * C.sizeof(C.c_void_p)
     assert binding.HistSpec.life_edges.offset == 16 and binding.HistSpec.n_turn_bins.offset == 28

@@ -426,6 +426,62 @@ def test_trace_replay(aig):
     assert int(n[0].item()) == int(g["n_acc"][longest])
 
 
+def _lj_workload(n_att, n_rep, trap):
+    """Config 1 (trap off, two-body) or config 0 (RF trap) geometry with a Lennard-Jones-type potential
+    of exponents (n_att, n_rep) whose well sits at r_e = 12 a0 with the depth of the benchmark one."""
+    w = inputs.config(0 if trap else 1)
+    kw = w.params()
+    re, De = 12.0, kw["C4"] ** 2 / (4 * kw["C8"])
+    # V = -Cn/r^n + Cm/r^m with minimum -De at re:  Cn = De m re^n / (m - n), Cm = De n re^m / (m - n)
+    kw["C4"] = De * n_rep * re ** n_att / (n_rep - n_att)
+    kw["C8"] = De * n_att * re ** n_rep / (n_rep - n_att)
+    kw.update(n_att=n_att, n_rep=n_rep)
+    return w, kw
+
+
+@pytest.mark.parametrize("n_att,n_rep,trap", [(6, 12, False), (3, 9, True), (4, 6, True), (4, 8, True)])
+def test_general_potential(aig, n_att, n_rep, trap):
+    """NEXT-1: V = -C_n/r^n + C_m/r^m through the general force routine (even and odd
+    exponents, with and without the RF trap): one step and whole trajectories against the oracle, and
+    bit-identical results from the per-thread and the six-lane kernel."""
+    w, kw = _lj_workload(n_att, n_rep, trap)
+    n = 1500 + 7
+    y0 = inputs.generate_y0(w, n=n)
+    po, pg = orc.make_params(**kw), aig.make_params(**kw)
+    # one attempted step from states along real trajectories of THIS potential
+    ys, ts, hs = [], [], []
+    for i in range(40):
+        tt, yy, _ = orc.integrate_trace(po, y0[:, i], w.t_max, w.rtol, w.atol, cap=4000)
+        for j in range(1, len(tt) - 1, max(1, len(tt) // 8)):
+            ys.append(yy[j]); ts.append(tt[j]); hs.append(tt[j + 1] - tt[j])
+    y, t, h = np.ascontiguousarray(np.array(ys).T), np.array(ts), np.array(hs)
+    yo, eo = orc.step_once(po, y, t, h, w.rtol, w.atol)
+    yg, eg = aig.aig_step_once(pg, _dev(y), _dev(t), _dev(h), w.rtol, w.atol)
+    rel = block_rel(yg.cpu().numpy(), yo, ref_extra=y)
+    assert np.all(rel <= 4 * step_tolerance(y)), (rel / step_tolerance(y)).max()   # pow() vs repeated squaring: a few ulp
+    assert np.mean(rel <= 1e-14) > 0.85
+    # whole trajectories
+    g = _host(aig.aig_integrate(pg, _dev(y0), w.t_max, w.rtol, w.atol))
+    o = orc.integrate(po, y0, w.t_max, w.rtol, w.atol, threads=8)
+    ws = w.replace(N=n)
+    direct = (o["n_turn"] <= 1) & (g["n_turn"] <= 1) & (o["status"] == 0) & (g["status"] == 0) & (o["r_min"] > SHORT_RANGE)
+    assert direct.sum() > 0.1 * n
+    assert np.max(np.abs(g["n_acc"][direct].astype(int) - o["n_acc"][direct].astype(int))) <= 2
+    yo_s = o["y_final"] + (g["t_final"] - o["t_final"]) * orc.rhs(po, o["t_final"], o["y_final"])
+    assert block_rel(g["y_final"], yo_s)[direct].max() <= 1e-6
+    assert np.max(np.abs(g["angle"][direct] - o["angle"][direct])) <= 1e-6
+    assert abs(g["complex_flag"].mean() - o["complex_flag"].mean()) <= 3 * math.sqrt(0.25 / n) + 1e-9
+    # the six-lane kernel computes the same bits
+    try:
+        aig.set_schedule(plan=0, budget=1, tail_iters=0)
+        g2 = _host(aig.aig_integrate(pg, _dev(y0), w.t_max, w.rtol, w.atol))
+    finally:
+        aig.set_schedule()
+    for k in g:
+        assert np.array_equal(g[k].view(np.uint8), g2[k].view(np.uint8)), k
+    del ws
+
+
 def test_degenerate_inputs(aig):
     import torch
     w = inputs.config(0)
