@@ -102,6 +102,13 @@ def potential_CnDe(n: int, m: int, Cn: float, De: float):
     return Cm, Re
 
 
+def potential_DeRe(n: int, m: int, De: float, Re: float):
+    """'DeRe' front-end of PAPER.md:428: given the well depth De and the equilibrium distance Re of
+    V = -Cn/r^n + Cm/r^m, return (Cn, Cm).  From V'(Re) = 0 and V(Re) = -De:
+    Cn = De m Re^n / (m - n),  Cm = De n Re^m / (m - n)."""
+    return De * m * Re ** n / (m - n), De * n * Re ** m / (m - n)
+
+
 def config(i: int, **overrides) -> Workload:
     """The five BASELINE.json configs (index 0..4).  Config 4's sweep point is chosen with
     ``q=...``/``rtol=...`` overrides (atol follows as rtol*1e-2 unless given)."""

@@ -76,3 +76,15 @@ def test_prefix_and_offset_reproducibility_and_sharding():
         assert all(spans[i][1] == spans[i + 1][0] for i in range(world - 1))
         sizes = [hi - lo for lo, hi in spans]
         assert max(sizes) - min(sizes) <= 1
+
+
+def test_potential_front_ends_are_consistent():
+    """'CnCm', 'CnDe', 'DeRe' describe the same V = -Cn/r^n + Cm/r^m."""
+    for n, m, De, Re in ((4, 8, 0.012, 9.0), (6, 12, 3e-4, 12.0), (3, 9, 0.5, 2.5)):
+        Cn, Cm = inputs.potential_DeRe(n, m, De, Re)
+        V = lambda r: -Cn / r ** n + Cm / r ** m
+        assert abs(V(Re) + De) <= 1e-14 * De                       # depth
+        h = 1e-5 * Re
+        assert abs(V(Re + h) - V(Re - h)) <= 1e-9 * De             # minimum at Re
+        Cm2, Re2 = inputs.potential_CnDe(n, m, Cn, De)             # and back through 'CnDe'
+        assert abs(Cm2 / Cm - 1) <= 1e-13 and abs(Re2 / Re - 1) <= 1e-13
