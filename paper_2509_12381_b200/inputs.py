@@ -150,6 +150,30 @@ def config(i: int, **overrides) -> Workload:
     return w.replace(**overrides) if overrides else w
 
 
+def paper_workload(ntheta: int = 50, nphi: int = 50, theta=(0.0, math.pi / 2), phi=(0.0, math.pi / 2),
+                   **overrides) -> Workload:
+    """NEXT-2: the paper's OWN workload (not a BASELINE.json config): Yb+ + Rb, the atom launched head-on
+    at fixed speed v0 = sqrt(3 k_B T / m_a) from an equal-solid-angle (theta, phi) grid on the sphere
+    r0 = 5000 a0 towards an ion at rest at the centre of a linear Paul trap, integrated for 1 ms with no
+    exit radius (parameter listing Fig. 10 at :291-345).  Default grid: the
+    50 x 50 first-octant benchmark of :102, :116.  The listing is partly garbled in the text
+    (reading S28): taken here are
+      m_ion 170.936323 amu, m_atom 86.9091805310 amu, T_atom 1 uK; potential 'CnDe' n = 4, m = 8,
+      C4 = 159.5455, De = 1 K k_B  =>  C8 = 2.00949488627505e9, Re = 70.84 a0 (both printed);
+      ax = ay = -2.982e-4, az = -2 ax, qx = 0.219, qy = -qx, qz = 0, Omega = 2 pi 2.5 MHz;
+      tmax = 1000 us, maxsteps 1e6, rtol 1e-10, atol 1e-20.
+    A radial minimum counts as a bounce inside r_turn = 500 a0 (the paper gives no formula)."""
+    Cm, _Re = potential_CnDe(4, 8, 159.5455, 1.0 * KB)
+    ax = -2.982e-4
+    w = Workload(name="paper", N=int(ntheta) * int(nphi), seed=0, kind="grid",
+                 m_ion=170.936323 * AMU, m_atom=86.9091805310 * AMU, C4=159.5455, C8=Cm,
+                 a=(ax, ax, -2.0 * ax), q=(0.219, -0.219, 0.0), omega_rf=omega_from_mhz(2.5),
+                 r_exit=0.0, r_turn=500.0, max_steps=1_000_000,
+                 t_max=1000e-6 / AU_TIME_S, rtol=1e-10, atol=1e-20, T_ion=0.0, T_atom=1.0e-6, R0=5000.0, b_max=0.0,
+                 notes=dict(ntheta=int(ntheta), nphi=int(nphi), theta=tuple(theta), phi=tuple(phi)))
+    return w.replace(**overrides) if overrides else w
+
+
 def uniforms(seed: int, n: int, offset: int = 0) -> np.ndarray:
     """Rows [offset, offset+n) of the (N, 10) uniform matrix of stream ``seed``."""
     bg = np.random.PCG64(seed)
@@ -162,6 +186,8 @@ def generate_y0(w: Workload, n: int | None = None, offset: int = 0) -> np.ndarra
     """Initial conditions ``y0[12][n]`` (float64, C-contiguous) for trajectories
     offset .. offset+n-1 of workload ``w`` (default: all ``w.N``)."""
     n = w.N if n is None else int(n)
+    if w.kind == "grid":
+        return _grid_y0(w, n, offset)
     U = uniforms(w.seed, n, offset)
     y0 = np.zeros((12, n), dtype=np.float64)
     two_pi = 2.0 * math.pi
@@ -203,6 +229,31 @@ def generate_y0(w: Workload, n: int | None = None, offset: int = 0) -> np.ndarra
         y0[9:12] = (w.m_ion / M) * vrel
     else:
         raise ValueError(w.kind)
+    return np.ascontiguousarray(y0)
+
+
+def grid_angles(w: Workload):
+    """(theta[ntheta], phi[nphi]) of a "grid" workload (positions = "uniform"): nphi evenly
+    spaced phi between phimin and phimax; theta = arccos(1 - 2u) with ntheta evenly spaced u between
+    (1 - cos thetamin)/2 and (1 - cos thetamax)/2, so that every (theta, phi) occupies the same solid angle."""
+    nt, nph = w.notes["ntheta"], w.notes["nphi"]
+    (t0, t1), (p0, p1) = w.notes["theta"], w.notes["phi"]
+    u = np.linspace((1.0 - math.cos(t0)) / 2.0, (1.0 - math.cos(t1)) / 2.0, nt)
+    return np.arccos(1.0 - 2.0 * u), np.linspace(p0, p1, nph)
+
+
+def _grid_y0(w: Workload, n: int, offset: int) -> np.ndarray:
+    """eq. (12)-(13): atom at r0 (sin th cos ph, sin th sin ph, cos th) with velocity
+    -v0 times the same unit vector, v0 = sqrt(3 k_B T / m_a); ion at rest at the origin.  Trajectory
+    i <-> (theta index i // nphi, phi index i % nphi)."""
+    th, ph = grid_angles(w)
+    idx = np.arange(offset, offset + n)
+    t, f = th[idx // len(ph)], ph[idx % len(ph)]
+    nhat = np.stack([np.sin(t) * np.cos(f), np.sin(t) * np.sin(f), np.cos(t)])
+    v0 = math.sqrt(3.0 * KB * w.T_atom / w.m_atom)
+    y0 = np.zeros((12, n), dtype=np.float64)
+    y0[6:9] = w.R0 * nhat
+    y0[9:12] = -v0 * nhat
     return np.ascontiguousarray(y0)
 
 

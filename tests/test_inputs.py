@@ -88,3 +88,22 @@ def test_potential_front_ends_are_consistent():
         assert abs(V(Re + h) - V(Re - h)) <= 1e-9 * De             # minimum at Re
         Cm2, Re2 = inputs.potential_CnDe(n, m, Cn, De)             # and back through 'CnDe'
         assert abs(Cm2 / Cm - 1) <= 1e-13 and abs(Re2 / Re - 1) <= 1e-13
+
+
+def test_paper_grid_workload():
+    """NEXT-2: head-on launch from an equal-solid-angle grid."""
+    w = inputs.paper_workload(ntheta=40, nphi=30)
+    y0 = inputs.generate_y0(w)
+    assert y0.shape == (12, 1200) and np.all(y0[0:6] == 0)                  # ion at rest at the origin
+    r = np.linalg.norm(y0[6:9], axis=0)
+    v = np.linalg.norm(y0[9:12], axis=0)
+    assert np.allclose(r, 5000.0, rtol=1e-15)
+    assert np.allclose(v, math.sqrt(3 * inputs.KB * 1e-6 / w.m_atom), rtol=1e-15)
+    assert np.allclose(y0[9:12] / v, -y0[6:9] / r, atol=1e-15)              # head-on
+    th, ph = inputs.grid_angles(w)
+    assert np.allclose(np.diff(np.cos(th)), np.diff(np.cos(th))[0])         # equal steps in cos(theta): equal solid angle
+    assert np.allclose(np.diff(ph), np.diff(ph)[0]) and th[0] == 0 and abs(th[-1] - math.pi / 2) < 1e-12
+    assert np.array_equal(inputs.generate_y0(w, n=7, offset=95), y0[:, 95:102])   # slices reproduce
+    # the paper's printed derived constants (Fig. 10): Cm and tmax
+    assert abs(w.C8 / 2.00949488627505397797e+09 - 1) < 1e-13
+    assert abs(w.t_max * inputs.AU_TIME_S - 1e-3) < 1e-15
