@@ -180,7 +180,10 @@ __device__ __forceinline__ void ckpt_store(const Ckpt& K, long long slot, long l
 // `out`) when it has taken `budget` accepted steps -- as long as this stage has handed over fewer
 // than `soft_cap` trajectories (the six-lane integrator has half the throughput per FP64
 // operation: it is for the few, not for the many; a trajectory that is kept is asked again one
-// budget later) -- or `tail_iters` iterations after its warp has seen the queue empty; when the
+// budget later), and only once it is `mean_factor` times longer than the mean of the trajectories
+// this launch has finished (a workload where every trajectory is long is the per-thread kernel's
+// job: nothing is handed over before 32 have finished) -- or when, `tail_iters` iterations after its
+// warp has seen the queue empty, the warp has `drain_lanes` or fewer trajectories left; when the
 // slots are exhausted it simply keeps stepping.  Suspension never changes a trajectory's
 // arithmetic, only where it continues.
 struct Sched {
@@ -194,6 +197,9 @@ struct Sched {
     int budget;
     int tail_iters;
     int refill_batch, refill_wait;
+    int drain_lanes;            // after the queue ran dry a warp hands its trajectories over once it has this few left
+    unsigned long long* stats;  // [0] accepted steps, [1] number of the trajectories this launch has finished
+    int mean_factor;            // hand over only beyond mean_factor x their mean (0: the plain budget)
     unsigned long long* timeline;
 };
 
@@ -231,6 +237,16 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
         const unsigned need = __ballot_sync(FULL, !live);
         if (need && (__popc(need) >= S.refill_batch || waited >= S.refill_wait || dry)) {
             waited = 0;
+            {   // accepted steps and count of what this warp has finished since its last service
+                const unsigned fm = __ballot_sync(FULL, pending >= 0);
+                if (fm) {
+                    const unsigned steps = __reduce_add_sync(FULL, pending >= 0 ? (unsigned)T.c.n_acc : 0u);
+                    if (lane == 0) {
+                        atomicAdd(S.stats + 0, (unsigned long long)steps);
+                        atomicAdd(S.stats + 1, (unsigned long long)__popc(fm));
+                    }
+                }
+            }
             if (pending >= 0) {
                 const double v0[3] = {s_v0[0][threadIdx.x], s_v0[1][threadIdx.x], s_v0[2][threadIdx.x]};
                 store_traj(v0, N, idx, T, C, pending, O);
@@ -260,6 +276,9 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
         } else if (need) {
             ++waited;
         }
+        // warp-uniform: the queue is empty, the grace period is over and few lanes are still alive: at
+        // fewer than ~11 lanes the six-lane kernel does more steps per SM and second than this one
+        const bool drain = dry && since_dry > S.tail_iters && (32 - __popc(need)) <= S.drain_lanes;
         if (dry) ++since_dry;
         // ---- one attempted step for every live lane
         if (live) {
@@ -269,11 +288,18 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
             if (st >= 0) {
                 pending = st;
                 live = false;
-            } else if (may_suspend && (T.c.n_acc >= stop_at || since_dry > S.tail_iters)) {
+            } else if (may_suspend && (T.c.n_acc >= stop_at || drain)) {
                 bool room = true;
-                if (since_dry <= S.tail_iters) {  // budget hand-over: only while the six-lane queue is short
+                if (!drain) {
+                    // budget hand-over: only while the six-lane queue is short, and only for a trajectory
+                    // that is long compared with what this launch has finished so far
                     const long long used = (long long)(*(volatile unsigned long long*)S.n_out) - soft_first;
                     room = used < S.soft_cap;
+                    if (room && S.mean_factor > 0) {
+                        const unsigned long long cnt = *(volatile unsigned long long*)(S.stats + 1);
+                        const unsigned long long sum = *(volatile unsigned long long*)(S.stats + 0);
+                        room = (cnt >= 32ULL) && ((unsigned long long)T.c.n_acc * cnt >= (unsigned long long)S.mean_factor * sum);
+                    }
                     if (!room) stop_at += S.budget;
                 }
                 if (room) {
@@ -292,10 +318,14 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
 }
 
 // ---- six lanes per trajectory: continues the slots [*begin, min(*end, cap)) of `in` to their end
+// nq queues, served in this order: the pass's own slot range first, then the ranges of the stages
+// before it (their bulk passes are complete, so their slots are too): a pass that runs out of work
+// helps drain what an earlier, smaller pass is still working through.
 struct SplitSched {
     unsigned long long* timeline;
-    unsigned long long* queue;
-    const unsigned long long *begin, *end;
+    int nq;
+    unsigned long long* queue[4];
+    const unsigned long long *begin[4], *end[4];
     Ckpt in;
 };
 
@@ -308,9 +338,14 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
     const int lane = threadIdx.x & 31;
     const SplitRole R = make_role(P);
     const bool leader = !R.ghost && (lane == R.base);
-    const long long first = (long long)*S.begin;
-    const long long last = (long long)((*S.end < (unsigned long long)S.in.cap) ? *S.end : (unsigned long long)S.in.cap);
-    const long long total = last - first;
+    int qi = 0;  // warp-uniform: the queue being served
+    long long first = 0, total = 0;
+    auto open_queue = [&]() {
+        const unsigned long long e = *S.end[qi];
+        first = (long long)*S.begin[qi];
+        total = (long long)(e < (unsigned long long)S.in.cap ? e : (unsigned long long)S.in.cap) - first;
+    };
+    open_queue();
     // benign state for lanes without a trajectory (they take part in every shuffle)
     SplitState Y;
     Y.xi = 1.0 + R.k;
@@ -327,15 +362,22 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
     C.n_rej_ = C.n_turn_ = 0;
     long long idx = -1;
     bool live = false;
-    bool dry = (total <= 0);
+    bool dry = false;  // warp-uniform: every queue has been seen empty
 
     // refill: every idle group takes the next slot of the queue (one atomicAdd per warp)
-    auto refill = [&]() {
+    auto refill_once = [&]() -> bool {   // returns true when another round may place more groups
         const unsigned need = __ballot_sync(FULL, leader && !live);
-        if (need == 0u || dry) return;
+        if (need == 0u || dry) return false;
+        while (total <= 0) {  // skip empty ranges
+            if (++qi >= S.nq) {
+                dry = true;
+                return false;
+            }
+            open_queue();
+        }
         const int cnt = __popc(need);
         unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(S.queue, (unsigned long long)cnt);
+        if (lane == 0) base = atomicAdd(S.queue[qi], (unsigned long long)cnt);
         base = __shfl_sync(FULL, base, 0);
         if (!R.ghost && ((need >> R.base) & 1u)) {
             const long long cand = (long long)base + __popc(need & ((1u << R.base) - 1u));
@@ -364,7 +406,19 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
                 live = true;
             }
         }
-        if ((long long)base + cnt >= total) dry = true;
+        if ((long long)base + cnt >= total) {  // this range is exhausted: go on with the next one
+            if (++qi >= S.nq) {
+                dry = true;
+                return false;
+            }
+            open_queue();
+            return true;
+        }
+        return false;
+    };
+    auto refill = [&]() {
+        while (refill_once()) {
+        }
     };
 
     stage_begin(S.timeline);
@@ -990,6 +1044,8 @@ struct SchedConfig {
     int split_sms = 32;       // SMs a six-lane pass takes for itself beside a bulk pass (one 8-warp block each)
     int split_grid_b = 8;     // last six-lane pass: one-warp blocks per SM (it has the GPU to itself)
     int soft_cap = 16384;     // budget hand-overs per bulk stage (drain hand-overs come on top)
+    int mean_factor = 4;      // ... and only of trajectories this many times longer than the finished ones' mean
+    int drain_lanes = 10;     // queue empty: a warp hands over what it still runs once this few lanes are alive
     double slow0 = 0.5;       // class 0: candidates with u^2 < slow0 <u^2>
     double slow1 = 0.1;       // class 1 also takes anything with u^2 < slow1 <u^2>
     int refill_batch = 8;     // idle lanes of a warp that trigger its refill ...
@@ -1055,7 +1111,8 @@ enum Counter {
     kCntBound = 5,   // bound[0 .. kMaxStages]
     kCntSnap = 10,   // snap[0 .. kMaxStages], snap[0] = 0
     kCntQueueBulk = 16,   // work queue of bulk pass i
-    kCntQueueSplit = 20   // work queue of split pass i
+    kCntQueueSplit = 20,  // work queue of split pass i
+    kCntStats = 52        // [2 i], [2 i + 1]: accepted steps / number of the trajectories bulk pass i has finished
 };
 
 Ckpt ckpt_at(unsigned char* base, long long cap)
@@ -1200,6 +1257,9 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         S.tail_iters = cfg.tail_iters;
         S.refill_batch = cfg.refill_batch;
         S.refill_wait = cfg.refill_wait;
+        S.drain_lanes = cfg.drain_lanes;
+        S.stats = counters + kCntStats + 2 * i;
+        S.mean_factor = cfg.mean_factor;
         S.timeline = counters + kCntTime + 2 * (1 + 2 * i);
         const long long grid = (i == 0) ? blocks : blocks_beside;
         integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)grid, kBlock, 0, cs>>>(K, y0, N, O, S);
@@ -1209,9 +1269,12 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         SplitSched T;
         T.in = slots;
         T.timeline = counters + kCntTime + 2 * (2 + 2 * i);
-        T.queue = counters + kCntQueueSplit + i;
-        T.begin = counters + kCntSnap + i;
-        T.end = counters + kCntSnap + i + 1;
+        T.nq = i + 1;
+        for (int j = 0; j <= i; ++j) {  // own range first, then the earlier stages'
+            T.queue[j] = counters + kCntQueueSplit + (i - j);
+            T.begin[j] = counters + kCntSnap + (i - j);
+            T.end[j] = counters + kCntSnap + (i - j) + 1;
+        }
         if (i + 1 < stages) {
             // beside the next bulk pass: one block per SM it owns (the dynamic shared memory request
             // leaves no room for a bulk block next to it)

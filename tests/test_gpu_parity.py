@@ -482,6 +482,33 @@ def test_general_potential(aig, n_att, n_rep, trap):
     del ws
 
 
+def test_paper_grid_workload(aig):
+    """NEXT-2: the paper's own workload (head-on launch from an equal-solid-angle grid, linear Paul trap,
+    shallow 'CnDe' potential, no exit radius; Fig. 10) on a 10 x 10 grid over
+    1/20 of its time span: every trajectory ends on t_max; the ones that bounce at most once agree with
+    the oracle to the parity bars (they all reach the well: r_min ~ 60 a0), the bounce counts as a
+    distribution."""
+    w = inputs.paper_workload(ntheta=10, nphi=10, t_max=2.0e12)
+    y0 = inputs.generate_y0(w)
+    g = run_gpu(aig, w, y0)
+    po = orc.make_params(**w.params())
+    o = orc.integrate(po, y0, w.t_max, w.rtol, w.atol, threads=8)
+    y1 = y0.copy()
+    y1[6:9] = np.nextafter(y1[6:9], np.inf)
+    o1 = orc.integrate(po, y1, w.t_max, w.rtol, w.atol, threads=8)
+    assert np.all(g["status"] == 1) and np.all(o["status"] == 1) and np.all(g["t_final"] == w.t_max)
+    d = (g["n_turn"] <= 1) & (o["n_turn"] <= 1) & (o1["n_turn"] <= 1)
+    assert d.sum() >= 20
+    assert np.max(np.abs(g["n_acc"][d].astype(int) - o["n_acc"][d].astype(int))) <= 2
+    assert np.array_equal(g["n_turn"][d], o["n_turn"][d])
+    rel, ref = block_rel(g["y_final"], o["y_final"]), block_rel(o1["y_final"], o["y_final"])
+    assert rel[d].max() <= 1e-6 and rel[d].max() <= 30 * ref[d].max() + 1e-9
+    assert np.max(np.abs(g["r_min"][d] / o["r_min"][d] - 1)) <= 1e-6
+    assert abs(g["complex_flag"].mean() - o["complex_flag"].mean()) <= 3 * math.sqrt(0.25 * 2 / w.N)
+    assert stats.ks_2samp(g["n_turn"], o["n_turn"]).pvalue > 0.01
+    assert stats.ks_2samp(g["n_acc"], o["n_acc"]).pvalue > 0.01
+
+
 def test_degenerate_inputs(aig):
     import torch
     w = inputs.config(0)
