@@ -323,6 +323,7 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
 // helps drain what an earlier, smaller pass is still working through.
 struct SplitSched {
     unsigned long long* timeline;
+    unsigned long long* loaded;  // diagnostics: trajectories this pass has taken
     int nq;
     unsigned long long* queue[4];
     const unsigned long long *begin[4], *end[4];
@@ -379,6 +380,10 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
         unsigned long long base = 0;
         if (lane == 0) base = atomicAdd(S.queue[qi], (unsigned long long)cnt);
         base = __shfl_sync(FULL, base, 0);
+        if (lane == 0) {
+            const long long got = total - (long long)base;
+            if (got > 0) atomicAdd(S.loaded, (unsigned long long)(got < cnt ? got : cnt));
+        }
         if (!R.ghost && ((need >> R.base) & 1u)) {
             const long long cand = (long long)base + __popc(need & ((1u << R.base) - 1u));
             if (cand < total) {
@@ -570,15 +575,27 @@ plan_kernel(const double* __restrict__ y0, const long long N, const PlanArgs A, 
     }
 }
 
-// bound[0..3] = prefix sums of the class counts, cursors at the class starts
+// cursors at the class starts; bound[0..3] = the three stages' ranges of order[].  A stage is a
+// class, except that empty classes at the end are skipped so that the LAST stage (the one whose
+// six-lane pass has the whole GPU) is never empty while an earlier one is not: with a degenerate
+// input (every trajectory in one class, e.g. a fixed launch speed) all the work is in the last stage.
 __global__ void plan_bounds_kernel(unsigned long long* counters, int bound0, int front)
 {
+    unsigned long long start[4];
     unsigned long long acc = 0;
     for (int c = 0; c < 3; ++c) {
-        counters[bound0 + c] = acc;
+        start[c] = acc;
         counters[kCntCursor + c] = acc;
         acc += counters[kCntClass + c];
         if (c == 1) counters[front] = acc;  // classes 0 and 1 (diagnostics)
+    }
+    start[3] = acc;
+    int last = 2;  // last non-empty class
+    while (last > 0 && start[last + 1] == start[last]) --last;
+    const int shift = 2 - last;  // stage s holds class s - shift (stages below `shift` are empty)
+    for (int st = 0; st <= 3; ++st) {
+        const int c = st - shift;
+        counters[bound0 + st] = (c <= 0) ? 0 : start[c];
     }
     counters[bound0 + 3] = acc;
 }
@@ -1112,6 +1129,7 @@ enum Counter {
     kCntSnap = 10,   // snap[0 .. kMaxStages], snap[0] = 0
     kCntQueueBulk = 16,   // work queue of bulk pass i
     kCntQueueSplit = 20,  // work queue of split pass i
+    kCntLoaded = 61,      // diagnostics: trajectories split pass i has taken (its own and earlier stages')
     kCntStats = 52        // [2 i], [2 i + 1]: accepted steps / number of the trajectories bulk pass i has finished
 };
 
@@ -1269,6 +1287,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         SplitSched T;
         T.in = slots;
         T.timeline = counters + kCntTime + 2 * (2 + 2 * i);
+        T.loaded = counters + kCntLoaded + i;
         T.nq = i + 1;
         for (int j = 0; j <= i; ++j) {  // own range first, then the earlier stages'
             T.queue[j] = counters + kCntQueueSplit + (i - j);
