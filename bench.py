@@ -41,7 +41,7 @@ FLOPS_PER_ATTEMPT = 900.0
 FP64_PEAK_NOMINAL = 148 * 4 * 16 * 2 * 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of one integrate_kernel launch at the bench
 # workload, from the ncu --set full capture summarised in profiles/ (None until captured).
-INTEGRATE_DRAM_TRAFFIC_BYTES = 3.03e9  # profiles/r01c_integrate_full.md: the six integrator kernels of one call
+INTEGRATE_DRAM_TRAFFIC_BYTES = 3.02e9  # profiles/r01d_integrate_full.md: the six integrator kernels of one call
 
 WORKLOAD_NAME = "configs[4] N=4194304 q=0.1 rtol=1e-10 atol=1e-12 seed=4"
 SWEEP_Q = (0.1, 0.2, 0.4)
