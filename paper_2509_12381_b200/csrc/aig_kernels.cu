@@ -1209,6 +1209,23 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     if (cudaMemcpyAsync(counters + kCntN, &n64, sizeof(n64), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return AIG_ERR_CUDA;
 
+    {
+        // CUDA loads a kernel's code at its first launch (lazy module loading), and loading may have to
+        // wait for the kernels that are running: the first call would serialise the passes that are meant
+        // to overlap.  Touch every kernel of the schedule before anything is enqueued.
+        cudaFuncAttributes fa;
+        if (cudaFuncGetAttributes(&fa, integrate_kernel<TRAP, kBlock, kBlocksPerSM>) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, integrate_split_kernel<TRAP, kSplitWarps, 1>) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, integrate_split_kernel<TRAP, 1, kSplitMinBlocks>) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, plan_mean_kernel) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, plan_kernel<0>) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, plan_kernel<1>) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, plan_bounds_kernel) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, bounds_kernel) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, snapshot_kernel) != cudaSuccess ||
+            cudaFuncGetAttributes(&fa, head_start_kernel) != cudaSuccess)
+            return AIG_ERR_CUDA;
+    }
     int bps = 0, sms = 0;
     int rc = bulk_capacity<TRAP>(&bps, &sms);
     if (rc) return rc;
