@@ -509,6 +509,27 @@ def test_paper_grid_workload(aig):
     assert stats.ks_2samp(g["n_acc"], o["n_acc"]).pvalue > 0.01
 
 
+def test_paper_complex_probability(aig):
+    """The one physics number the paper prints for its production run: 59.87 % of the head-on trajectories
+    form a complex (tests/golden/paper_constants.txt).  A 100 x 100 full-sphere grid of the same
+    workload over the full millisecond (10^4 trajectories of ~3e5 steps each) must agree within 3 binomial
+    sigma.  Not a pin of the oracle: the bounce criterion r_turn = 500 a0 is a reading (S28)."""
+    import os
+    golden = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")) as fh:
+        for line in fh:
+            if "=" in line and not line.startswith("#"):
+                k, v = line.split("#")[0].split("=")
+                golden[k.strip()] = float(v)
+    w = inputs.paper_workload(ntheta=100, nphi=100, theta=(0.0, math.pi), phi=(0.0, 2 * math.pi))
+    g = run_gpu(aig, w, inputs.generate_y0(w))
+    assert np.all(g["status"] >= 1) and np.all(g["status"] <= 2)          # t_max or maxsteps: there is no exit radius
+    assert (g["status"] == 2).mean() < 0.005 and g["n_acc"].max() <= 1_000_000
+    p = float(g["complex_flag"].mean())
+    sigma = math.sqrt(golden["complex_probability"] * (1 - golden["complex_probability"]) / w.N)
+    assert abs(p - golden["complex_probability"]) <= 3 * sigma, (p, sigma)
+
+
 def test_degenerate_inputs(aig):
     import torch
     w = inputs.config(0)
