@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libaig.so")
 SOURCES = ["aig_kernels.cu"]
-DEPS = ["aig_kernels.cu", "aig_device.cuh", "dp45_nystrom_tableau.inc", "trig_constants.inc", os.path.join("..", "..", "include", "aig.h")]
+DEPS = ["aig_kernels.cu", "aig_device.cuh", "aig_split.cuh", "dp45_nystrom_tableau.inc", "trig_constants.inc", os.path.join("..", "..", "include", "aig.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-fmad=false",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
