@@ -1093,10 +1093,12 @@ SchedConfig sched_config()
             if (got >= 5) c.plan = pl;
             if (got >= 6 && kp >= 0.0) c.kappa = kp;
         }
-        if (const char* e = std::getenv("AIG_REFILL")) {  // "batch,wait,slow0,slow1" (tuning aid)
-            int b = c.refill_batch, w = c.refill_wait;
+        if (const char* e = std::getenv("AIG_REFILL")) {  // "batch,wait,slow0,slow1,mean_factor,drain_lanes" (tuning aid)
+            int b = c.refill_batch, w = c.refill_wait, mf = c.mean_factor, dl = c.drain_lanes;
             double s0 = c.slow0, s1 = c.slow1;
-            const int got = std::sscanf(e, "%d,%d,%lf,%lf", &b, &w, &s0, &s1);
+            const int got = std::sscanf(e, "%d,%d,%lf,%lf,%d,%d", &b, &w, &s0, &s1, &mf, &dl);
+            if (got >= 5 && mf >= 0) c.mean_factor = mf;
+            if (got >= 6 && dl >= 0) c.drain_lanes = dl;
             if (got >= 1 && b >= 1) c.refill_batch = b;
             if (got >= 2 && w >= 0) c.refill_wait = w;
             if (got >= 3 && s0 >= 0.0) c.slow0 = s0;
