@@ -530,6 +530,25 @@ def test_paper_complex_probability(aig):
     assert abs(p - golden["complex_probability"]) <= 3 * sigma, (p, sigma)
 
 
+def test_large_rf_phase(aig):
+    """|Omega t| beyond the range of the branch-free cos (1e5 rad): the library switches to the kernels
+    that call libdevice's cos (TRAP_RF_BIG), in both integrator kernels; same parity bars, and the same
+    bits from the per-thread and the six-lane kernel."""
+    w = inputs.config(0).replace(N=600, t0=4.0e14, t_max=4.0e14 + 2.0e11)
+    assert w.omega_rf * w.t0 > 1.0e5
+    y0 = inputs.generate_y0(w)
+    g, o = run_gpu(aig, w, y0), run_orc(w, y0)
+    _compare_direct(w, y0, g, o)
+    assert abs(int(g["complex_flag"].sum()) - int(o["complex_flag"].sum())) <= 3 * math.sqrt(600 * 0.07) + 1
+    try:
+        aig.set_schedule(plan=0, budget=1, tail_iters=0)
+        g2 = run_gpu(aig, w, y0)
+    finally:
+        aig.set_schedule()
+    for k in g:
+        assert np.array_equal(g[k].view(np.uint8), g2[k].view(np.uint8)), k
+
+
 def test_degenerate_inputs(aig):
     import torch
     w = inputs.config(0)
