@@ -268,6 +268,7 @@ typedef struct orc_obs_state {
     int any_min;   /* a radial minimum has been seen */
     int64_t n_turn;
     double t_first, t_last; /* times of the first / last counted turning point */
+    double x_first[3];      /* ion position at the first counted turning point ("position") */
     double r_min;           /* min over t0 and accepted step ends of the atom-ion distance */
 } orc_obs_state;
 
@@ -289,7 +290,10 @@ static int orc_atomion_observe(double t_new, const double *y, void *o)
         st->any_min = 1;
         if (r < st->p->r_turn) {
             st->n_turn++;
-            if (st->n_turn == 1) st->t_first = t_new;
+            if (st->n_turn == 1) {
+                st->t_first = t_new;
+                for (int k = 0; k < 3; ++k) st->x_first[k] = y[k]; /* rows 0-2: ion position */
+            }
             st->t_last = t_new;
         }
     }
@@ -314,7 +318,7 @@ int orc_integrate(const orc_params *p, const double *y0 /* [12][N] */, int64_t N
                   double rtol, double atol, int64_t i_begin, int64_t i_end,
                   double *y_final /* [12][N] */, double *t_final, double *lifetime,
                   double *angle, double *r_min, int32_t *n_acc, int32_t *n_rej, int32_t *n_turn,
-                  int32_t *status, uint8_t *complex_flag)
+                  int32_t *status, uint8_t *complex_flag, double *x_turn1 /* [3][N] or NULL */)
 {
     if (!p || !y0 || N < 0 || i_begin < 0 || i_end > N) return -1;
     if (!(rtol > 0.0) || atol < 0.0 || !(t_max > p->t0)) return -1;
@@ -327,6 +331,7 @@ int orc_integrate(const orc_params *p, const double *y0 /* [12][N] */, int64_t N
         st.n_turn = 0;
         st.t_first = 0.0;
         st.t_last = 0.0;
+        st.x_first[0] = st.x_first[1] = st.x_first[2] = NAN; /* no bounce: no position (reading S29) */
         orc_rel(y, &st.r_min, &st.s_prev);
         int64_t na, nr;
         int stt;
@@ -344,6 +349,8 @@ int orc_integrate(const orc_params *p, const double *y0 /* [12][N] */, int64_t N
         lifetime[i] = (st.n_turn >= 2) ? st.t_last - st.t_first : 0.0; /* PAPER.md:495 */
         angle[i] = orc_angle(&y[9], &yf[9]); /* initial vs final atom velocity, lab frame */
         r_min[i] = st.r_min;
+        if (x_turn1)
+            for (int kk = 0; kk < 3; ++kk) x_turn1[kk * N + i] = st.x_first[kk];
     }
     return 0;
 }
@@ -360,6 +367,7 @@ int orc_integrate_trace(const orc_params *p, const double *y0 /* [12] */, double
     st.any_min = 0;
     st.n_turn = 0;
     st.t_first = st.t_last = 0.0;
+    st.x_first[0] = st.x_first[1] = st.x_first[2] = NAN;
     orc_rel(y0, &st.r_min, &st.s_prev);
     return orc_dp45_integrate(orc_rhs_atomion, p, 12, p->t0, y0, t_max, rtol, atol, p->max_steps,
                               orc_atomion_observe, &st, yf, &tf, &na, &nr, status, trace_t,

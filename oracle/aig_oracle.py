@@ -127,7 +127,7 @@ def integrate(p: OrcParams, y0, t_max, rtol, atol, threads: int = 1) -> dict:
     out = dict(y_final=np.zeros((12, N)), t_final=np.zeros(N), lifetime=np.zeros(N), angle=np.zeros(N),
                r_min=np.zeros(N), n_acc=np.zeros(N, np.int32), n_rej=np.zeros(N, np.int32),
                n_turn=np.zeros(N, np.int32), status=np.zeros(N, np.int32),
-               complex_flag=np.zeros(N, np.uint8))
+               complex_flag=np.zeros(N, np.uint8), x_turn1=np.zeros((3, N)))
     L = lib()
 
     def run(lo, hi):
@@ -136,7 +136,7 @@ def integrate(p: OrcParams, y0, t_max, rtol, atol, threads: int = 1) -> dict:
                              _dp(out["t_final"]), _dp(out["lifetime"]), _dp(out["angle"]),
                              _dp(out["r_min"]), _ip(out["n_acc"]), _ip(out["n_rej"]),
                              _ip(out["n_turn"]), _ip(out["status"]),
-                             out["complex_flag"].ctypes.data_as(C.POINTER(C.c_uint8)))
+                             out["complex_flag"].ctypes.data_as(C.POINTER(C.c_uint8)), _dp(out["x_turn1"]))
         if rc:
             raise ValueError(f"orc_integrate rc={rc}")
 
@@ -271,23 +271,30 @@ def histogram(obs: dict, angle_edges, life_edges, n_turn_bins: int = 64) -> dict
 # ---------------------------------------------------------------------------------------------
 # NEXT-1: the paper's remaining per-trajectory observables and its "outliers"
 # ---------------------------------------------------------------------------------------------
-OUTLIER_KEYS = ("angle", "n_turn", "lifetime", "transfer", "dist", "n_acc", "KE")
+OUTLIER_KEYS = ("angle", "n_turn", "lifetime", "transfer", "dist", "n_acc", "KE", "position")
 
 
-def observables(p: OrcParams, y0, y_final) -> dict:
+def observables(p: OrcParams, y0, y_final, x_turn1=None) -> dict:
     """The observables of PAPER.md:495-497 that follow from the initial and final states alone,
     written as their definitions (float64, one trajectory per column):
       dist     final atom-ion distance                     |x_atom - x_ion| at the end
       KE       final kinetic energy of the ion             m_ion |v_ion|^2 / 2
       transfer momentum transferred by the atom            m_atom |v_atom(end) - v_atom(t0)|
-    (the paper names them without formulas; readings S24-S26 of DESIGN.md)."""
+      position how far the ion is from the origin during   |x_ion| at the step end that counts the first
+               the first bounce (needs x_turn1[3][N] of     bounce; NaN for a trajectory without one
+               integrate())
+    (the paper names them without formulas; readings S24-S26 and S29 of DESIGN.md)."""
     y0 = np.asarray(y0, dtype=np.float64)
     yf = np.asarray(y_final, dtype=np.float64)
     d = yf[6:9] - yf[0:3]
     dv = yf[9:12] - y0[9:12]
-    return {"dist": np.sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]),
-            "KE": 0.5 * p.m_ion * (yf[3] * yf[3] + yf[4] * yf[4] + yf[5] * yf[5]),
-            "transfer": p.m_atom * np.sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2])}
+    obs = {"dist": np.sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]),
+           "KE": 0.5 * p.m_ion * (yf[3] * yf[3] + yf[4] * yf[4] + yf[5] * yf[5]),
+           "transfer": p.m_atom * np.sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2])}
+    if x_turn1 is not None:
+        x = np.asarray(x_turn1, dtype=np.float64)
+        obs["position"] = np.sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2])
+    return obs
 
 
 def outliers(obs: dict) -> dict:

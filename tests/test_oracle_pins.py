@@ -580,6 +580,76 @@ def test_observables_free_motion_exact():
     assert np.allclose(ob["dist"], np.linalg.norm(d_lin, axis=0), rtol=1e-10)
 
 
+def test_position_free_motion_closed_form():
+    """"position" (how far the ion is from the origin during the first bounce; reading
+    S29).  No potential, no trap: both particles move on straight lines, the only radial minimum is at
+    t* = t0 - d0.u / |u|^2, and the ion is then at x0 + v0 (t* - t0).  The recorded point is the ion's
+    position at the first accepted step end at or after t*: on that line, no earlier than t* and at most
+    one maximal step (0.1 of the span) later."""
+    w = inputs.config(0).replace(N=64)
+    y0 = inputs.generate_y0(w)
+    kw = w.params()
+    kw.update(C4=0.0, C8=0.0, omega_rf=0.0, r_turn=float("inf"))
+    p = orc.make_params(**kw)
+    o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=2)
+    assert np.all(o["n_turn"] == 1)
+    d0, u = y0[6:9] - y0[0:3], y0[9:12] - y0[3:6]
+    tau_star = -np.sum(d0 * u, axis=0) / np.sum(u * u, axis=0)
+    disp = o["x_turn1"] - y0[0:3]
+    vi = y0[3:6]
+    tau = np.sum(disp * vi, axis=0) / np.sum(vi * vi, axis=0)
+    assert np.max(np.linalg.norm(disp - vi * tau, axis=0)) <= 1e-9 * np.max(np.linalg.norm(disp, axis=0))
+    assert np.all(tau >= tau_star * (1 - 1e-12)) and np.all(tau - tau_star <= 0.1 * (w.t_max - p.t0))
+    ob = orc.observables(p, y0, o["y_final"], o["x_turn1"])
+    assert np.allclose(ob["position"], np.linalg.norm(y0[0:3] + vi * tau, axis=0), rtol=1e-9)
+
+
+def test_position_two_body_momentum():
+    """Trap off, zero total momentum (config 1): the centre of mass X stays where it was, so at any time
+    x_ion - X = -(m_atom / M) (x_atom - x_ion): the ion's distance from X at the first bounce is m_atom / M
+    times the atom-ion distance there, which is at least the smallest distance seen and, for a trajectory
+    with a single bounce, at most that of the step end before the sign change."""
+    w = inputs.config(1).replace(N=300)
+    y0 = inputs.generate_y0(w)
+    p = orc.make_params(**w.params())
+    o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=4)
+    M = p.m_ion + p.m_atom
+    X = (p.m_ion * y0[0:3] + p.m_atom * y0[6:9]) / M
+    has = o["n_turn"] >= 1
+    assert has.sum() > 50 and np.all(np.isnan(o["x_turn1"][:, ~has])) and np.all(np.isfinite(o["x_turn1"][:, has]))
+    r_first = np.linalg.norm(o["x_turn1"] - X, axis=0)[has] * M / p.m_atom
+    assert np.all(r_first >= o["r_min"][has] * (1 - 1e-9))
+    one = o["n_turn"][has] == 1
+    assert np.all(r_first[one] < 2.0 * o["r_min"][has][one]) and np.all(r_first < w.params()["r_turn"])
+    # about half of the single bounces have their smallest step-end distance at the recorded point itself
+    assert 0.2 < np.mean(np.abs(r_first[one] / o["r_min"][has][one] - 1) < 1e-9) < 0.8
+
+
+def test_position_against_replay_brute_force():
+    """In the RF trap (config 0): recompute the first counted turning point from the replay's record with
+    NumPy -- s = d.u at every accepted step end, first sign change - to + with r < r_turn -- and compare
+    the ion position stored there value for value; trajectories without one hold NaN."""
+    w = inputs.config(0).replace(N=48)
+    y0 = inputs.generate_y0(w)
+    kw = w.params()
+    p = orc.make_params(**kw)
+    o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=4)
+    seen = 0
+    for i in range(w.N):
+        t, y, _ = orc.integrate_trace(p, y0[:, i], w.t_max, w.rtol, w.atol)
+        rows = np.vstack([y0[:, i][None, :], y])
+        d, u = rows[:, 6:9] - rows[:, 0:3], rows[:, 9:12] - rows[:, 3:6]
+        s, r = np.sum(d * u, axis=1), np.linalg.norm(d, axis=1)
+        hit = np.flatnonzero((s[:-1] < 0) & (s[1:] >= 0) & (r[1:] < kw["r_turn"]))
+        assert len(hit) == o["n_turn"][i]
+        if len(hit):
+            assert np.array_equal(o["x_turn1"][:, i], rows[hit[0] + 1, 0:3])
+            seen += 1
+        else:
+            assert np.all(np.isnan(o["x_turn1"][:, i]))
+    assert seen >= 10
+
+
 def test_outliers_definition():
     rng = np.random.Generator(np.random.PCG64(7))
     n = 500
