@@ -74,7 +74,7 @@ typedef struct aig_params {
 } aig_params;
 
 /* Per-trajectory outputs: caller-allocated DEVICE buffers, each of length N
- * (y_final: 12*N, SoA like y0).  Any pointer except y_final/status may NOT be NULL. */
+ * (y_final: 12*N, SoA like y0; x_turn1: 3*N).  No pointer except x_turn1 may be NULL. */
 typedef struct aig_out {
     double *y_final;       /* state at the last accepted step end (PAPER.md:192 yend1..12) */
     double *t_final;       /* time of that step end (tend) */
@@ -86,6 +86,10 @@ typedef struct aig_out {
     int32_t *n_turn;       /* counted inner turning points ("bounces") */
     int32_t *status;       /* AIG_STATUS_* */
     uint8_t *complex_flag; /* 1 if n_turn >= 2 (one bounce = simple) */
+    double *x_turn1;       /* OPTIONAL (NULL = not recorded), [3][N] SoA: ion position at the accepted step end
+                              that counted the first turning point -- the paper's "position" observable is its
+                              norm ("how far the ion is from the origin during the first bounce", PAPER.md:495;
+                              DESIGN.md reading S29); NaN for a trajectory with n_turn = 0 */
 } aig_out;
 
 /* Bin edges of the observable histograms: DEVICE pointers to strictly increasing doubles
@@ -137,26 +141,31 @@ int aig_histogram(const aig_out *obs, int64_t N, const aig_hist_spec *spec, cons
 
 /* ---- NEXT-1: the paper's remaining observables and its outliers ------------------ */
 
-/* Observables of PAPER.md:495-497 that follow from the initial and final states alone: DEVICE
- * arrays of length N, written by aig_observables.  The paper names them without formulas; the
- * readings are DESIGN.md S24-S26:
+/* Observables of PAPER.md:495-497 that follow from the initial and final states (and, for
+ * `position`, from aig_out.x_turn1): DEVICE arrays of length N, written by aig_observables.  The
+ * paper names them without formulas; the readings are DESIGN.md S24-S26, S29:
  *   dist      "the final atom-ion distance"          |x_atom - x_ion| at the end
  *   KE        "the final kinetic energy of the ion"  m_ion |v_ion|^2 / 2
- *   transfer  "the momentum transfered by the atom"  m_atom |v_atom(end) - v_atom(t0)|          */
+ *   transfer  "the momentum transfered by the atom"  m_atom |v_atom(end) - v_atom(t0)|
+ *   position  "how far the ion is from the origin    |x_turn1|, NaN without a bounce; OPTIONAL (NULL =
+ *              during the first bounce"               skipped), needs out->x_turn1 of aig_integrate     */
 typedef struct aig_obs_extra {
     double *dist, *KE, *transfer;
+    double *position;
 } aig_obs_extra;
 
-/* dist, KE, transfer of N trajectories from y0 (DEVICE [12][N]) and out->y_final as written by
- * aig_integrate (only y_final of `out` is read).  One HBM-bound kernel on `cuda_stream`. */
+/* dist, KE, transfer (and position) of N trajectories from y0 (DEVICE [12][N]) and out->y_final as
+ * written by aig_integrate (only y_final, and x_turn1 when extra->position is set, are read).  One
+ * HBM-bound kernel on `cuda_stream`. */
 int aig_observables(const aig_params *p, const double *y0, const aig_out *out, int64_t N,
                     const aig_obs_extra *extra, void *cuda_stream);
 
 /* "outliers" (the trajectories with the highest and lowest value of each
- * observable): result (DEVICE int64 [7][2]) receives, for the observables
- *   0 angle, 1 n_turn ("bounces"), 2 lifetime, 3 transfer, 4 dist, 5 n_acc ("nsteps"), 6 KE
+ * observable): result (DEVICE int64 [8][2]) receives, for the observables
+ *   0 angle, 1 n_turn ("bounces"), 2 lifetime, 3 transfer, 4 dist, 5 n_acc ("nsteps"), 6 KE, 7 position
  * the index of the smallest ([k][0]) and of the largest ([k][1]) value; the smallest index wins a
- * tie, NaNs are skipped, -1 when nothing qualifies (N = 0).  One pass over the seven arrays.
+ * tie, NaNs are skipped (trajectories without a bounce have no position), -1 when nothing qualifies
+ * (N = 0, or extra->position = NULL for row 7).  One pass over the eight arrays.
  * workspace: DEVICE scratch of aig_outliers_workspace_bytes() bytes, 16-byte aligned. */
 size_t aig_outliers_workspace_bytes(void);
 int aig_outliers(const aig_out *out, const aig_obs_extra *extra, int64_t N, int64_t *result,

@@ -36,7 +36,7 @@ class Out(C.Structure):
     _fields_ = [("y_final", C.c_void_p), ("t_final", C.c_void_p), ("lifetime", C.c_void_p),
                 ("angle", C.c_void_p), ("r_min", C.c_void_p), ("n_acc", C.c_void_p),
                 ("n_rej", C.c_void_p), ("n_turn", C.c_void_p), ("status", C.c_void_p),
-                ("complex_flag", C.c_void_p)]
+                ("complex_flag", C.c_void_p), ("x_turn1", C.c_void_p)]   # x_turn1: optional, None = not recorded
 
 
 class HistSpec(C.Structure):
@@ -118,12 +118,14 @@ def _stream_ptr(stream):
     return C.c_void_p(s.cuda_stream)
 
 
-def alloc_out(N: int, device="cuda"):
-    """Caller-owned device buffers for aig_integrate (dict of torch tensors)."""
+def alloc_out(N: int, device="cuda", position: bool = False):
+    """Caller-owned device buffers for aig_integrate (dict of torch tensors).  position=True adds the
+    optional x_turn1 [3, N] (ion position at the first bounce)."""
     torch = _torch()
     f8 = dict(dtype=torch.float64, device=device)
     i4 = dict(dtype=torch.int32, device=device)
-    return dict(y_final=torch.empty((12, N), **f8), t_final=torch.empty(N, **f8),
+    extra = dict(x_turn1=torch.empty((3, N), **f8)) if position else {}
+    return dict(**extra, y_final=torch.empty((12, N), **f8), t_final=torch.empty(N, **f8),
                 lifetime=torch.empty(N, **f8), angle=torch.empty(N, **f8), r_min=torch.empty(N, **f8),
                 n_acc=torch.empty(N, **i4), n_rej=torch.empty(N, **i4), n_turn=torch.empty(N, **i4),
                 status=torch.empty(N, **i4), complex_flag=torch.empty(N, dtype=torch.uint8, device=device))
@@ -133,6 +135,7 @@ def _out_struct(bufs) -> Out:
     o = Out()
     for f in OUT_FIELDS:
         setattr(o, f, bufs[f].data_ptr())
+    o.x_turn1 = bufs["x_turn1"].data_ptr() if bufs.get("x_turn1") is not None else None
     return o
 
 
@@ -183,20 +186,29 @@ def aig_histogram(obs, angle_edges, life_edges, n_turn_bins: int = 64, hist=None
 
 
 class ObsExtra(C.Structure):
-    _fields_ = [("dist", C.c_void_p), ("KE", C.c_void_p), ("transfer", C.c_void_p)]
+    _fields_ = [("dist", C.c_void_p), ("KE", C.c_void_p), ("transfer", C.c_void_p), ("position", C.c_void_p)]
 
 
-OUTLIER_KEYS = ("angle", "n_turn", "lifetime", "transfer", "dist", "n_acc", "KE")   # order of aig_outliers' result rows
+# order of aig_outliers' result rows
+OUTLIER_KEYS = ("angle", "n_turn", "lifetime", "transfer", "dist", "n_acc", "KE", "position")
+
+
+def _extra_struct(extra) -> ObsExtra:
+    pos = extra.get("position")
+    return ObsExtra(extra["dist"].data_ptr(), extra["KE"].data_ptr(), extra["transfer"].data_ptr(),
+                    pos.data_ptr() if pos is not None else None)
 
 
 def aig_observables(params: Params, y0, obs, extra=None, stream=None):
-    """dist, KE, transfer (include/aig.h) of the trajectories in ``obs`` (dict from aig_integrate)."""
+    """dist, KE, transfer (include/aig.h) of the trajectories in ``obs`` (dict from aig_integrate), and
+    position when ``obs`` holds x_turn1 (alloc_out(position=True))."""
     torch = _torch()
     N = y0.shape[1]
     assert y0.is_cuda and y0.dtype == torch.float64 and y0.shape[0] == 12 and y0.is_contiguous()
     if extra is None:
-        extra = {k: torch.empty(N, dtype=torch.float64, device=y0.device) for k in ("dist", "KE", "transfer")}
-    e = ObsExtra(*[extra[k].data_ptr() for k in ("dist", "KE", "transfer")])
+        keys = ("dist", "KE", "transfer") + (("position",) if obs.get("x_turn1") is not None else ())
+        extra = {k: torch.empty(N, dtype=torch.float64, device=y0.device) for k in keys}
+    e = _extra_struct(extra)
     o = _out_struct(obs)
     L = lib()
     L.aig_observables.restype = C.c_int
@@ -207,7 +219,8 @@ def aig_observables(params: Params, y0, obs, extra=None, stream=None):
 
 
 def aig_outliers(obs, extra, stream=None):
-    """int64 CUDA tensor [7, 2]: index of the smallest / largest value of each OUTLIER_KEYS observable."""
+    """int64 CUDA tensor [8, 2]: index of the smallest / largest value of each OUTLIER_KEYS observable
+    (row "position" is -1, -1 when ``extra`` has none)."""
     torch = _torch()
     N = obs["angle"].numel()
     dev = obs["angle"].device
@@ -217,7 +230,7 @@ def aig_outliers(obs, extra, stream=None):
     L.aig_outliers.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
     ws = torch.empty(int(L.aig_outliers_workspace_bytes()), dtype=torch.uint8, device=dev)
     res = torch.empty((len(OUTLIER_KEYS), 2), dtype=torch.int64, device=dev)
-    e = ObsExtra(*[extra[k].data_ptr() for k in ("dist", "KE", "transfer")])
+    e = _extra_struct(extra)
     o = _out_struct(obs)
     _check(L.aig_outliers(C.byref(o), C.byref(e), N, res.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "aig_outliers")
     res._ws = ws  # keep the scratch alive until the stream has run
@@ -262,10 +275,10 @@ def aig_run_host(params: Params, y0_host: np.ndarray, t_max, rtol, atol, angle_e
     dt = dict(y_final=(np.float64, (12, N)), t_final=(np.float64, (N,)), lifetime=(np.float64, (N,)),
               angle=(np.float64, (N,)), r_min=(np.float64, (N,)), n_acc=(np.int32, (N,)),
               n_rej=(np.int32, (N,)), n_turn=(np.int32, (N,)), status=(np.int32, (N,)),
-              complex_flag=(np.uint8, (N,)))
+              complex_flag=(np.uint8, (N,)), x_turn1=(np.float64, (3, N)))
     res = {} if out is None else out
     o = Out()
-    for f in OUT_FIELDS:
+    for f in OUT_FIELDS + ("x_turn1",):
         if f in want:
             if f not in res:
                 res[f] = np.empty(dt[f][1], dtype=dt[f][0])

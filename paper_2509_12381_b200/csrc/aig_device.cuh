@@ -495,7 +495,7 @@ __device__ __forceinline__ void init_traj(const KParams& P, Traj& T, Cold& C)
 // behind the error estimate is what bounds the latency of a step.
 template <class Cold>
 __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, double err, const StepTimes& ST,
-                                           double r2, double s, bool live, bool& accepted)
+                                           double r2, double s, bool live, bool& accepted, bool& first_turn)
 {
     const double z = inv_fifth_root(err * P.inv_rtol);  // (err/rtol)^(-1/5)
     const bool acc = (err <= P.rtol);                   // NaN rejects
@@ -537,16 +537,21 @@ __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, d
     if (Cold::kInRegisters) {
         C.rmin2() = (a & (r2 < C.rmin2())) ? r2 : C.rmin2();
         const bool c = a & counted;
-        C.t_first() = (c & (C.n_turn() == 0)) ? ST.t_new : C.t_first();
+        first_turn = c & (C.n_turn() == 0);
+        C.t_first() = first_turn ? ST.t_new : C.t_first();
         C.t_last() = c ? ST.t_new : C.t_last();
         C.n_turn() += c ? 1 : 0;
         C.n_rej() += r ? 1 : 0;
     } else {
+        first_turn = false;
         if (a) {
             if (r2 < C.rmin2()) C.rmin2() = r2;
             if (counted) {
                 const int nt = ++C.n_turn();
-                if (nt == 1) C.t_first() = ST.t_new;
+                if (nt == 1) {
+                    C.t_first() = ST.t_new;
+                    first_turn = true;
+                }
                 C.t_last() = ST.t_new;
             }
         }
@@ -562,13 +567,14 @@ __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, d
 }
 
 // finish_core for the per-thread integrator: on return T holds the state to continue from (or
-// the final state).
+// the final state).  first_turn: this step counted the trajectory's first turning point (the
+// "position" observable of PAPER.md:495 is the ion position T.X[0..2] at this moment).
 template <class Cold>
-__device__ __forceinline__ int finish_attempt(const KParams& P, Traj& T, Cold& C, const Attempt& R)
+__device__ __forceinline__ int finish_attempt(const KParams& P, Traj& T, Cold& C, const Attempt& R, bool& first_turn)
 {
     bool accepted;
     const StepTimes ST = step_times(P, T.c);
-    const int st = finish_core(P, T.c, C, R.err, ST, R.r2, R.s, true, accepted);
+    const int st = finish_core(P, T.c, C, R.err, ST, R.r2, R.s, true, accepted, first_turn);
     if (accepted) {
 #pragma unroll
         for (int i = 0; i < 6; ++i) {

@@ -68,6 +68,7 @@ struct OutPtrs {
     double *y_final, *t_final, *lifetime, *angle, *r_min;
     int *n_acc, *n_rej, *n_turn, *status;
     unsigned char* complex_flag;
+    double* x_turn1;  // [3][N] ion position at the first counted turning point, or nullptr (not recorded)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -284,7 +285,12 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
         if (live) {
             Attempt R;
             dp45_attempt<TRAP>(P, T, R);
-            const int st = finish_attempt(P, T, C, R);
+            bool first_turn;
+            const int st = finish_attempt(P, T, C, R, first_turn);
+            if (first_turn && O.x_turn1) {  // once per trajectory ("position")
+#pragma unroll
+                for (int k = 0; k < 3; ++k) O.x_turn1[k * N + idx] = T.X[k];
+            }
             if (st >= 0) {
                 pending = st;
                 live = false;
@@ -445,8 +451,10 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
             SplitAttempt A;
             StepTimes ST;
             split_attempt<TRAP>(P, R, K, Y, A, ST);
-            bool accepted;
-            const int s1 = finish_core(P, K, C, A.err, ST, A.r2, A.s, live & (st < 0), accepted);
+            bool accepted, first_turn;
+            const int s1 = finish_core(P, K, C, A.err, ST, A.r2, A.s, live & (st < 0), accepted, first_turn);
+            // once per trajectory ("position"): lane (k, 0) holds component k of the ion
+            if (first_turn && R.e == 0 && O.x_turn1) O.x_turn1[R.k * N + idx] = A.Y.xi;
             Y.xi = accepted ? A.Y.xi : Y.xi;
             Y.vi = accepted ? A.Y.vi : Y.vi;
             Y.a1i = accepted ? A.Y.a1i : Y.a1i;
@@ -785,7 +793,8 @@ trace_kernel(const KParams P, const double* __restrict__ y0, const long long cap
         const int before = T.c.n_acc;
         Attempt R;
         dp45_attempt<TRAP>(P, T, R);
-        st = finish_attempt(P, T, C, R);
+        bool first_turn;
+        st = finish_attempt(P, T, C, R, first_turn);
         if (T.c.n_acc != before) {
             const long long j = (long long)before;
             if (j < cap) {
@@ -809,11 +818,12 @@ trace_kernel(const KParams P, const double* __restrict__ y0, const long long cap
 // ------------------------------------------------------------------------------------------
 // NEXT-1: the paper's remaining observables and its outliers (:521)
 // ------------------------------------------------------------------------------------------
-// HBM-bound: reads the final state (96 B) and the initial atom velocity (24 B), writes 24 B.
+// HBM-bound: reads the final state (96 B) and the initial atom velocity (24 B), writes 24 B; with
+// `position` 24 B more are read (the ion position at the first bounce) and 8 B more written.
 __global__ void __launch_bounds__(256)
 observables_kernel(const double* __restrict__ y0, const double* __restrict__ yf, const long long N,
                    const double m_ion, const double m_atom, double* __restrict__ dist, double* __restrict__ ke,
-                   double* __restrict__ transfer)
+                   double* __restrict__ transfer, const double* __restrict__ x_turn1, double* __restrict__ position)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
@@ -825,12 +835,16 @@ observables_kernel(const double* __restrict__ y0, const double* __restrict__ yf,
         dist[i] = sqrt(sum3(d0 * d0, d1 * d1, d2 * d2));
         ke[i] = (0.5 * m_ion) * sum3(v0 * v0, v1 * v1, v2 * v2);
         transfer[i] = m_atom * sqrt(sum3(w0 * w0, w1 * w1, w2 * w2));
+        if (position) {  // NaN where there was no bounce (x_turn1 holds NaN there)
+            const double p0 = x_turn1[0 * N + i], p1 = x_turn1[1 * N + i], p2 = x_turn1[2 * N + i];
+            position[i] = sqrt(sum3(p0 * p0, p1 * p1, p2 * p2));
+        }
     }
 }
 
-// arg-min / arg-max of seven observables in one pass: (value, index) pairs, the smaller index wins
+// arg-min / arg-max of eight observables in one pass: (value, index) pairs, the smaller index wins
 // a tie, NaNs are skipped, index -1 = nothing seen.
-constexpr int kOutlierObs = 7;  // angle, n_turn, lifetime, transfer, dist, n_acc, KE
+constexpr int kOutlierObs = 8;  // angle, n_turn, lifetime, transfer, dist, n_acc, KE, position
 struct Extreme {
     double v;
     long long i;
@@ -855,6 +869,7 @@ __device__ __forceinline__ Extreme shfl_extreme(const Extreme e, int off)
 
 struct OutlierArgs {
     const double *angle, *lifetime, *transfer, *dist, *ke;
+    const double* position;        // may be nullptr: the row then reads -1, -1
     const int *n_turn, *n_acc;
     Extreme* partial;              // [gridDim.x][kOutlierObs][2]
     unsigned int* ticket;          // blocks that have finished
@@ -875,7 +890,7 @@ outliers_kernel(const OutlierArgs a, const long long N)
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
         const double x[kOutlierObs] = {a.angle[i],    (double)a.n_turn[i], a.lifetime[i], a.transfer[i],
-                                       a.dist[i],     (double)a.n_acc[i],  a.ke[i]};
+                                       a.dist[i],     (double)a.n_acc[i],  a.ke[i],       a.position ? a.position[i] : nan("")};
 #pragma unroll
         for (int k = 0; k < kOutlierObs; ++k) {
             if (x[k] == x[k]) {
@@ -1389,8 +1404,13 @@ int aig_integrate(const aig_params* p, const double* y0, int64_t N, double t_max
         return AIG_ERR_ALIGN;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const KParams K = make_kparams(p, t_max, rtol, atol);
+    if (out->x_turn1) {
+        if (!aligned(out->x_turn1, 8)) return AIG_ERR_ALIGN;
+        // all-ones bytes = NaN: "no bounce, no position"; the kernels overwrite the rest once per trajectory
+        if (cudaMemsetAsync(out->x_turn1, 0xFF, 3 * (size_t)N * sizeof(double), st) != cudaSuccess) return AIG_ERR_CUDA;
+    }
     OutPtrs O{out->y_final, out->t_final, out->lifetime, out->angle, out->r_min,
-              out->n_acc,   out->n_rej,   out->n_turn,   out->status, out->complex_flag};
+              out->n_acc,   out->n_rej,   out->n_turn,   out->status, out->complex_flag, out->x_turn1};
     switch (trap_mode(p, t_max) + 4 * (general_potential(p) ? POT_GENERAL : POT_4_8)) {
         case TRAP_RF: return launch_integrate<TRAP_RF>(p, K, y0, N, O, workspace, st);
         case TRAP_RF_BIG: return launch_integrate<TRAP_RF_BIG>(p, K, y0, N, O, workspace, st);
@@ -1515,15 +1535,16 @@ int aig_observables(const aig_params* p, const double* y0, const aig_out* out, i
     if (N < 0 || N > (1LL << 40)) return AIG_ERR_SIZE;
     if (N == 0) return AIG_OK;
     if (!y0 || !out || !out->y_final || !extra->dist || !extra->KE || !extra->transfer) return AIG_ERR_NULL;
+    if (extra->position && !out->x_turn1) return AIG_ERR_NULL;
     if (!aligned(y0, 8) || !aligned(out->y_final, 8) || !aligned(extra->dist, 8) || !aligned(extra->KE, 8) ||
-        !aligned(extra->transfer, 8))
+        !aligned(extra->transfer, 8) || !aligned(extra->position, 8) || !aligned(out->x_turn1, 8))
         return AIG_ERR_ALIGN;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return AIG_ERR_CUDA;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return AIG_ERR_CUDA;
     const long long blocks = std::min<long long>((N + 255) / 256, (long long)sms * 8);
     observables_kernel<<<(unsigned)blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
-        y0, out->y_final, N, p->m_ion, p->m_atom, extra->dist, extra->KE, extra->transfer);
+        y0, out->y_final, N, p->m_ion, p->m_atom, extra->dist, extra->KE, extra->transfer, out->x_turn1, extra->position);
     g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
@@ -1559,6 +1580,7 @@ int aig_outliers(const aig_out* out, const aig_obs_extra* extra, int64_t N, int6
     a.transfer = N ? extra->transfer : nullptr;
     a.dist = N ? extra->dist : nullptr;
     a.ke = N ? extra->KE : nullptr;
+    a.position = N ? extra->position : nullptr;
     a.ticket = static_cast<unsigned int*>(workspace);
     a.partial = reinterpret_cast<Extreme*>(static_cast<unsigned char*>(workspace) + 256);
     a.result = reinterpret_cast<long long*>(result);
@@ -1589,7 +1611,8 @@ int aig_run_host(const aig_params* p, const double* y0_host, int64_t N, double t
     }
     const size_t flag_bytes = (n + 255) / 256 * 256;
     const size_t ws_bytes = round_up(aig_workspace_bytes(N), 256);
-    const size_t total = 2 * b_y + 4 * b_d + 4 * b_i + flag_bytes + ws_bytes + 8 * (hist_words + edge_words) + 8192;
+    const size_t b_x = out_host->x_turn1 ? 3 * b_d : 0;
+    const size_t total = 2 * b_y + 4 * b_d + b_x + 4 * b_i + flag_bytes + ws_bytes + 8 * (hist_words + edge_words) + 8192;
     unsigned char* slab = nullptr;
     cudaStream_t st = nullptr;
     if (cudaMalloc(&slab, total) != cudaSuccess) return AIG_ERR_CUDA;
@@ -1617,6 +1640,7 @@ int aig_run_host(const aig_params* p, const double* y0_host, int64_t N, double t
     d.n_turn = reinterpret_cast<int32_t*>(take(b_i));
     d.status = reinterpret_cast<int32_t*>(take(b_i));
     d.complex_flag = take(flag_bytes);
+    d.x_turn1 = b_x ? reinterpret_cast<double*>(take(b_x)) : nullptr;
     void* ws = take(ws_bytes);
     if (cudaMemcpyAsync(d_y0, y0_host, b_y, cudaMemcpyHostToDevice, st) != cudaSuccess) return fail(AIG_ERR_CUDA);
     rc = aig_integrate(p, d_y0, N, t_max, rtol, atol, &d, ws, st);
@@ -1665,6 +1689,7 @@ int aig_run_host(const aig_params* p, const double* y0_host, int64_t N, double t
         if (o->n_turn) ok = ok && cudaMemcpyAsync(o->n_turn, d.n_turn, b_i, D2H, st) == cudaSuccess;
         if (o->status) ok = ok && cudaMemcpyAsync(o->status, d.status, b_i, D2H, st) == cudaSuccess;
         if (o->complex_flag) ok = ok && cudaMemcpyAsync(o->complex_flag, d.complex_flag, n, D2H, st) == cudaSuccess;
+        if (o->x_turn1) ok = ok && cudaMemcpyAsync(o->x_turn1, d.x_turn1, b_x, D2H, st) == cudaSuccess;
         if (!ok) return fail(AIG_ERR_CUDA);
     }
     if (cudaStreamSynchronize(st) != cudaSuccess) return fail(AIG_ERR_CUDA);

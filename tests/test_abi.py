@@ -60,7 +60,8 @@ def test_struct_layouts_match_header():
     assert C.sizeof(binding.Params) == 14 * 8 + 8 + 8  # 14 doubles (2+2+3+3+1+1+1+1) + int64 + 2 int32
     assert binding.Params.n_att.offset == 15 * 8 and binding.Params.n_rep.offset == 15 * 8 + 4
     assert binding.Params.max_steps.offset == 14 * 8
-    assert C.sizeof(binding.Out) == 10 * C.sizeof(C.c_void_p)
+    assert C.sizeof(binding.Out) == 11 * C.sizeof(C.c_void_p)          # ten required outputs + optional x_turn1
+    assert C.sizeof(binding.ObsExtra) == 4 * C.sizeof(C.c_void_p)     # dist, KE, transfer + optional position
     assert binding.HistSpec.life_edges.offset == 16 and binding.HistSpec.n_turn_bins.offset == 28
     assert C.sizeof(binding.Hist) == 5 * C.sizeof(C.c_void_p)
 

@@ -67,9 +67,10 @@ def step_tolerance(y):
     return 1e-14 + 30 * np.finfo(float).eps * xmax / r
 
 
-def run_gpu(aig, w, y0):
+def run_gpu(aig, w, y0, position=False):
     p = aig.make_params(**w.params())
-    return _host(aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol))
+    out = aig.alloc_out(y0.shape[1], "cuda", position=True) if position else None
+    return _host(aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol, out=out))
 
 
 def run_orc(w, y0, threads=8):
@@ -214,7 +215,7 @@ def test_schedule_invariance(aig):
     try:
         for kw in schedules:
             aig.set_schedule(**kw)
-            g = run_gpu(aig, w, y0)
+            g = run_gpu(aig, w, y0, position=True)   # with the optional first-bounce record (x_turn1)
             assert np.all(g["status"] <= 1)
             if ref is None:
                 ref = g
@@ -354,18 +355,37 @@ def test_observables_and_outliers(aig):
     outliers index for index (integer work: exact), on several blocks and a ragged tail, with ties
     and NaNs, and for N = 0."""
     import torch
-    w = inputs.config(2).replace(N=20000 + 13)
+    w = inputs.config(2).replace(N=20000 + 13, r_turn=3000.0)   # a quarter of the trajectories pass beyond r_turn: no bounce
     y0 = inputs.generate_y0(w)
     p = aig.make_params(**w.params())
     y0d = _dev(y0)
-    out = aig.aig_integrate(p, y0d, w.t_max, w.rtol, w.atol)
+    out = aig.aig_integrate(p, y0d, w.t_max, w.rtol, w.atol, out=aig.alloc_out(w.N, "cuda", position=True))
     extra = aig.aig_observables(p, y0d, out)
     res = aig.aig_outliers(out, extra)
     g = _host(out)
     e = {k: v.cpu().numpy() for k, v in extra.items()}
-    ref = orc.observables(orc.make_params(**w.params()), y0, g["y_final"])
-    for k in ("dist", "KE", "transfer"):
-        assert np.max(np.abs(e[k] - ref[k]) / np.maximum(np.abs(ref[k]), 1e-300)) <= 4e-16 * 4, k
+    ref = orc.observables(orc.make_params(**w.params()), y0, g["y_final"], g["x_turn1"])
+    for k in ("dist", "KE", "transfer", "position"):
+        fin = np.isfinite(ref[k])
+        assert np.array_equal(fin, np.isfinite(e[k])), k
+        assert np.max(np.abs(e[k] - ref[k])[fin] / np.maximum(np.abs(ref[k][fin]), 1e-300)) <= 4e-16 * 4, k
+    # "position" (PAPER.md:495): the ion position at the first bounce, against the oracle's record.  No
+    # bounce <=> NaN; where both took the same steps (same accepted count, one bounce outside the
+    # short-range well) the recorded points agree like the final states do.
+    o = run_orc(w, y0)
+    assert np.array_equal(np.isnan(g["x_turn1"]).all(axis=0), g["n_turn"] == 0)
+    assert np.array_equal(np.isnan(g["x_turn1"]).any(axis=0), g["n_turn"] == 0)
+    assert 0.02 < np.mean(g["n_turn"] == 0) < 0.98
+    same = (g["n_acc"] == o["n_acc"]) & (g["n_turn"] == 1) & (o["n_turn"] == 1) & (o["status"] == 0) & \
+           (o["r_min"] > SHORT_RANGE)
+    assert same.sum() > 5000, same.sum()
+    dx = np.linalg.norm(g["x_turn1"] - o["x_turn1"], axis=0)[same] / np.linalg.norm(o["x_turn1"], axis=0)[same]
+    assert dx.max() <= 1e-6, dx.max()
+    # deep bounces amplify rounding (DESIGN.md "Parity metric") but the first bounce is reached before that
+    deep = (g["n_acc"] == o["n_acc"]) & (g["n_turn"] >= 1) & (o["n_turn"] >= 1) & (o["r_min"] <= SHORT_RANGE)
+    if deep.sum() >= 20:
+        dd = np.linalg.norm(g["x_turn1"] - o["x_turn1"], axis=0)[deep] / np.linalg.norm(o["x_turn1"], axis=0)[deep]
+        assert np.median(dd) <= 1e-6, np.median(dd)
     allobs = dict(g)
     allobs.update(e)
     want = orc.outliers(allobs)
@@ -396,7 +416,7 @@ def test_trace_replay(aig):
     w = inputs.config(2).replace(N=4096)
     y0 = inputs.generate_y0(w)
     p = aig.make_params(**w.params())
-    out = aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol)
+    out = aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol, out=aig.alloc_out(w.N, "cuda", position=True))
     g = _host(out)
     longest = int(np.argmax(g["lifetime"]))
     direct = int(np.flatnonzero((g["n_turn"] <= 1) & (g["r_min"] > SHORT_RANGE) & (g["status"] == 0))[0])
@@ -411,6 +431,17 @@ def test_trace_replay(aig):
         tt, yy = t[:na].cpu().numpy(), y[:, :na].cpu().numpy()
         assert np.array_equal(yy[:, -1].view(np.uint64), g["y_final"][:, i].view(np.uint64))
         assert tt[-1] == g["t_final"][i] and np.all(np.diff(tt) > 0)
+        # the first counted turning point, recomputed from the record with NumPy: x_turn1 is the ion
+        # position of that row, value for value
+        rows = np.hstack([y0[:, i:i + 1], yy])
+        d, u = rows[6:9] - rows[0:3], rows[9:12] - rows[3:6]
+        sdot, r = np.sum(d * u, axis=0), np.linalg.norm(d, axis=0)
+        hit = np.flatnonzero((sdot[:-1] < 0) & (sdot[1:] >= 0) & (r[1:] < w.params()["r_turn"]))
+        if g["n_turn"][i] == 0:
+            assert len(hit) == 0 and np.all(np.isnan(g["x_turn1"][:, i]))
+        else:
+            assert len(hit) >= 1
+            assert np.array_equal(g["x_turn1"][:, i].view(np.uint64), rows[0:3, hit[0] + 1].view(np.uint64))
     # step by step against the oracle's record on the direct trajectory
     po = orc.make_params(**w.params())
     to, yo, st = orc.integrate_trace(po, y0[:, direct], w.t_max, w.rtol, w.atol)
@@ -631,9 +662,10 @@ def test_run_host_end_to_end(aig):
     y0 = inputs.generate_y0(w)
     ae, le = inputs.histogram_edges()
     p = aig.make_params(**w.params())
-    res = aig.aig_run_host(p, y0, w.t_max, w.rtol, w.atol, ae, le)
-    dev = run_gpu(aig, w, y0)
+    res = aig.aig_run_host(p, y0, w.t_max, w.rtol, w.atol, ae, le, want=aig.OUT_FIELDS + ("x_turn1",))
+    dev = run_gpu(aig, w, y0, position=True)
     for k in ("y_final", "t_final", "angle", "lifetime", "n_acc", "n_rej", "n_turn", "status", "complex_flag"):
         assert np.array_equal(res[k], dev[k]), k       # same kernels, same inputs: bit-identical
+    assert np.array_equal(res["x_turn1"].view(np.uint64), dev["x_turn1"].view(np.uint64))
     ref = orc.histogram(dev, ae, le, 64)
     assert all(np.array_equal(res["hist"][k], ref[k]) for k in ref)
