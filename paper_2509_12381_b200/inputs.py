@@ -151,7 +151,7 @@ def config(i: int, **overrides) -> Workload:
 
 
 def paper_workload(ntheta: int = 50, nphi: int = 50, theta=(0.0, math.pi / 2), phi=(0.0, math.pi / 2),
-                   **overrides) -> Workload:
+                   positions: str = "uniform", collisiontype: str = "head-on", **overrides) -> Workload:
     """NEXT-2: the paper's OWN workload (not a BASELINE.json config): Yb+ + Rb, the atom launched head-on
     at fixed speed v0 = sqrt(3 k_B T / m_a) from an equal-solid-angle (theta, phi) grid on the sphere
     r0 = 5000 a0 towards an ion at rest at the centre of a linear Paul trap, integrated for 1 ms with no
@@ -162,15 +162,23 @@ def paper_workload(ntheta: int = 50, nphi: int = 50, theta=(0.0, math.pi / 2), p
       C4 = 159.5455, De = 1 K k_B  =>  C8 = 2.00949488627505e9, Re = 70.84 a0 (both printed);
       ax = ay = -2.982e-4, az = -2 ax, qx = 0.219, qy = -qx, qz = 0, Omega = 2 pi 2.5 MHz;
       tmax = 1000 us, maxsteps 1e6, rtol 1e-10, atol 1e-20.
-    A radial minimum counts as a bounce inside r_turn = 500 a0 (the paper gives no formula)."""
+    A radial minimum counts as a bounce inside r_turn = 500 a0 (the paper gives no formula).
+    positions = "random": ntheta * nphi directions drawn uniformly in solid angle inside the
+    (theta, phi) window instead of the grid.  collisiontype = "thermal": normal velocity
+    components for atom (T_atom) and ion (T_ion = 10 uK, the listing's other temperature; reading S30) and a
+    normal ion position of standard deviation sqrt(k_B T_ion / m_ion) / omega, omega = (Omega/2) sqrt(ax + qx^2/2)."""
+    if positions not in ("uniform", "random") or collisiontype not in ("head-on", "thermal"):
+        raise ValueError("positions: 'uniform' | 'random'; collisiontype: 'head-on' | 'thermal'")
     Cm, _Re = potential_CnDe(4, 8, 159.5455, 1.0 * KB)
     ax = -2.982e-4
     w = Workload(name="paper", N=int(ntheta) * int(nphi), seed=0, kind="grid",
                  m_ion=170.936323 * AMU, m_atom=86.9091805310 * AMU, C4=159.5455, C8=Cm,
                  a=(ax, ax, -2.0 * ax), q=(0.219, -0.219, 0.0), omega_rf=omega_from_mhz(2.5),
                  r_exit=0.0, r_turn=500.0, max_steps=1_000_000,
-                 t_max=1000e-6 / AU_TIME_S, rtol=1e-10, atol=1e-20, T_ion=0.0, T_atom=1.0e-6, R0=5000.0, b_max=0.0,
-                 notes=dict(ntheta=int(ntheta), nphi=int(nphi), theta=tuple(theta), phi=tuple(phi)))
+                 t_max=1000e-6 / AU_TIME_S, rtol=1e-10, atol=1e-20,
+                 T_ion=10.0e-6 if collisiontype == "thermal" else 0.0, T_atom=1.0e-6, R0=5000.0, b_max=0.0,
+                 notes=dict(ntheta=int(ntheta), nphi=int(nphi), theta=tuple(theta), phi=tuple(phi),
+                            positions=positions, collisiontype=collisiontype))
     return w.replace(**overrides) if overrides else w
 
 
@@ -242,18 +250,55 @@ def grid_angles(w: Workload):
     return np.arccos(1.0 - 2.0 * u), np.linspace(p0, p1, nph)
 
 
+PAPER_DRAWS = 16  # uniforms per trajectory of a "grid" workload: 0-1 direction, 2-15 seven Box-Muller pairs
+
+
+def secular_frequency(w: Workload) -> float:
+    """omega = (Omega_rf / 2) sqrt(a_x + q_x^2 / 2): "the trap's secular frequency in the x direction" (PAPER.md:282)."""
+    return 0.5 * w.omega_rf * math.sqrt(w.a[0] + 0.5 * w.q[0] ** 2)
+
+
+def _paper_uniforms(seed: int, n: int, offset: int) -> np.ndarray:
+    bg = np.random.PCG64(seed)
+    if offset:
+        bg.advance(offset * PAPER_DRAWS)
+    return np.random.Generator(bg).random((n, PAPER_DRAWS))
+
+
 def _grid_y0(w: Workload, n: int, offset: int) -> np.ndarray:
     """eq. (12)-(13): atom at r0 (sin th cos ph, sin th sin ph, cos th) with velocity
     -v0 times the same unit vector, v0 = sqrt(3 k_B T / m_a); ion at rest at the origin.  Trajectory
-    i <-> (theta index i // nphi, phi index i % nphi)."""
-    th, ph = grid_angles(w)
-    idx = np.arange(offset, offset + n)
-    t, f = th[idx // len(ph)], ph[idx % len(ph)]
+    i <-> (theta index i // nphi, phi index i % nphi).  notes["positions"] = "random" draws the directions
+    (PAPER.md:483), notes["collisiontype"] = "thermal" the velocities and the ion position."""
+    positions = w.notes.get("positions", "uniform")
+    thermal = w.notes.get("collisiontype", "head-on") == "thermal"
+    U = _paper_uniforms(w.seed, n, offset) if (thermal or positions == "random") else None
+    if positions == "random":
+        (t0, t1), (p0, p1) = w.notes["theta"], w.notes["phi"]
+        u0, u1 = (1.0 - math.cos(t0)) / 2.0, (1.0 - math.cos(t1)) / 2.0
+        t = np.arccos(1.0 - 2.0 * (u0 + (u1 - u0) * U[:, 0]))
+        f = p0 + (p1 - p0) * U[:, 1]
+    else:
+        th, ph = grid_angles(w)
+        idx = np.arange(offset, offset + n)
+        t, f = th[idx // len(ph)], ph[idx % len(ph)]
     nhat = np.stack([np.sin(t) * np.cos(f), np.sin(t) * np.sin(f), np.cos(t)])
-    v0 = math.sqrt(3.0 * KB * w.T_atom / w.m_atom)
     y0 = np.zeros((12, n), dtype=np.float64)
     y0[6:9] = w.R0 * nhat
-    y0[9:12] = -v0 * nhat
+    if not thermal:
+        v0 = math.sqrt(3.0 * KB * w.T_atom / w.m_atom)
+        y0[9:12] = -v0 * nhat
+        return np.ascontiguousarray(y0)
+    # nine standard normals per trajectory: Box-Muller on explicit uniforms (pairs (2+2j, 3+2j))
+    two_pi = 2.0 * math.pi
+    rad = np.sqrt(-2.0 * np.log1p(-U[:, 2::2]))      # [n, 7]
+    ang = two_pi * U[:, 3::2]
+    z = np.concatenate([rad * np.cos(ang), rad * np.sin(ang)], axis=1)   # [n, 14] independent N(0, 1)
+    s_a = math.sqrt(KB * w.T_atom / w.m_atom)
+    s_i = math.sqrt(KB * w.T_ion / w.m_ion)
+    y0[9:12] = s_a * z[:, 0:3].T
+    y0[3:6] = s_i * z[:, 3:6].T
+    y0[0:3] = (s_i / secular_frequency(w)) * z[:, 6:9].T
     return np.ascontiguousarray(y0)
 
 

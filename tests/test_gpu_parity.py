@@ -540,6 +540,34 @@ def test_paper_grid_workload(aig):
     assert stats.ks_2samp(g["n_acc"], o["n_acc"]).pvalue > 0.01
 
 
+def test_paper_thermal_random_workload(aig):
+    """NEXT-2, the paper's other launch modes (PAPER.md:282 "thermal", :483 "random" positions): normal
+    velocities for both particles and a normal ion position in the trap, directions drawn uniformly over
+    the sphere.  Most atoms fly past (no bounce inside r_turn), the ion oscillates in the RF trap for the
+    whole span: accepted steps +-2, final states <= 1e-6 on everything with at most one bounce, bounce
+    counts equal there; the first-bounce record is NaN exactly where there was none."""
+    w = inputs.paper_workload(12, 12, theta=(0.0, math.pi), phi=(0.0, 2 * math.pi), positions="random",
+                              collisiontype="thermal", t_max=2.0e12)
+    y0 = inputs.generate_y0(w)
+    g = run_gpu(aig, w, y0, position=True)
+    po = orc.make_params(**w.params())
+    o = orc.integrate(po, y0, w.t_max, w.rtol, w.atol, threads=8)
+    y1 = y0.copy()
+    y1[6:9] = np.nextafter(y1[6:9], np.inf)
+    o1 = orc.integrate(po, y1, w.t_max, w.rtol, w.atol, threads=8)
+    assert np.all(g["status"] == 1) and np.all(o["status"] == 1) and np.all(g["t_final"] == w.t_max)
+    d = (g["n_turn"] <= 1) & (o["n_turn"] <= 1) & (o1["n_turn"] <= 1)
+    assert d.sum() >= 100 and (g["n_turn"] == 0).sum() >= 50 and (g["n_turn"] >= 1).sum() >= 10
+    assert np.max(np.abs(g["n_acc"][d].astype(int) - o["n_acc"][d].astype(int))) <= 2
+    assert np.array_equal(g["n_turn"][d], o["n_turn"][d])
+    rel, ref = block_rel(g["y_final"], o["y_final"]), block_rel(o1["y_final"], o["y_final"])
+    assert rel[d].max() <= 1e-6 or rel[d].max() <= 30 * ref[d].max() + 1e-9, (rel[d].max(), ref[d].max())
+    miss = d & (o["n_turn"] == 0)
+    assert rel[miss].max() <= 1e-6 and np.max(np.abs(g["r_min"][miss] / o["r_min"][miss] - 1)) <= 1e-6
+    assert np.array_equal(np.isnan(g["x_turn1"]).any(axis=0), g["n_turn"] == 0)
+    assert np.min(g["n_acc"]) > 5000     # the ion's micromotion alone takes ~100 steps per RF period
+
+
 def test_paper_complex_probability(aig):
     """The one physics number the paper prints for its production run: 59.87 % of the head-on trajectories
     form a complex (tests/golden/paper_constants.txt).  A 100 x 100 full-sphere grid of the same

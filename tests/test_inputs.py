@@ -2,6 +2,7 @@
 import math
 
 import numpy as np
+import pytest
 
 from paper_2509_12381_b200 import inputs
 
@@ -107,3 +108,51 @@ def test_paper_grid_workload():
     # the paper's printed derived constants (Fig. 10): Cm and tmax
     assert abs(w.C8 / 2.00949488627505397797e+09 - 1) < 1e-13
     assert abs(w.t_max * inputs.AU_TIME_S - 1e-3) < 1e-15
+
+
+def test_paper_random_positions_and_thermal_mode():
+    """NEXT-2, PAPER.md:483 ("random" positions: uniform in solid angle inside the window) and :282
+    ("thermal": normal velocity components of standard deviation sqrt(k_B T / m), normal ion position of
+    standard deviation sqrt(k_B T_ion / m_ion) / omega, omega = (Omega/2) sqrt(ax + qx^2/2))."""
+    n_t, n_p = 200, 200
+    w = inputs.paper_workload(n_t, n_p, theta=(0.3, 2.0), phi=(0.5, 4.0), positions="random", collisiontype="thermal")
+    y0 = inputs.generate_y0(w)
+    n = n_t * n_p
+    assert y0.shape == (12, n)
+    r = np.linalg.norm(y0[6:9], axis=0)
+    assert np.allclose(r, 5000.0, rtol=1e-14)
+    cth = y0[8] / r
+    phi = np.mod(np.arctan2(y0[7], y0[6]), 2 * math.pi)
+    assert cth.min() >= math.cos(2.0) - 1e-12 and cth.max() <= math.cos(0.3) + 1e-12
+    assert phi.min() >= 0.5 - 1e-12 and phi.max() <= 4.0 + 1e-12
+    # uniform in solid angle: cos(theta) and phi uniform on their windows (Kolmogorov-Smirnov)
+    from scipy import stats
+    assert stats.kstest(cth, stats.uniform(math.cos(2.0), math.cos(0.3) - math.cos(2.0)).cdf).pvalue > 1e-3
+    assert stats.kstest(phi, stats.uniform(0.5, 3.5).cdf).pvalue > 1e-3
+    # the nine normal components: zero mean, the stated standard deviations, uncorrelated
+    s_a = math.sqrt(inputs.KB * 1.0e-6 / w.m_atom)
+    s_i = math.sqrt(inputs.KB * 10.0e-6 / w.m_ion)
+    om = 0.5 * (2 * math.pi * 2.5e6 * inputs.AU_TIME_S) * math.sqrt(-2.982e-4 + 0.5 * 0.219 ** 2)
+    assert abs(inputs.secular_frequency(w) / om - 1) < 1e-12
+    assert abs(om / inputs.AU_TIME_S / (2 * math.pi) / 192.36e3 - 1) < 1e-3      # ~192 kHz for the listing's trap
+    Z = np.vstack([y0[9:12] / s_a, y0[3:6] / s_i, y0[0:3] / (s_i / om)])
+    tol = 5.0 / math.sqrt(n)
+    assert np.max(np.abs(Z.mean(axis=1))) < tol
+    assert np.max(np.abs(Z.std(axis=1) - 1)) < tol
+    Cc = np.corrcoef(Z)
+    assert np.max(np.abs(Cc - np.eye(9))) < tol
+    for k in range(9):
+        assert stats.kstest(Z[k], "norm").pvalue > 1e-4, k
+    # slices of the stream reproduce (sharding), head-on grid unchanged by the new arguments
+    assert np.array_equal(inputs.generate_y0(w, n=9, offset=1234), y0[:, 1234:1243])
+    g0 = inputs.generate_y0(inputs.paper_workload(12, 7))
+    g1 = inputs.generate_y0(inputs.paper_workload(12, 7, positions="uniform", collisiontype="head-on"))
+    assert np.array_equal(g0, g1) and np.all(g0[0:6] == 0)
+    # mixed modes: grid directions with thermal velocities; random directions head-on
+    gt = inputs.generate_y0(inputs.paper_workload(12, 7, collisiontype="thermal"))
+    assert np.array_equal(gt[6:9], g0[6:9]) and np.all(gt[0:6] != 0)
+    rh = inputs.generate_y0(inputs.paper_workload(12, 7, positions="random"))
+    v = np.linalg.norm(rh[9:12], axis=0)
+    assert np.all(rh[0:6] == 0) and np.allclose(rh[9:12] / v, -rh[6:9] / 5000.0, atol=1e-15)
+    with pytest.raises(ValueError):
+        inputs.paper_workload(4, 4, positions="grid")
