@@ -876,29 +876,74 @@ struct OutlierArgs {
     long long* result;             // [kOutlierObs][2]: index of the minimum, of the maximum
 };
 
-__global__ void __launch_bounds__(256)
+// the eight observables of trajectory i as doubles (a missing position array reads NaN: skipped)
+__device__ __forceinline__ void outlier_load(const OutlierArgs& a, long long i, double (&x)[kOutlierObs])
+{
+    x[0] = a.angle[i];
+    x[1] = (double)a.n_turn[i];
+    x[2] = a.lifetime[i];
+    x[3] = a.transfer[i];
+    x[4] = a.dist[i];
+    x[5] = (double)a.n_acc[i];
+    x[6] = a.ke[i];
+    x[7] = a.position ? a.position[i] : nan("");
+}
+// a thread visits its indices in ascending order, so a strict comparison keeps the smallest index of a
+// tie; the running extrema carry the visit number (32 bits; -1 = nothing yet), not the index
+struct Running {
+    double v;
+    int n;
+};
+__device__ __forceinline__ void outlier_fold(const double (&x)[kOutlierObs], int n, Running (&lo)[kOutlierObs],
+                                             Running (&hi)[kOutlierObs])
+{
+#pragma unroll
+    for (int k = 0; k < kOutlierObs; ++k) {
+        const bool ok = (x[k] == x[k]);
+        const bool tl = ok & ((x[k] < lo[k].v) | (lo[k].n < 0));
+        const bool th = ok & ((x[k] > hi[k].v) | (hi[k].n < 0));
+        lo[k].v = tl ? x[k] : lo[k].v;
+        lo[k].n = tl ? n : lo[k].n;
+        hi[k].v = th ? x[k] : hi[k].v;
+        hi[k].n = th ? n : hi[k].n;
+    }
+}
+
+__global__ void __launch_bounds__(256, 2)
 outliers_kernel(const OutlierArgs a, const long long N)
 {
     __shared__ Extreme s_part[8][kOutlierObs][2];
     __shared__ bool s_last;
+    Running rlo[kOutlierObs], rhi[kOutlierObs];
+#pragma unroll
+    for (int k = 0; k < kOutlierObs; ++k) {
+        rlo[k].v = rhi[k].v = 0.0;
+        rlo[k].n = rhi[k].n = -1;
+    }
+    // two trajectories per iteration, all sixteen loads issued before the first comparison (HBM latency)
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long start = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long i = start;
+    int n = 0;  // visit number: index = start + n * stride
+    for (; i + stride < N; i += 2 * stride, n += 2) {
+        double x0[kOutlierObs], x1[kOutlierObs];
+        outlier_load(a, i, x0);
+        outlier_load(a, i + stride, x1);
+        outlier_fold(x0, n, rlo, rhi);
+        outlier_fold(x1, n + 1, rlo, rhi);
+    }
+    if (i < N) {
+        double x0[kOutlierObs];
+        outlier_load(a, i, x0);
+        outlier_fold(x0, n, rlo, rhi);
+    }
     Extreme lo[kOutlierObs], hi[kOutlierObs];
 #pragma unroll
     for (int k = 0; k < kOutlierObs; ++k) {
-        lo[k].v = hi[k].v = 0.0;
-        lo[k].i = hi[k].i = -1;
-    }
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
-        const double x[kOutlierObs] = {a.angle[i],    (double)a.n_turn[i], a.lifetime[i], a.transfer[i],
-                                       a.dist[i],     (double)a.n_acc[i],  a.ke[i],       a.position ? a.position[i] : nan("")};
-#pragma unroll
-        for (int k = 0; k < kOutlierObs; ++k) {
-            if (x[k] == x[k]) {
-                const Extreme e{x[k], i};
-                lo[k] = pick_min(lo[k], e);
-                hi[k] = pick_max(hi[k], e);
-            }
-        }
+        lo[k].v = rlo[k].v;
+        lo[k].i = rlo[k].n < 0 ? -1 : start + (long long)rlo[k].n * stride;
+        hi[k].v = rhi[k].v;
+        hi[k].i = rhi[k].n < 0 ? -1 : start + (long long)rhi[k].n * stride;
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -932,6 +977,7 @@ outliers_kernel(const OutlierArgs a, const long long N)
         const int k = act ? (c >> 1) : 0, m = c & 1;
         Extreme e{0.0, -1};
         if (act)
+#pragma unroll 4
             for (unsigned b = sub; b < gridDim.x; b += 16) {
                 const Extreme f = a.partial[((size_t)b * kOutlierObs + k) * 2 + m];
                 e = m ? pick_max(e, f) : pick_min(e, f);
@@ -1584,7 +1630,9 @@ int aig_outliers(const aig_out* out, const aig_obs_extra* extra, int64_t N, int6
     a.ticket = static_cast<unsigned int*>(workspace);
     a.partial = reinterpret_cast<Extreme*>(static_cast<unsigned char*>(workspace) + 256);
     a.result = reinterpret_cast<long long*>(result);
-    long long blocks = std::min<long long>(std::max<long long>(1, (N + 255) / 256), std::min<long long>((long long)sms * 4, kOutlierBlocksMax));
+    int occ = 0;  // one wave of resident blocks: the last block to finish folds the partials
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, outliers_kernel, 256, 0) != cudaSuccess || occ < 1) return AIG_ERR_CUDA;
+    long long blocks = std::min<long long>(std::max<long long>(1, (N + 255) / 256), std::min<long long>((long long)sms * occ, kOutlierBlocksMax));
     outliers_kernel<<<(unsigned)blocks, 256, 0, st>>>(a, N);
     g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
