@@ -316,6 +316,11 @@ def run_ours(args) -> int:
         cpu = {"value": args.cpu_sample / dt, "unit": "trajectories/s", "cores": cores, "kind": "oracle",
                "sample": f"first {args.cpu_sample} trajectories of the bench workload, {cores} threads, {dt:.2f} s wall",
                "accepted_steps_per_s": a / dt}
+        # the same oracle single-threaded on one core, over a shorter prefix
+        n1 = min(args.cpu_sample, 32768)
+        dt1, a1, _r1 = _oracle_sample(w, n1, 1)
+        cpu["one_core"] = {"value": n1 / dt1, "unit": "trajectories/s", "accepted_steps_per_s": a1 / dt1,
+                           "sample": f"first {n1} trajectories, 1 thread, {dt1:.2f} s wall"}
 
     if rank == 0:
         line = {
