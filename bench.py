@@ -110,6 +110,16 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def _measured_hbm_gbs():
+    """(GB/s, "measured" | "fallback"): HBM copy rate of this pool's B200s as the driver measured it
+    (MEASURED_PEAKS.json), else the profiling guide's fallback figure."""
+    try:
+        with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return 6650.0, "fallback"
+
+
 def _oracle_sample(w, n_sample: int, threads: int):
     """Time the oracle, as it stands, on the first n_sample trajectories of workload w."""
     from oracle import aig_oracle as orc
@@ -307,6 +317,37 @@ def run_ours(args) -> int:
                               "alg_tflops_per_gpu": tf, "frac_fp64_peak": tf * 1e12 / FP64_PEAK_NOMINAL,
                               "complex_fraction": c / (world * N)})
 
+    # ---- the widening kernels, outside the timed region: aig_observables and
+    #      aig_outliers over the bench workload's results, each timed alone with CUDA events, L2 flushed
+    side = None
+    if world == 1 and not args.no_side:
+        hbm, hbm_kind = _measured_hbm_gbs()
+        outp = aig.alloc_out(N, dev, position=True)
+        p = aig.make_params(**w.params())
+        aig.aig_integrate(p, y0, w.t_max, w.rtol, w.atol, out=outp, workspace=ws)
+        extra = aig.aig_observables(p, y0, outp)
+        aig.aig_outliers(outp, extra)
+        torch.cuda.synchronize()
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+        side = {}
+        # algorithmic bytes per trajectory: observables 12 + 3 + 3 doubles in, 4 out; outliers 6 doubles + 2 int32 in
+        for name, fn, bpt in (("observables_kernel", lambda: aig.aig_observables(p, y0, outp, extra=extra), 176),
+                              ("outliers_kernel", lambda: aig.aig_outliers(outp, extra), 56)):
+            ts = []
+            for _ in range(5):
+                flush.zero_()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                fn()
+                b.record()
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            ms = float(np.median(ts))
+            gbs = bpt * N / (ms * 1e-3) / 1e9
+            side[name] = {"us": round(ms * 1e3, 1), "bytes_per_trajectory": bpt, "achieved_gbs": round(gbs, 1),
+                          "peak_gbs": hbm, "peak_kind": hbm_kind, "frac": round(gbs / hbm, 3), "bound": "hbm"}
+        del outp, extra, flush
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import aig_oracle as orc
@@ -349,7 +390,7 @@ def run_ours(args) -> int:
                          "hbm_bytes_algorithmic": 241 * N},
             "kernel": info,
             "e2e": e2e, "gpu_launches": int(launches_timed), "clocks": clocks,
-            "cpu_baseline": cpu, "sweep": sweep,
+            "cpu_baseline": cpu, "side_kernels": side, "sweep": sweep,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -367,6 +408,7 @@ def main() -> int:
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-side", action="store_true", help="skip timing aig_observables / aig_outliers")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=2097152)
     ap.add_argument("--ref-sample", type=int, default=262144)
