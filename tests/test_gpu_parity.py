@@ -668,9 +668,7 @@ def test_histogram_exact(aig):
     n = 5000  # several blocks + ragged tail
     y0 = inputs.generate_y0(w.replace(seed=11), n=n)
     p = aig.make_params(**w.params())
-    # configs[4] exactly as bench.py launches it; configs[3] also records the first-bounce position
-    bufs = aig.alloc_out(w.N, "cuda", position=True) if cfg == 3 else None
-    out = aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol, out=bufs)
+    out = aig.aig_integrate(p, _dev(y0), w.t_max, w.rtol, w.atol)
     ae, le = inputs.histogram_edges()
     hist = aig.aig_histogram(out, _dev(ae), _dev(le), 64)
     H = aig.hist_to_numpy(hist)
