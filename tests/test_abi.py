@@ -56,7 +56,7 @@ def test_version_strerror_workspace(lib):
 
 
 def test_struct_layouts_match_header():
-    # aig_params: 13 doubles + int64 ; aig_out: 10 pointers ; aig_hist_spec: ptr,i32,ptr,i32,i32
+    # aig_params: 14 doubles + int64 + 2 int32 ; aig_out: 10 pointers + optional x_turn1 ; aig_hist_spec: ptr,i32,ptr,i32,i32
     assert C.sizeof(binding.Params) == 14 * 8 + 8 + 8  # 14 doubles (2+2+3+3+1+1+1+1) + int64 + 2 int32
     assert binding.Params.n_att.offset == 15 * 8 and binding.Params.n_rep.offset == 15 * 8 + 4
     assert binding.Params.max_steps.offset == 14 * 8
