@@ -89,6 +89,15 @@ def test_argument_validation_happens_before_any_device_work(lib):
     spec = binding.HistSpec(0x1000, 0, 0x1000, 4, 4)
     h = binding.Hist(*([0x1000] * 5))
     assert lib.aig_histogram(C.byref(o2), 4, C.byref(spec), C.byref(h), None) == -2
+    # the optional first-bounce record: a misaligned x_turn1 is rejected; position needs x_turn1
+    o3 = binding.Out(*([0x1000] * 10), 0x1004)
+    assert lib.aig_integrate(C.byref(p), 0x1000, 4, 1.0, 1e-6, 0.0, C.byref(o3), 0x1000, None) == -6
+    lib.aig_observables.restype = C.c_int
+    lib.aig_observables.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    ex = binding.ObsExtra(0x1000, 0x1000, 0x1000, 0x1000)
+    assert lib.aig_observables(C.byref(p), 0x1000, C.byref(o2), 4, C.byref(ex), None) == -1
+    ex_bad = binding.ObsExtra(0x1000, 0x1000, 0x1000, 0x1004)
+    assert lib.aig_observables(C.byref(p), 0x1000, C.byref(o3), 4, C.byref(ex_bad), None) == -6
 
 
 def test_no_cpu_fallback_without_cuda():
