@@ -24,8 +24,13 @@
  * Hamiltonian eq. (1)-(2), exact free motion, the harmonic-trap closed form
  * (PAPER.md:432), Mathieu stability / secular frequency, two-body
  * conservation laws, the Langevin capture fraction, the classical deflection-angle
- * quadrature, and DOP853 cross-checks.  Parity UNPINNED pointwise for complex-forming
- * (chaotic) trajectories: ensemble statistics only.
+ * quadrature, and DOP853 cross-checks; the step-size controller (O3.3-O3.7: safety factors,
+ * exponent, growth limit and its threshold, shrink floor, halving, kept step after a failure,
+ * hmin = 16 ulp, last-step stretch, both ends of the step in the error scale) on the
+ * quadrature problem y' = A t^4, where err = |A| (71/270000) h^5 / thr exactly and every step
+ * sequence is computable by hand; lifetime / first / last bounce by a NumPy recomputation
+ * from the replay record.  Parity UNPINNED pointwise for complex-forming (chaotic)
+ * trajectories: ensemble statistics only.
  */
 #include <math.h>
 #include <stdint.h>

@@ -114,6 +114,137 @@ def test_controller_rejects_and_recovers():
     assert abs(r["y"][0] - exact) < 1e-4 * abs(exact) + 1e-5
 
 
+# ------------------------------------------------------------------------------------------
+# the step-size controller ("exactly the same" as ode45:
+# reading S1).  Pinned on the quadrature problem y' = A t^4, where everything is computable by hand:
+# a Runge-Kutta pair of orders 5(4) integrates t^4 exactly with its 5th-order weights, and its error
+# estimate sum_j E_j f(t + c_j h) = A h^4 sum_j E_j c_j^4 (the lower powers vanish by the order
+# conditions) does not depend on t.  With the published tableau kappa = sum_j E_j c_j^4 = 71/270000,
+# so with thr = atol/rtol above |y| the scaled estimate is err = |A| kappa h^5 / thr EXACTLY, and
+#     err(h)/rtol = (h/h*)^5,   h* = (rtol thr / (|A| kappa))^(1/5).
+# ode45's rule then gives hand-computable step sequences:
+#   accepted, no failure:  h <- h / (1.25 (err/rtol)^(1/5)) = 0.8 h*  whatever h was, unless
+#                          1.25 (err/rtol)^(1/5) <= 0.2, i.e. h <= 0.16 h*: then h <- 5 h
+#   first failure:         h <- h max(0.1, 0.8 (rtol/err)^(1/5)) = max(0.1 h, 0.8 h*);  later ones: h/2
+#   after a step that had a failure the step size is kept
+# ------------------------------------------------------------------------------------------
+from fractions import Fraction as _F
+
+_DP_C = [_F(0), _F(1, 5), _F(3, 10), _F(4, 5), _F(8, 9), _F(1), _F(1)]            # Dormand & Prince 1980
+_DP_E = [_F(71, 57600), _F(0), _F(-71, 16695), _F(71, 1920), _F(-17253, 339200), _F(22, 525), _F(-1, 40)]
+_KAPPA = sum(e * c**4 for e, c in zip(_DP_E, _DP_C))
+
+
+def _quartic(A=1.0, B=0.0):
+    return lambda t, y: np.array([A * t**4 + B * t])
+
+
+def _hstar(rtol, thr, A=1.0):
+    return (rtol * thr / (abs(A) * float(_KAPPA))) ** 0.2
+
+
+def test_controller_error_constant_of_the_pair():
+    assert _KAPPA == _F(71, 270000)
+    assert all(sum(e * c**k for e, c in zip(_DP_E, _DP_C)) == 0 for k in range(4))
+    # one attempted step of the oracle: err = |A| kappa h^5 / thr whatever t is
+    for t, h in ((0.0, 0.5), (3.0, 0.25), (-2.0, 0.125)):
+        _, err = orc.generic_step(_quartic(2.0), t, np.array([0.0]), h, rtol=1e-3, atol=1e3)   # thr = 1e6
+        assert abs(err / (2.0 * float(_KAPPA) * h**5 / 1e6) - 1) < 1e-7
+
+
+def test_controller_steady_step_growth_limit_and_safety_factor():
+    rtol, atol = 1e-12, 1e-6                      # thr = 1e6 stays above |y| = t^5/5
+    hs = _hstar(rtol, atol / rtol)
+    for frac, second in ((0.12, 5 * 0.12), (0.15, 5 * 0.15), (0.18, 0.8), (0.5, 0.8)):
+        # the initial-step rule gives h0 = 0.8 rtol^(1/5) thr / f(t0); choose t0 so that h0 = frac h*
+        t0 = (0.8 * rtol**0.2 * (atol / rtol) / (frac * hs)) ** 0.25
+        r = orc.generic_integrate(_quartic(), t0, np.array([0.0]), t0 + 400 * hs, rtol, atol, cap=16)
+        steps = np.diff(np.concatenate([[t0], r["trace_t"][:8]])) / hs
+        assert r["n_rej"] == 0
+        # frac <= 0.16: growth limit 5 (then 0.8 h* from 0.6 h* or 0.75 h*); above: straight to 0.8 h*
+        expect = [frac, second] + [0.8] * 6
+        # tolerance: sum_j E_j k_j cancels from ~t^4 down to kappa h^4, so err carries a relative rounding
+        # noise ~ eps (t/h)^4 / kappa (2.7e-5 in h for the 0.18 h* step); every misreading of the rule is > 1 %
+        assert np.allclose(steps, expect, rtol=1e-4, atol=0), (frac, steps)
+        assert np.allclose(steps[3:], 0.8, rtol=2e-6, atol=0), (frac, steps)
+
+
+def test_controller_exponent_is_one_fifth():
+    # the steady step 0.8 h* scales as rtol^(1/5): a factor 10^5 in rtol is a factor 10 in h
+    thr = 1e6
+    h = []
+    for rtol in (1e-9, 1e-14):
+        r = orc.generic_integrate(_quartic(), 0.0, np.array([0.0]), 100 * _hstar(rtol, thr), rtol, rtol * thr, cap=8)
+        h.append(np.diff(r["trace_t"][:8])[-1])
+    assert abs(h[0] / h[1] / 10.0 - 1) < 1e-5
+    assert abs(h[0] / (0.8 * _hstar(1e-9, thr)) - 1) < 1e-5
+
+
+def test_controller_failed_attempts_shrink_floor_halving_and_kept_step():
+    rtol, atol = 1e-12, 1e-6
+    hs = _hstar(rtol, atol / rtol)
+    # f(0) = 0, so the first attempt is hmax = span/10.  (a) hmax = 24 h*: 0.8 (rtol/err)^(1/5) = 1/30 is
+    # below the floor 0.1 -> 2.4 h* (fails), halved -> 1.2 h* (fails), halved -> 0.6 h* (accepted):
+    # three rejections; the step size is kept after a step with failures, then 0.8 h* for good
+    r = orc.generic_integrate(_quartic(), 0.0, np.array([0.0]), 240 * hs, rtol, atol, cap=8)
+    assert r["n_rej"] == 3
+    assert np.allclose(r["trace_t"][:5] / hs, [0.6, 1.2, 2.0, 2.8, 3.6], rtol=2e-6, atol=0)
+    # (b) hmax = 3 h*: one rejection, 3 h* x 0.8 (1/243)^(1/5) = 0.8 h* (above the floor), kept once
+    r = orc.generic_integrate(_quartic(), 0.0, np.array([0.0]), 30 * hs, rtol, atol, cap=8)
+    assert r["n_rej"] == 1
+    assert np.allclose(r["trace_t"][:4] / hs, [0.8, 1.6, 2.4, 3.2], rtol=2e-6, atol=0)
+    # (c) hmax = 1.5 h*: 1.5 x 0.8 / 1.5 = 0.8 h* again (the shrink aims at err = 0.8^5 rtol)
+    r = orc.generic_integrate(_quartic(), 0.0, np.array([0.0]), 15 * hs, rtol, atol, cap=8)
+    assert r["n_rej"] == 1 and abs(r["trace_t"][0] / hs / 0.8 - 1) < 2e-6
+
+
+def test_controller_hmin_is_16_ulp_and_nan_shrinks_by_the_floor():
+    # a NaN right-hand side from t0 = 1, span 10 (hmax = 1): attempts at 1, then the floor 0.1, then
+    # halved each time: 0.1/2^m > hmin = 16 ulp(1) = 2^-48 up to m = 44 (5.7e-15 > 3.6e-15), the next
+    # attempt is clamped to hmin and is the last: 1 + 45 + 1 = 47 rejections, nothing accepted
+    g = lambda t, y: np.array([float("nan")])
+    r = orc.generic_integrate(g, 1.0, np.array([1.0]), 11.0, 1e-6, 1e-9)
+    assert r["status"] == 3 and r["n_acc"] == 0 and r["t"] == 1.0 and r["n_rej"] == 47
+    # hmin follows the spacing of doubles at t: from t0 = 2^20 it is 2^-28; 0.1/2^m > 2^-28 up to m = 24
+    r = orc.generic_integrate(g, 2.0**20, np.array([1.0]), 2.0**20 + 10.0, 1e-6, 1e-9)
+    assert r["status"] == 3 and r["n_rej"] == 27
+
+
+def test_controller_last_step_is_stretched_by_up_to_ten_percent():
+    rtol, atol = 1e-12, 1e-6
+    hs = _hstar(rtol, atol / rtol)
+    # steady steps of 0.8 h* (first attempt hmax < 8 h* fails once and lands on 0.8 h*, see above):
+    # with t_max = (36 + 1.05) x 0.8 h* the 37th step is stretched to 1.05 x 0.8 h* (1.1 h >= remainder);
+    # with 1.15 it is not: a 37th regular step and a short 38th
+    for tail, n_acc in ((1.05, 37), (1.15, 38), (0.4, 37)):
+        t_max = (36 + tail) * 0.8 * hs
+        r = orc.generic_integrate(_quartic(), 0.0, np.array([0.0]), t_max, rtol, atol, cap=64)
+        assert r["status"] == 1 and r["t"] == t_max and r["n_rej"] == 1
+        assert r["n_acc"] == n_acc, (tail, r["n_acc"])
+        assert abs(r["trace_t"][35] / (36 * 0.8 * hs) - 1) < 1e-5
+        assert abs(r["y"][0] / (t_max**5 / 5) - 1) < 1e-12        # t^4 is integrated exactly
+
+
+def test_error_scale_uses_both_ends_of_the_step():
+    # err = h |sum E k| / max(|y|, |ynew|, thr) with thr = 1e-30 out of the way.
+    # y' = A t^4 + B t from y(0) = 0: |y| = 0, so the scale is |ynew| = B h^2/2 + A h^5/5
+    A, B, h = 3.0, 2.0, 0.5
+    ynew, err = orc.generic_step(_quartic(A, B), 0.0, np.array([0.0]), h, rtol=1.0, atol=1e-30)
+    assert abs(ynew[0] / (B * h**2 / 2 + A * h**5 / 5) - 1) < 1e-14
+    assert abs(err / (A * float(_KAPPA) * h**5 / ynew[0]) - 1) < 1e-9
+    # and from y(0) = -1 with ynew closer to zero: the scale is |y|
+    ynew, err = orc.generic_step(_quartic(A, B), 0.0, np.array([-1.0]), h, rtol=1.0, atol=1e-30)
+    assert abs(ynew[0]) < 1.0 and abs(err / (A * float(_KAPPA) * h**5 / 1.0) - 1) < 1e-9
+    # with thr above both, the scale is thr
+    ynew, err = orc.generic_step(_quartic(A, B), 0.0, np.array([-1.0]), h, rtol=1e-3, atol=1e-2)
+    assert abs(err / (A * float(_KAPPA) * h**5 / 10.0) - 1) < 1e-9
+    # in the loop: the first attempt (hmax, because f(0) = 0) is accepted at once when the scale is |ynew|
+    hmax = 0.5
+    A = 0.5**5 * 1e-6 * (B * hmax**2 / 2) / (float(_KAPPA) * hmax**5)      # err(hmax) ~ rtol / 32
+    r = orc.generic_integrate(_quartic(A, B), 0.0, np.array([0.0]), 10 * hmax, 1e-6, 1e-36, cap=4)
+    assert r["n_rej"] == 0 and r["trace_t"][0] == hmax
+
+
 def test_max_steps_and_failure_status():
     f = lambda t, y: -y
     r = orc.generic_integrate(f, 0.0, np.array([1.0]), 10.0, 1e-10, 1e-13, max_steps=7)
@@ -648,6 +779,38 @@ def test_position_against_replay_brute_force():
         else:
             assert np.all(np.isnan(o["x_turn1"][:, i]))
     assert seen >= 10
+
+
+def test_lifetime_first_and_last_bounce_against_replay_brute_force():
+    """PAPER.md:495: "lifetime ... the amount of time between the first and last bounce".  Recomputed from
+    the replay record with NumPy for multi-bounce trajectories of config 2 (q = 0.2): the counted turning
+    points are the sign changes - to + of s = d.u at accepted step ends with r < r_turn (readings S5, S7),
+    lifetime = t(last) - t(first), complex <=> at least two, to the bit; with r_turn = 50 a0 as well (the
+    short-range complexes, several bounces each)."""
+    w = inputs.config(2).replace(N=4096)
+    y0 = inputs.generate_y0(w)
+    checked = {math.inf: 0, 50.0: 0}
+    many = 0
+    for r_turn in (math.inf, 50.0):
+        kw = {**w.params(), "r_turn": r_turn}
+        p = orc.make_params(**kw)
+        o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol, threads=8)
+        multi = np.flatnonzero(o["n_turn"] >= 2)
+        assert len(multi) >= 10
+        for i in multi[:16]:
+            t, y, _ = orc.integrate_trace(p, y0[:, i], w.t_max, w.rtol, w.atol)
+            rows = np.vstack([y0[:, i][None, :], y])
+            d, u = rows[:, 6:9] - rows[:, 0:3], rows[:, 9:12] - rows[:, 3:6]
+            s, r = np.sum(d * u, axis=1), np.linalg.norm(d, axis=1)
+            hit = np.flatnonzero((s[:-1] < 0) & (s[1:] >= 0) & (r[1:] < r_turn))
+            assert len(hit) == o["n_turn"][i] and o["complex_flag"][i] == 1
+            assert o["lifetime"][i] == t[hit[-1]] - t[hit[0]] and o["lifetime"][i] > 0
+            assert len(t) == o["n_acc"][i] and t[-1] == o["t_final"][i]
+            checked[r_turn] += 1
+            many += len(hit) >= 3
+        single = np.flatnonzero(o["n_turn"] == 1)[:4]
+        assert np.all(o["lifetime"][single] == 0) and np.all(o["complex_flag"][single] == 0)
+    assert checked[math.inf] >= 10 and checked[50.0] >= 10 and many >= 5
 
 
 def test_outliers_definition():
