@@ -167,14 +167,15 @@ __device__ __forceinline__ double trap_w(double wa, double wb, double cs)
     return (trap_of(TRAP) == TRAP_STATIC) ? wa : fma(wb, cs, wa);
 }
 
-// Accelerations of both particles at positions (xi, xa), cos(Omega t) = cs.
-// eq. (4)-(6): ion  acc_k = -(1/m_i)(dV/dr)(d_k/r) - w_k(t) x_k  [the trap product first: it does not wait for 1/r^2];  eq. (8)-(10): atom acc_k = +(1/m_a)(dV/dr)(d_k/r)
-// with d = x_ion - x_atom.  X = (xi, xa), Aout = (Ai, Aa).
+// Accelerations of both particles from the relative position D = x_ion - x_atom and the ion position
+// Xi (the trap acts on the ion only), cos(Omega t) = cs.
+// eq. (4)-(6): ion  acc_k = -(1/m_i)(dV/dr)(d_k/r) - w_k(t) x_k  [the trap product first: it does not wait for 1/r^2];  eq. (8)-(10): atom acc_k = +(1/m_a)(dV/dr)(d_k/r).
+// Aout = (Ai, Aa).
 template <int TRAP>
-__device__ __forceinline__ void accel(const KParams& P, double cs, const double (&X)[6], double (&Aout)[6],
-                                      double& r2_out)
+__device__ __forceinline__ void accel(const KParams& P, double cs, const double (&D)[3], const double (&Xi)[3],
+                                      double (&Aout)[6], double& r2_out)
 {
-    const double d0 = X[0] - X[3], d1 = X[1] - X[4], d2 = X[2] - X[5];
+    const double d0 = D[0], d1 = D[1], d2 = D[2];
     const double r2 = sum3(d0 * d0, d1 * d1, d2 * d2);
     double gi, ga;
     force_factors<TRAP>(P, r2, gi, ga);
@@ -190,26 +191,38 @@ __device__ __forceinline__ void accel(const KParams& P, double cs, const double 
         for (int k = 0; k < 3; ++k) {
             const double w = trap_w<TRAP>(P.wa[k], P.wb[k], cs);
             const double dk = (k == 0) ? d0 : (k == 1 ? d1 : d2);
-            Aout[k] = fma(gi, dk, -(w * X[k]));
+            Aout[k] = fma(gi, dk, -(w * Xi[k]));
         }
     }
     r2_out = r2;
 }
 
-// Position component of stage S+1 (S = 1..6): x + c h v + h^2 sum_{l <= S-2} abar_{S,l} A_l
-// (older stages first, so the newest acceleration closes the chain).  A[l] = this component's A_l.
+// Stage positions (Nystrom form).  Stage S+1 (S = 1..6) sits at x + c h v + h^2 sum_{l <= S-2} abar_{S,l} A_l
+// (older stages first, so the newest acceleration closes the chain); A[l] = this component's A_l.
+// The force needs the RELATIVE position d = x_ion - x_atom, at the repulsive wall to far better than
+// the spacing of doubles at |x| ~ 1e3 a0 (the force goes as r^-9 with r ~ 7.6 a0: a difference of two
+// rounded lab-frame stage positions would carry eps |x| / r ~ 1e-14 into r and ten times that into the
+// force).  So the relative position has a chain of its own, started from d(t) = x_ion - x_atom and
+// u(t) = v_ion - v_atom at the beginning of the step:
+//     d_s = d + c h u + h^2 (acc_ion - acc_atom),   acc = sum_l abar_{S,l} A_l,
+// accurate to the spacing of doubles at |d|.  The ion's own stage position is still formed (the trap
+// force needs it, to ordinary accuracy), the atom's only at the step end (stage 7 = the new state).
 template <int S>
-__device__ __forceinline__ double stage_pos(double x, double v, double hc, double h2, const double (&A)[7])
+__device__ __forceinline__ double stage_acc(const double (&A)[7])
 {
-    const double base = fma(hc, v, x);
-    if (S < 2) return base;
+    static_assert(S >= 2 && S <= 6, "stages 3..7");
     double acc = kAbar[S][0] * A[0];
 #pragma unroll
     for (int l = 1; l <= S - 2; ++l) {
         if (S == 6 && l == 1) continue;  // abar_72 = 0 exactly
         acc = fma(kAbar[S][l], A[l], acc);
     }
-    return fma(h2, acc, base);
+    return acc;
+}
+// x + c h v + h^2 acc  (also the relative position, with x -> d, v -> u, acc -> acc_ion - acc_atom)
+__device__ __forceinline__ double stage_pos(double x, double v, double hc, double h2, double acc)
+{
+    return fma(h2, acc, fma(hc, v, x));
 }
 
 // 16 * (spacing of doubles above |t|): ode45's hmin = 16 eps(t)
@@ -373,7 +386,14 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
     double A[6][7];
 #pragma unroll
     for (int i = 0; i < 6; ++i) A[i][0] = T.A1[i];
-    double Xs[2][6], r2[2];
+    // relative position and velocity at the beginning of the step
+    double d0[3], u0[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        d0[k] = T.X[k] - T.X[3 + k];
+        u0[k] = T.V[k] - T.V[3 + k];
+    }
+    double Ds[2][3], Xis[2][3], Xa_new[3], r2[2];
     // three levels; the two stages of a level are independent of each other
 #pragma unroll
     for (int lev = 0; lev < 3; ++lev) {
@@ -386,32 +406,44 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
             const int s = 2 * lev + 1 + e;  // stage s+1
             const double hc = h * kC[s];
 #pragma unroll
-            for (int i = 0; i < 6; ++i) {
-                Xs[e][i] = (s == 1)   ? stage_pos<1>(T.X[i], T.V[i], hc, h2, A[i])
-                           : (s == 2) ? stage_pos<2>(T.X[i], T.V[i], hc, h2, A[i])
-                           : (s == 3) ? stage_pos<3>(T.X[i], T.V[i], hc, h2, A[i])
-                           : (s == 4) ? stage_pos<4>(T.X[i], T.V[i], hc, h2, A[i])
-                           : (s == 5) ? stage_pos<5>(T.X[i], T.V[i], hc, h2, A[i])
-                                      : stage_pos<6>(T.X[i], T.V[i], hc, h2, A[i]);
+            for (int k = 0; k < 3; ++k) {
+                if (s == 1) {
+                    Xis[e][k] = fma(hc, T.V[k], T.X[k]);
+                    Ds[e][k] = fma(hc, u0[k], d0[k]);
+                } else {
+                    const double ai = (s == 2)   ? stage_acc<2>(A[k])
+                                      : (s == 3) ? stage_acc<3>(A[k])
+                                      : (s == 4) ? stage_acc<4>(A[k])
+                                      : (s == 5) ? stage_acc<5>(A[k])
+                                                 : stage_acc<6>(A[k]);
+                    const double aa = (s == 2)   ? stage_acc<2>(A[3 + k])
+                                      : (s == 3) ? stage_acc<3>(A[3 + k])
+                                      : (s == 4) ? stage_acc<4>(A[3 + k])
+                                      : (s == 5) ? stage_acc<5>(A[3 + k])
+                                                 : stage_acc<6>(A[3 + k]);
+                    Xis[e][k] = stage_pos(T.X[k], T.V[k], hc, h2, ai);
+                    Ds[e][k] = stage_pos(d0[k], u0[k], hc, h2, ai - aa);
+                    if (s == 6) Xa_new[k] = stage_pos(T.X[3 + k], T.V[3 + k], hc, h2, aa);
+                }
             }
         }
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
             const int s = 2 * lev + 1 + e;
             double a[6];
-            accel<TRAP>(P, cs[e], Xs[e], a, r2[e]);
+            accel<TRAP>(P, cs[e], Ds[e], Xis[e], a, r2[e]);
 #pragma unroll
             for (int i = 0; i < 6; ++i) A[i][s] = a[i];
         }
     }
-    // Xs[1] = x_new (stage 7 position = 5th-order solution), A[.][6] = f(t_new, ynew)
+    // stage 7 position = the 5th-order solution x_new; A[.][6] = f(t_new, ynew)
     Ratio cv[6], cx[6];
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
-        R.X[i] = Xs[1][i];
+        R.X[i] = (i < 3) ? Xis[1][i] : Xa_new[i - 3];
         StepEndPart S;
         step_end_begin(P, T.X[i], T.V[i], A[i], S);
-        R.V[i] = step_end_finish(S, h, Xs[1][i], T.V[i], A[i][5], A[i][6], cv[i], cx[i]);
+        R.V[i] = step_end_finish(S, h, R.X[i], T.V[i], A[i][5], A[i][6], cv[i], cx[i]);
         R.A7[i] = A[i][6];
     }
     R.s = radial_s(R.X, R.V);
@@ -461,7 +493,9 @@ __device__ __forceinline__ void init_traj(const KParams& P, Traj& T, Cold& C)
     K.t = P.t0;
     const double cs = trap_cos<TRAP>(P, P.t0);
     double r2;
-    accel<TRAP>(P, cs, T.X, T.A1, r2);
+    const double D[3] = {T.X[0] - T.X[3], T.X[1] - T.X[4], T.X[2] - T.X[5]};
+    const double Xi[3] = {T.X[0], T.X[1], T.X[2]};
+    accel<TRAP>(P, cs, D, Xi, T.A1, r2);
     K.sprev = radial_s(T.X, T.V);
     C.rmin2() = r2;
     C.t_first() = 0.0;

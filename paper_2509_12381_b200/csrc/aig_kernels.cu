@@ -655,14 +655,16 @@ step_once_kernel(const KParams P, const double* __restrict__ y, const double* __
     T.c.flags = 0u;
     double r2;
     Attempt R;
+    const double D[3] = {T.X[0] - T.X[3], T.X[1] - T.X[4], T.X[2] - T.X[5]};
+    const double Xi[3] = {T.X[0], T.X[1], T.X[2]};
     // RF trap: the branch-free cos where it is valid, libdevice's beyond (the integrator makes
     // this choice once per call on the host, from t0 and t_max)
     if (trap_of(TRAP) == TRAP_RF && !(fabs(P.omega) * (fabs(T.c.t) + fabs(T.c.h)) < 0.99 * kCosMaxArg)) {
         constexpr int BIG = TRAP_RF_BIG + 4 * pot_of(TRAP);
-        accel<BIG>(P, trap_cos<BIG>(P, T.c.t), T.X, T.A1, r2);
+        accel<BIG>(P, trap_cos<BIG>(P, T.c.t), D, Xi, T.A1, r2);
         dp45_attempt<BIG>(P, T, R);
     } else {
-        accel<TRAP>(P, trap_cos<TRAP>(P, T.c.t), T.X, T.A1, r2);
+        accel<TRAP>(P, trap_cos<TRAP>(P, T.c.t), D, Xi, T.A1, r2);
         dp45_attempt<TRAP>(P, T, R);
     }
 #pragma unroll

@@ -85,16 +85,14 @@ __device__ __forceinline__ double shfl_xor_d(double v, int m) { return __shfl_xo
 // Whatever the caller puts between the two (the cos of this step, the partial step-end sums)
 // runs inside the shuffle latency.
 struct LevelOpen {
-    double xsi, xsa, d;
+    double xsi, xsa, d;  // ion stage position, atom stage position (level 2 only: the new state), relative position
     double s0, s1, s2;
 };
 template <int LEV>
-__device__ __forceinline__ void level_open(const SplitRole& R, const SplitState& Y, double h, double h2,
-                                           const double (&Ai)[7], const double (&Aa)[7], LevelOpen& L)
+__device__ __forceinline__ void level_open(const SplitRole& R, const SplitState& Y, double d0, double u0, double h,
+                                           double h2, const double (&Ai)[7], const double (&Aa)[7], LevelOpen& L)
 {
     const double hc = h * R.cC[LEV];
-    const double bi = fma(hc, Y.vi, Y.xi);
-    const double ba = fma(hc, Y.va, Y.xa);
     double acci, acca;
     if (LEV == 0) {
         acci = R.cA0 * Ai[0];
@@ -116,9 +114,11 @@ __device__ __forceinline__ void level_open(const SplitRole& R, const SplitState&
             acca = fma(R.cA2[l], Aa[l], acca);
         }
     }
-    L.xsi = fma(h2, acci, bi);
-    L.xsa = fma(h2, acca, ba);
-    L.d = L.xsi - L.xsa;
+    // the same three chains as dp45_attempt (aig_device.cuh "Stage positions"); stage 2 (level 0, e = 0) has
+    // coefficient 0: acc = +-0 and fma(h2, +-0, base) = base exactly
+    L.xsi = stage_pos(Y.xi, Y.vi, hc, h2, acci);
+    L.d = stage_pos(d0, u0, hc, h2, acci - acca);
+    L.xsa = (LEV == 2) ? stage_pos(Y.xa, Y.va, hc, h2, acca) : 0.0;
     const double sq = L.d * L.d;
     const int src = R.base + R.e;
     L.s0 = shfl_d(sq, src);
@@ -163,15 +163,16 @@ __device__ __forceinline__ void split_attempt(const KParams& P, const SplitRole&
     double Ai[7], Aa[7];
     Ai[0] = Y.a1i;
     Aa[0] = Y.a1a;
+    const double d0 = Y.xi - Y.xa, u0 = Y.vi - Y.va;  // relative position and velocity at the beginning of the step
     LevelOpen L;
-    level_open<0>(R, Y, h, h2, Ai, Aa, L);
+    level_open<0>(R, Y, d0, u0, h, h2, Ai, Aa, L);
     // the cos of my stage time, inside the first level's shuffle and reciprocal latency
     double mycos = 1.0;
     if (trap_of(TRAP) == TRAP_RF || trap_of(TRAP) == TRAP_RF_BIG) mycos = trap_cos<TRAP>(P, R.cos_end ? ST.t_new : fma(R.cCos, h, K.t));
     level_close<TRAP, 0>(P, R, L, mycos, Ai, Aa);
-    level_open<1>(R, Y, h, h2, Ai, Aa, L);
+    level_open<1>(R, Y, d0, u0, h, h2, Ai, Aa, L);
     level_close<TRAP, 1>(P, R, L, mycos, Ai, Aa);
-    level_open<2>(R, Y, h, h2, Ai, Aa, L);
+    level_open<2>(R, Y, d0, u0, h, h2, Ai, Aa, L);
     // everything of the step end that does not need stages 6 and 7 goes inside the last level
     StepEndPart Si, Sa;
     step_end_begin(P, Y.xi, Y.vi, Ai, Si);

@@ -1,10 +1,13 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
 
 Tolerances are BASELINE.json's north_star, written out here:
-  * one attempted step: ynew within 1e-14, relative to the magnitude of the position /
-    velocity 3-vector the component belongs to;
-  * direct (non-complex) trajectories at rtol = 1e-10: accepted step counts within +-2,
-    final states within 1e-6 (same metric) where the step counts agree;
+  * one attempted step: ynew within 1e-14 of the EXACTLY evaluated step (tests/true_step.py, 40 digits),
+    relative to the magnitude of the position / velocity 3-vector the component belongs to, and never
+    farther from it than twice the oracle's own distance; CUDA path and oracle then differ by no more than
+    the sum of the two distances;
+  * direct (non-complex) trajectories: accepted step counts within +-2, final states within 1e-6 (same
+    metric) once both are at the same time (the earlier stop is continued to the later one with the
+    oracle's integrator: the exit stop is a step-end test);
   * ensemble: complex fraction within 3 binomial sigma, two-sample KS p > 0.01 on the
     scattering angle and lifetime; chaotic complex trajectories are not compared pointwise.
 """
@@ -54,17 +57,29 @@ def block_rel(a, b, ref_extra=None):
     return worst
 
 
-def step_tolerance(y):
-    """north_star's 1e-14, plus the conditioning of eq. (4)-(10) in the lab frame: the force
-    ~ r^-9 sees d = x_ion - x_atom, so the 1-ulp differences between the rounded stage positions
-    of two implementations (size eps |x|, both particles) change it by ~2 * 10 eps |x| / r
-    relatively, and a step at the repulsive wall turns the velocity by h A / |v| ~ 1-3
-    (measured: the oracle's own response to a 1-ulp change of the
-    input positions is 1-2x what the CUDA path differs by).  Only states deep in the well
-    (r ~ 7.6 a0 at |x| ~ 1e3 a0) ever need the second term."""
-    r = np.linalg.norm(y[6:9] - y[0:3], axis=0)
-    xmax = np.max(np.abs(np.vstack([y[0:3], y[6:9]])), axis=0)
-    return 1e-14 + 30 * np.finfo(float).eps * xmax / r
+def step_distances(kw, y, t, h, yo, yg):
+    """Per state: distance of the oracle's and of the CUDA path's ynew from the exactly evaluated step
+    (tests/true_step.py), in the block metric above."""
+    import true_step
+    E = np.array([true_step.step_errors(kw, t[i], y[:, i], h[i], (yo[:, i], yg[:, i])) for i in range(y.shape[1])])
+    return E[:, 0], E[:, 1]
+
+
+def check_step(kw, y, t, h, yo, yg, tol=1e-14):
+    """north_star: "single-step results agree to <= 1e-14 relative".  Measured against the exact step:
+    the CUDA path is within 1e-14 of it on EVERY state (the relative position has a chain of its own,
+    DESIGN.md 7.1), the FP64 oracle -- which differences rounded lab-frame positions, as the paper's
+    f(t, y) does -- only away from the repulsive wall (there it is up to ~1.6e-13 off: eps |x| / r seen
+    by a force ~ r^-9).  So: (1) CUDA vs exact <= tol; (2) CUDA never farther from the exact step than
+    twice the oracle; (3) CUDA vs oracle <= the sum of the two distances (which is <= 1e-14 wherever the
+    oracle itself is that close)."""
+    e_orc, e_gpu = step_distances(kw, y, t, h, yo, yg)
+    assert e_gpu.max() <= tol, e_gpu.max()
+    assert np.all(e_gpu <= 2 * e_orc + tol)
+    rel = block_rel(yg, yo, ref_extra=y)
+    assert np.all(rel <= (e_orc + e_gpu) * (1 + 1e-6) + 1e-16), (rel - e_orc - e_gpu).max()
+    assert np.all(rel[e_orc <= tol / 2] <= tol)
+    return e_orc, e_gpu
 
 
 def run_gpu(aig, w, y0, position=False):
@@ -104,17 +119,19 @@ def _mid_flight_states(w, n, seed):
     return np.ascontiguousarray(np.array(ys).T), np.array(ts), np.array(hs)
 
 
-@pytest.mark.parametrize("cfg", [0, 1, 3])
-def test_step_once_parity(aig, cfg):
-    w = inputs.config(cfg)
+@pytest.mark.parametrize("cfg,kw", [(0, {}), (1, {}), (3, {}), (4, {"q_trap": 0.4}), (4, {"q_trap": 0.2, "rtol": 1e-12})])
+def test_step_once_parity(aig, cfg, kw):
+    w = inputs.config(cfg, **kw)
     y, t, h = _mid_flight_states(w, 96, seed=cfg)
     assert y.shape[1] > 300        # several blocks of 128 threads and a ragged tail
     yo, eo = orc.step_once(orc.make_params(**w.params()), y, t, h, w.rtol, w.atol)
     yg, eg = aig.aig_step_once(aig.make_params(**w.params()), _dev(y), _dev(t), _dev(h), w.rtol, w.atol)
     yg, eg = yg.cpu().numpy(), eg.cpu().numpy()
-    rel = block_rel(yg, yo, ref_extra=y)
-    assert np.all(rel <= step_tolerance(y)), (rel / step_tolerance(y)).max()
-    assert np.mean(rel <= 1e-14) > 0.9
+    e_orc, e_gpu = check_step(w.params(), y, t, h, yo, yg)
+    r = np.linalg.norm(y[6:9] - y[0:3], axis=0)
+    assert (r < 10).sum() >= 5        # states at the repulsive wall are part of the sample
+    print(f"cfg {cfg} {kw}: max distance from the exact step: CUDA {e_gpu.max():.2e}, oracle {e_orc.max():.2e}; "
+          f"within 1e-14: CUDA {np.mean(e_gpu <= 1e-14):.3f}, oracle {np.mean(e_orc <= 1e-14):.3f}")
     # the estimate is a cancelling sum (rounding-order sensitive): compare loosely, and only
     # where it is not itself at rounding level
     big = eo > 1e-3 * w.rtol
@@ -147,20 +164,65 @@ def test_step_once_static_trap_and_edge_sizes(aig):
 SHORT_RANGE = 50.0   # a0; hits bottom out at r_min ~ 7.6 a0, misses stay above ~500 a0 (S5)
 
 
-def _shift_to(o, p, t_target):
-    """Oracle final states moved along their own tangent to the stop times of the other run.
-    The exit-radius stop is a step-end test (reading S8): the stop time inherits the step-size
-    noise of the start-up phase, and beyond r_exit the motion is
-    free to ~1e-12, so y(t_o) + (t - t_o) f(t_o, y(t_o)) is the same trajectory at time t."""
-    return o["y_final"] + (t_target - o["t_final"]) * orc.rhs(p, o["t_final"], o["y_final"])
+def _continue_to(kw, rtol, atol, y, t_from, t_to):
+    """States y[12][n] at times t_from[n] continued to t_to[n] >= t_from[n] with the ORACLE's integrator
+    (exit radius disabled, same tolerances): lands exactly on t_to."""
+    out = y.copy()
+    for i in np.flatnonzero(t_to > t_from):
+        p = orc.make_params(**{**kw, "t0": float(t_from[i]), "r_exit": 0.0})
+        r = orc.integrate(p, y[:, i:i + 1], float(t_to[i]), rtol, atol)
+        assert r["status"][0] == 1 and r["t_final"][0] == t_to[i]
+        out[:, i] = r["y_final"][:, 0]
+    return out
 
 
-def _compare_direct(w, y0, g, o, tol=1e-6):
+def _at_common_time(w, ya, ta, yb, tb, kw=None):
+    """The exit-radius stop is a step-end test (reading S8: no event location), so the stop time inherits
+    the step-size noise of the whole run and two runs may stop a step apart.  Final states are compared at
+    the SAME time: whichever run stopped earlier is continued to the other's stop time with the oracle's
+    integrator."""
+    kw = kw or w.params()
+    tc = np.maximum(ta, tb)
+    return _continue_to(kw, w.rtol, w.atol, ya, ta, tc), _continue_to(kw, w.rtol, w.atol, yb, tb, tc)
+
+
+def _final_state_rel(w, a, b, sel, kw=None):
+    """block_rel of the final states of runs a and b on the trajectories sel, at a common time."""
+    idx = np.flatnonzero(sel)
+    ya, yb = _at_common_time(w, a["y_final"][:, idx], a["t_final"][idx], b["y_final"][:, idx], b["t_final"][idx], kw)
+    rel = np.full(len(sel), np.nan)
+    rel[idx] = block_rel(ya, yb)
+    return rel
+
+
+def _dop853_distance(w, y0, run, idx, kw=None):
+    """Distance of run's final states from scipy's DOP853 at rtol = 1e-13 (an 8th-order library integrator
+    with its own controller), each at the run's own stop time."""
+    from scipy import integrate as sci
+    p = orc.make_params(**(kw or w.params()))
+    fun = lambda t, yy: orc.rhs(p, t, np.asarray(yy).reshape(12, 1))[:, 0]
+    out = []
+    for i in idx:
+        ref = sci.solve_ivp(fun, (p.t0, float(run["t_final"][i])), y0[:, i], method="DOP853", rtol=1e-13, atol=1e-24)
+        assert ref.status == 0
+        out.append(block_rel(run["y_final"][:, i:i + 1], ref.y[:, -1][:, None])[0])
+    return np.array(out)
+
+
+def _compare_direct(w, y0, g, o, tol=1e-6, kw=None):
     """north_star: on direct (non-complex) trajectories accepted step counts agree to +-2 and final
-    states to <= 1e-6.  'Direct' = at most one turning point and never inside the short-range well;
-    single-bounce trajectories that do reach it amplify a 1-ulp change of y0 by ~1e12 in the oracle
-    itself, so they are compared against that measured sensitivity."""
-    p = orc.make_params(**w.params())
+    states to <= 1e-6.  'Direct' = at most one turning point, stopped on the exit radius.
+      * far (never inside the short-range well): final states <= 1e-6 at a common time, angle <= 1e-6,
+        stop times within one maximal step of each other; r_min (a step-end sample) <= 1e-6 where both
+        runs sampled at the same times;
+      * single bounces that reach the well (r ~ 7.6 a0): there the method's truncation error is amplified
+        by many orders of magnitude (the oracle at these tolerances is 1e-3 .. 1 away from a DOP853
+        solution at rtol = 1e-13) and so is every rounding: the CUDA path must be (a) as close to the
+        DOP853 solution as the oracle is (never more than twice as far), and (b) no farther from the
+        oracle than twice what the oracle's own answer moves under a 1-ulp change of y0 (median and 90 %
+        quantile of the sample)."""
+    kw = kw or w.params()
+    p = orc.make_params(**kw)
     y1 = y0.copy()
     y1[6:9] = np.nextafter(y1[6:9], np.inf)         # 1-ulp perturbation of the atom position
     o1 = orc.integrate(p, y1, w.t_max, w.rtol, w.atol, threads=8)
@@ -173,18 +235,23 @@ def _compare_direct(w, y0, g, o, tol=1e-6):
     far = direct & (o["r_min"] > SHORT_RANGE) & (g["r_min"] > SHORT_RANGE)
     short = direct & (o["r_min"] <= SHORT_RANGE)
     assert far.sum() > 0.2 * len(far)
-    rel = block_rel(g["y_final"], _shift_to(o, p, g["t_final"]))
+    rel = _final_state_rel(w, g, o, direct, kw)
     assert rel[far].max() <= tol, rel[far].max()
-    assert np.max(np.abs(g["t_final"][far] / o["t_final"][far] - 1)) <= 1e-4
+    # a step is at most hmax = (t_max - t0) / 10 long: the two stops are within one step of each other
+    assert np.max(np.abs(g["t_final"][far] - o["t_final"][far])) <= 0.1 * (w.t_max - p.t0)
     # final velocities are asymptotic: the angle does not depend on the stop time
     assert np.max(np.abs(g["angle"][far] - o["angle"][far])) <= 1e-6
-    assert np.max(np.abs(g["r_min"][far] / o["r_min"][far] - 1)) <= 1e-6
+    same = far & (g["n_acc"] == o["n_acc"]) & (np.abs(g["t_final"] / o["t_final"] - 1) <= 1e-6)
+    assert same.sum() > 0.5 * far.sum()
+    assert np.max(np.abs(g["r_min"][same] / o["r_min"][same] - 1)) <= 1e-6
     assert np.max(np.abs(g["r_min"][short] / o["r_min"][short] - 1), initial=0.0) <= 1e-3
     if short.sum() >= 20:
-        # the CUDA path must be indistinguishable from a rounding-level perturbation of the oracle
-        ref = block_rel(o1["y_final"], _shift_to(o, p, o1["t_final"]))
-        assert np.median(rel[short]) <= 5 * np.median(ref[short]) + 1e-9, (np.median(rel[short]), np.median(ref[short]))
-        assert rel[short].max() <= 30 * ref[short].max() + 1e-9, (rel[short].max(), ref[short].max())
+        ref = _final_state_rel(w, o1, o, short, kw)
+        for qt in (0.5, 0.9):
+            assert np.quantile(rel[short], qt) <= 2 * np.quantile(ref[short], qt) + 1e-9, (qt, np.quantile(rel[short], qt), np.quantile(ref[short], qt))
+        pick = np.flatnonzero(short)[:8]
+        e_g, e_o = _dop853_distance(w, y0, g, pick, kw), _dop853_distance(w, y0, o, pick, kw)
+        assert np.all(e_g <= 2 * e_o + 1e-9), (e_g, e_o)
     return far
 
 
@@ -244,8 +311,7 @@ def test_config1_two_body_physics(aig):
     dn = np.abs(gp["n_acc"][clear].astype(int) - o["n_acc"][clear].astype(int))
     assert dn.max() <= 2
     miss = clear & (b[:n_o] > bc) & (gp["n_acc"] == o["n_acc"])
-    shifted = _shift_to(o, orc.make_params(**w.params()), gp["t_final"])
-    assert block_rel(gp["y_final"][:, miss], shifted[:, miss]).max() <= 1e-6
+    assert _final_state_rel(w, gp, o, miss)[miss].max() <= 1e-6
     # Langevin capture at full size
     clear_all = np.abs(b / bc - 1) > 1e-3
     captured = g["r_min"] < bc / 2
@@ -309,14 +375,32 @@ def test_config3_prefix_heavy_light(aig):
     assert g["n_acc"].max() > 20 * np.median(g["n_acc"])   # the imbalance the refill queue is for
 
 
-@pytest.mark.parametrize("cfg,kw", [(4, {}), (3, {})])
+_Y0_CACHE = {}
+
+
+def _y0_cached(w):
+    """configs[4]'s nine sweep points share one y0 (seed 4, reading S18): generate the 4,194,304 states once."""
+    key = (w.N, w.seed, w.T_atom, w.T_ion, w.b_max, w.R0, w.m_ion, w.m_atom)
+    if key not in _Y0_CACHE:
+        _Y0_CACHE.clear()
+        _Y0_CACHE[key] = inputs.generate_y0(w)
+    return _Y0_CACHE[key]
+
+
+SWEEP = [(4, {"q_trap": q, "rtol": rtol}) for q in (0.1, 0.2, 0.4) for rtol in (1e-8, 1e-10, 1e-12)]
+
+
+@pytest.mark.parametrize("cfg,kw", SWEEP + [(3, {})])
 def test_full_size_sampled_outputs(aig, cfg, kw):
     """BASELINE.json's full sizes in the launch configuration bench.py times (configs[4]: N = 4,194,304,
-    default schedule; configs[3]: N = 1,048,576): outputs of a seeded sample of trajectories are compared
-    with the oracle one by one, the rest through properties that hold at any size."""
+    default schedule, ALL NINE points of its 3 x 3 sweep q x rtol with atol = rtol/100; configs[3]:
+    N = 1,048,576): outputs of a seeded sample of trajectories are compared with the oracle one by one,
+    the rest through properties that hold at any size."""
     import torch
     w = inputs.config(cfg, **kw)
-    y0 = inputs.generate_y0(w)
+    if cfg == 4:
+        assert w.atol == w.rtol * 1e-2 and w.N == 4194304
+    y0 = _y0_cached(w)
     p = aig.make_params(**w.params())
     # configs[4] exactly as bench.py launches it; configs[3] also records the first-bounce position
     bufs = aig.alloc_out(w.N, "cuda", position=True) if cfg == 3 else None
@@ -498,9 +582,7 @@ def test_general_potential(aig, n_att, n_rep, trap):
     y, t, h = np.ascontiguousarray(np.array(ys).T), np.array(ts), np.array(hs)
     yo, eo = orc.step_once(po, y, t, h, w.rtol, w.atol)
     yg, eg = aig.aig_step_once(pg, _dev(y), _dev(t), _dev(h), w.rtol, w.atol)
-    rel = block_rel(yg.cpu().numpy(), yo, ref_extra=y)
-    assert np.all(rel <= 4 * step_tolerance(y)), (rel / step_tolerance(y)).max()   # pow() vs repeated squaring: a few ulp
-    assert np.mean(rel <= 1e-14) > 0.85
+    check_step(kw, y, t, h, yo, yg.cpu().numpy(), tol=2e-14)    # repeated squaring: a few ulp on a force that turns the velocity
     # whole trajectories
     g = _host(aig.aig_integrate(pg, _dev(y0), w.t_max, w.rtol, w.atol))
     o = orc.integrate(po, y0, w.t_max, w.rtol, w.atol, threads=8)
@@ -508,8 +590,7 @@ def test_general_potential(aig, n_att, n_rep, trap):
     direct = (o["n_turn"] <= 1) & (g["n_turn"] <= 1) & (o["status"] == 0) & (g["status"] == 0) & (o["r_min"] > SHORT_RANGE)
     assert direct.sum() > 0.1 * n
     assert np.max(np.abs(g["n_acc"][direct].astype(int) - o["n_acc"][direct].astype(int))) <= 2
-    yo_s = o["y_final"] + (g["t_final"] - o["t_final"]) * orc.rhs(po, o["t_final"], o["y_final"])
-    assert block_rel(g["y_final"], yo_s)[direct].max() <= 1e-6
+    assert _final_state_rel(ws, g, o, direct, kw)[direct].max() <= 1e-6
     assert np.max(np.abs(g["angle"][direct] - o["angle"][direct])) <= 1e-6
     assert abs(g["complex_flag"].mean() - o["complex_flag"].mean()) <= 3 * math.sqrt(0.25 / n) + 1e-9
     # the six-lane kernel computes the same bits
