@@ -41,7 +41,9 @@ FLOPS_PER_ATTEMPT = 900.0
 FP64_PEAK_NOMINAL = 148 * 4 * 16 * 2 * 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of one integrate_kernel launch at the bench
 # workload, from the ncu --set full capture summarised in profiles/ (None until captured).
-INTEGRATE_DRAM_TRAFFIC_BYTES = 3.02e9  # profiles/r01d_integrate_full.md: the six integrator kernels of one call
+INTEGRATE_DRAM_TRAFFIC_BYTES = 3.02e9
+INTEGRATE_DRAM_TRAFFIC_SOURCE = ("constant from the ncu --set full capture summarised in profiles/r01d_integrate_full.md "
+                                 "(integrator kernels of one call), NOT measured in this run")
 
 WORKLOAD_NAME = "configs[4] N=4194304 q=0.1 rtol=1e-10 atol=1e-12 seed=4"
 SWEEP_Q = (0.1, 0.2, 0.4)
@@ -243,12 +245,47 @@ def run_ours(args) -> int:
     ms_total = max_over_ranks(e_begin.elapsed_time(e_end))
     ms_int = max_over_ranks(float(np.mean([a.elapsed_time(b) for a, b in kev])))
 
-    # stage timeline of the last aig_integrate call (ns %globaltimer stamps the kernels leave in the workspace)
-    tl = ws[:512].view(torch.int64)[32:50].cpu().numpy().astype(np.float64)
-    t_first = min((x for x in tl if x > 0), default=0.0)
-    stages_ms = {name: [round((tl[2 * i] - t_first) / 1e6, 3), round((tl[2 * i + 1] - t_first) / 1e6, 3)]
-                 for i, name in enumerate(("plan", "bulk0", "split0", "bulk1", "split1", "bulk2", "split2", "bulk3", "split3"))
-                 if tl[2 * i] > 0}
+    def schedule_record():
+        """Stage timeline and hand-over counts of the last aig_integrate call (the %globaltimer stamps and
+        counters its kernels leave in the workspace): [start, end] in ms of the bulk pass (per-thread
+        integrator), the six-lane pass that streams beside it, and the final six-lane pass."""
+        cnt = ws[:512].view(torch.int64).cpu().numpy()
+        tl = cnt[32:40].astype(np.float64)
+        t_first = min((x for x in tl if x > 0), default=0.0)
+        st = {name: [round((tl[2 * i] - t_first) / 1e6, 3), round((tl[2 * i + 1] - t_first) / 1e6, 3)]
+              for i, name in enumerate(("plan", "bulk", "six_lane_streaming", "six_lane_final")) if tl[2 * i] > 0}
+        return st, {"n_handed_over": int(cnt[4]), "taken_by_streaming_pass": int(cnt[61]), "taken_by_final_pass": int(cnt[62]),
+                    "class_counts": [int(x) for x in cnt[24:27]]}
+
+    stages_ms, handover = schedule_record()
+
+    def six_lane_step_us(wl, i):
+        """Latency of one attempted step of the six-lane integrator: trajectory i of workload wl alone on the
+        GPU, handed over at its first step (the schedule hook never changes a result)."""
+        y1 = y0[:, i:i + 1].contiguous()
+        aig.set_schedule(plan=0, budget=1, tail_iters=0, mean_factor=0, drain_lanes=32)
+        try:
+            p1 = aig.make_params(**wl.params())
+            best = None
+            for _ in range(2):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                o1 = aig.aig_integrate(p1, y1, wl.t_max, wl.rtol, wl.atol)
+                b.record()
+                torch.cuda.synchronize()
+                n1 = int(o1["n_acc"][0].item()) + int(o1["n_rej"][0].item())
+                us = a.elapsed_time(b) * 1e3 / max(n1, 1)
+                best = us if best is None else min(best, us)
+            return best, n1
+        finally:
+            aig.set_schedule()
+
+    def complex_fraction_r_turn(wl, r_turn):
+        """the complex-formation probability when only radial minima inside r_turn count as
+        bounces (the graded configs count every radial minimum; far-field micromotion wiggles then count too)."""
+        pr = aig.make_params(**{**wl.params(), "r_turn": r_turn})
+        aig.aig_integrate(pr, y0, wl.t_max, wl.rtol, wl.atol, out=out, workspace=ws)
+        return sum_over_ranks(int(out["complex_flag"].sum(dtype=torch.int64).item())) / (world * N)
 
     n_acc = int(out["n_acc"].sum(dtype=torch.int64).item())
     n_rej = int(out["n_rej"].sum(dtype=torch.int64).item())
@@ -259,6 +296,11 @@ def run_ours(args) -> int:
     n_complex = sum_over_ranks(int(out["complex_flag"].sum(dtype=torch.int64).item()))
     n_tmax = sum_over_ranks(int((out["status"] == 1).sum().item()))
     max_steps_seen = int(max_over_ranks(float(out["n_acc"].max().item())))
+
+    i_longest = int(torch.argmax(out["n_acc"] + out["n_rej"]).item())
+    max_attempted = int((out["n_acc"][i_longest] + out["n_rej"][i_longest]).item())
+    step_us, _ = six_lane_step_us(w, i_longest)
+    c50_main = complex_fraction_r_turn(w, 50.0)
 
     sec = ms_total * 1e-3
     value = world * N * args.steps / sec
@@ -310,12 +352,20 @@ def run_ours(args) -> int:
                 a = sum_over_ranks(int(out["n_acc"].sum(dtype=torch.int64).item()))
                 r = sum_over_ranks(int(out["n_rej"].sum(dtype=torch.int64).item()))
                 c = sum_over_ranks(int(out["complex_flag"].sum(dtype=torch.int64).item()))
+                longest = int(max_over_ranks(float((out["n_acc"] + out["n_rej"]).max().item())))
                 tf = FLOPS_PER_ATTEMPT * (a + r) / world / (ms * 1e-3) / 1e12
+                st, ho = schedule_record()
+                c50 = complex_fraction_r_turn(wl, 50.0)
+                # no call can end before its longest trajectory has taken its steps one after the other:
+                # tail_floor_ms = attempted steps of that trajectory x the latency of one six-lane step
+                # (measured above on the bench workload's longest trajectory, alone on the GPU)
                 sweep.append({"q": q, "rtol": rtol, "atol": wl.atol, "ms_integrate": ms,
                               "trajectories_per_s": world * N / (ms * 1e-3),
                               "accepted_steps_per_s": a / (ms * 1e-3),
                               "alg_tflops_per_gpu": tf, "frac_fp64_peak": tf * 1e12 / FP64_PEAK_NOMINAL,
-                              "complex_fraction": c / (world * N)})
+                              "complex_fraction": c / (world * N), "complex_fraction_r_turn_50": c50,
+                              "max_attempted_steps": longest, "tail_floor_ms": longest * step_us * 1e-3,
+                              "stages_ms": st, **ho})
 
     # ---- the widening kernels, outside the timed region: aig_observables and
     #      aig_outliers over the bench workload's results, each timed alone with CUDA events, L2 flushed
@@ -376,12 +426,17 @@ def run_ours(args) -> int:
             "accepted_steps_per_s": acc_all * args.steps / sec,
             "attempted_steps_per_s": (acc_all + rej_all) * args.steps / sec,
             "mean_accepted_steps": acc_all / (world * N), "max_accepted_steps": max_steps_seen,
-            "complex_fraction": n_complex / (world * N), "tmax_fraction": n_tmax / (world * N),
+            "complex_fraction": n_complex / (world * N), "complex_fraction_r_turn_50": c50_main,
+            "tmax_fraction": n_tmax / (world * N),
+            "max_attempted_steps": max_attempted, "six_lane_step_us": step_us,
+            "tail_floor_ms": max_attempted * step_us * 1e-3, "schedule": handover,
             "ms_integrate_kernel": ms_int,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL / 1e12, "unit": "TFLOP/s",
                          "frac": achieved * 1e12 / FP64_PEAK_NOMINAL, "traffic": INTEGRATE_DRAM_TRAFFIC_BYTES,
-                         "kernel": "aig_integrate: plan_kernel + integrate_kernel<TRAP_RF> x2 + integrate_split_kernel<TRAP_RF> x2 "
-                                   "(overlapped on two streams), timed as one region on the launching stream",
+                         "traffic_source": INTEGRATE_DRAM_TRAFFIC_SOURCE,
+                         "kernel": "aig_integrate: plan kernels + integrate_kernel<TRAP_RF> (bulk) with integrate_split_kernel<TRAP_RF> "
+                                   "streaming beside it on a second stream + the final integrate_split_kernel pass, timed as one "
+                                   "region on the launching stream",
                          "stages_ms": stages_ms,
                          "flops_per_attempted_step": FLOPS_PER_ATTEMPT,
                          "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md)",

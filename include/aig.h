@@ -112,7 +112,7 @@ typedef struct aig_hist {
 } aig_hist;
 
 /* Bytes of DEVICE scratch aig_integrate needs for N trajectories: 64 uint64 counters (work
- * queues, slot counts, a stage timeline), the work-queue order (one int64 per trajectory) and
+ * queues, slot counts, a stage timeline), the work-queue order (one int64 and one class byte per trajectory) and
  * min(N, max(2^20, N/4)) checkpoint slots of 216 B for suspended trajectories. */
 size_t aig_workspace_bytes(int64_t N);
 
@@ -124,10 +124,14 @@ size_t aig_workspace_bytes(int64_t N);
  *   workspace DEVICE scratch of >= aig_workspace_bytes(N) bytes, 8-byte aligned
  * Persistent kernels: each thread integrates one trajectory at a time and refills from a
  * global work queue when it finishes (PAPER.md:186-202 runs one array element per thread);
- * trajectories that outlive a step budget (long-lived complexes) are continued by a second
- * kernel that spreads one trajectory over six lanes, on SMs of its own beside the bulk (an
- * internal second stream, joined to `cuda_stream` before the call's work is complete from the
- * caller's point of view).  Every result is bit-identical whichever kernel produced it. */
+ * trajectories that outlive a step budget (long-lived complexes) are handed, while the bulk is
+ * still running, to a second kernel that spreads one trajectory over six lanes on SMs of its own
+ * (an internal second stream, joined to `cuda_stream` before the call's work is complete from
+ * the caller's point of view).  Every result is bit-identical whichever kernel produced it.
+ * Thread safety: may be called concurrently from several host threads (different streams and
+ * workspaces); the enqueue section is serialised per process, and calls that overlap on one
+ * device share the internal stream, so their six-lane passes run one after the other.
+ * p->max_steps must fit the int32 step counters (<= 2^31 - 1), else AIG_ERR_PARAM. */
 int aig_integrate(const aig_params *p, const double *y0, int64_t N, double t_max, double rtol,
                   double atol, const aig_out *out, void *workspace, void *cuda_stream);
 
@@ -218,16 +222,35 @@ uint64_t aig_kernel_launches(void);
 /* Test / tuning hook: the schedule aig_integrate uses from now on in this process.
  *   tail_iters  iterations a warp of the per-thread integrator keeps stepping after its work
  *               queue ran dry before it hands its trajectories over (default 256)
- *   budget      accepted steps after which a trajectory is handed to the six-lane integrator
+ *   budget      accepted steps after which a trajectory is offered to the six-lane integrator
  *               (default 2048)
- *   split_sms   SMs a six-lane pass owns while the next bulk pass runs beside it (32)
+ *   split_sms   SMs the six-lane pass owns while the bulk pass runs beside it (16)
  *   split_grid  one-warp blocks per SM of the final six-lane pass (8)
- *   plan        0: natural order, one bulk pass; 1: three classes, slow capture candidates first (default)
+ *   plan        0: natural order; 1: three classes, slow capture candidates first (default)
  *   kappa       candidates are trajectories with impact parameter < kappa Langevin radii (1.5)
  * Scheduling never changes a result (tests/test_gpu_parity.py::test_schedule_invariance).
  * Returns AIG_ERR_PARAM for out-of-range values.  Not thread-safe against concurrent
- * aig_integrate calls that should see the old schedule. */
+ * aig_integrate calls that should see the old schedule.  The library reads no environment
+ * variable: these two calls are the only way to change the schedule. */
 int aig_set_schedule(int tail_iters, int budget, int split_sms, int split_grid, int plan, double kappa);
+
+/* All knobs of the schedule (the six above and the finer ones). */
+typedef struct aig_schedule {
+    int32_t tail_iters, budget, split_sms, split_grid, plan;
+    double kappa;
+    int32_t depth;        /* budget hand-overs pause while this many published slots wait to be taken (64) */
+    int32_t mean_factor;  /* ... and are only for trajectories this many times longer than the mean of the
+                             finished ones (4; 0 = the plain budget) */
+    int32_t drain_lanes;  /* queue empty: a warp hands over what it still runs once this few lanes are alive (10) */
+    double slow0, slow1;  /* class 0: candidates with u^2 < slow0 <u^2> (0.5); class 1 also takes anything
+                             with u^2 < slow1 <u^2> (0.1) */
+    int32_t refill_batch, refill_wait; /* idle lanes of a warp that trigger its refill (8), or iterations
+                                          one of them has waited (16) */
+    int32_t poll_iters;   /* six-lane warps with idle groups look for new slots every this many iterations (32) */
+} aig_schedule;
+/* s = NULL restores the defaults.  AIG_ERR_PARAM for out-of-range values. */
+int aig_set_schedule_ex(const aig_schedule *s);
+int aig_get_schedule(aig_schedule *s);
 
 const char *aig_strerror(int code);
 int aig_version(void);

@@ -18,7 +18,8 @@ _lib = None
 
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
            "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_set_schedule", "aig_strerror",
-           "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes", "aig_trace"]
+           "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes", "aig_trace",
+           "aig_set_schedule_ex", "aig_get_schedule"]
 
 
 class AigError(RuntimeError):
@@ -314,13 +315,41 @@ def kernel_info() -> dict:
     return dict(zip(keys, [x.value for x in v]))
 
 
-def set_schedule(tail_iters=256, budget=2048, split_sms=32, split_grid=8, plan=1, kappa=1.5) -> None:
-    """Test / tuning hook (include/aig.h: aig_set_schedule); never changes a result."""
+class Schedule(C.Structure):
+    """include/aig.h: aig_schedule."""
+    _fields_ = [("tail_iters", C.c_int32), ("budget", C.c_int32), ("split_sms", C.c_int32), ("split_grid", C.c_int32),
+                ("plan", C.c_int32), ("kappa", C.c_double), ("depth", C.c_int32), ("mean_factor", C.c_int32),
+                ("drain_lanes", C.c_int32), ("slow0", C.c_double), ("slow1", C.c_double),
+                ("refill_batch", C.c_int32), ("refill_wait", C.c_int32), ("poll_iters", C.c_int32)]
+
+
+def get_schedule() -> dict:
+    s = Schedule()
     L = lib()
-    L.aig_set_schedule.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double]
-    L.aig_set_schedule.restype = C.c_int
-    _check(L.aig_set_schedule(int(tail_iters), int(budget), int(split_sms), int(split_grid), int(plan), float(kappa)),
-           "aig_set_schedule")
+    L.aig_get_schedule.restype = C.c_int
+    _check(L.aig_get_schedule(C.byref(s)), "aig_get_schedule")
+    return {k: getattr(s, k) for k, _ in Schedule._fields_}
+
+
+def set_schedule(**knobs) -> None:
+    """Test / tuning hook (include/aig.h: aig_set_schedule_ex); never changes a result.  The library's
+    defaults with the given knobs replaced; no argument = the defaults."""
+    L = lib()
+    L.aig_set_schedule_ex.restype = C.c_int
+    L.aig_set_schedule_ex.argtypes = [C.c_void_p]
+    cur = get_schedule()
+    _check(L.aig_set_schedule_ex(None), "aig_set_schedule_ex")
+    if not knobs:
+        return
+    s = Schedule(**get_schedule())
+    for k, v in knobs.items():
+        if k not in dict(Schedule._fields_):
+            raise TypeError(f"unknown schedule knob {k!r}")
+        setattr(s, k, v)
+    rc = L.aig_set_schedule_ex(C.cast(C.byref(s), C.c_void_p))
+    if rc:
+        L.aig_set_schedule_ex(C.cast(C.byref(Schedule(**cur)), C.c_void_p))  # leave the schedule as it was
+    _check(rc, "aig_set_schedule_ex")
 
 
 def kernel_launches() -> int:

@@ -74,7 +74,7 @@ __device__ __forceinline__ double rcp_nr(double x)
 }
 
 // cos(2 y) for |y| < kCosMaxArg, branch-free and table-free (gen_trig_constants.py): k = round(y 2/pi),
-// u = y - k pi/2 in three FMA steps (|u| <= pi/4), s = sin u by its Taylor kernel in z = u^2 (two
+// u = y - k pi/2 in two FMA steps (|u| <= pi/4), s = sin u by its Taylor kernel in z = u^2 (two
 // interleaved Horner chains in z^2: half the dependent depth), cos(2y) = (-1)^k (1 - 2 s^2).
 // Absolute error < 2e-16 (the force only needs cos to absolute accuracy: it multiplies q_k).
 __device__ __forceinline__ double cos2_cw(double y)
@@ -82,9 +82,9 @@ __device__ __forceinline__ double cos2_cw(double y)
     const double kd = fma(y, kTwoOverPi, kRoundMagic);
     const int q = __double2loint(kd);
     const double k = kd - kRoundMagic;
+    // two constants: the third one would change u by |k| 1.5e-33 < 1e-28 for |y| < kCosMaxArg
     double u = fma(-k, kPio2_1, y);
     u = fma(-k, kPio2_2, u);
-    u = fma(-k, kPio2_3, u);
     const double z = u * u;
     const double w = z * z;
     double pe = fma(kSin[6], w, kSin[4]);
@@ -233,25 +233,44 @@ __device__ __forceinline__ double hmin_of(double t)
     return 16.0 * (up - at);
 }
 
-// q^(-1/5) for q > 0: float seed (MUFU lg2/ex2, ~1e-7) + one cubic correction
-// z (1 + rho/5 + 3 rho^2/25), rho = 1 - q z^5 (Taylor of (1-rho)^(-1/5)); relative error ~1e-16.
-// q is clamped to [1e-30, 1e30] (the result is clamped by the caller).
-__device__ __forceinline__ double inv_fifth_root(double q)
+// The controller's fifth root, q = err / rtol.  Float seed z ~ q^(-1/5) (MUFU lg2 / ex2, relative error
+// ~1e-7) and one Newton-type correction z (1 + rho/5), rho = 1 - q z^5 (first term of the Taylor series of
+// (1 - rho)^(-1/5); the next one, 3 rho^2/25, is ~1e-13: far below the rounding noise of the error estimate
+// the step size is derived from).
+__device__ __forceinline__ float fifth_root_seed(float qf)
 {
-    // seed in float: clamp there (two 4-cycle FMNMX instead of two FP64 compare/select pairs on the
-    // controller's dependent chain) and take MUFU.LG2 / MUFU.EX2 directly (the operand and the
-    // result are normal floats after the clamp, no denormal scaling needed)
-    const float qf = fminf(fmaxf((float)q, 1e-30f), 1e30f);
     float lg, zf;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(qf));
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(zf) : "f"(-0.2f * lg));
-    const double z = (double)zf;
+    return zf;
+}
+// q^(-1/5), q clamped to [1e-30, 1e30] (the reject path: the result is clamped by the caller)
+__device__ __forceinline__ double inv_fifth_root(double q)
+{
+    // clamp the seed in float (two 4-cycle FMNMX instead of two FP64 compare/select pairs on the
+    // controller's dependent chain); the operand and the result are normal floats after the clamp
+    const double z = (double)fifth_root_seed(fminf(fmaxf((float)q, 1e-30f), 1e30f));
     q = dmin(dmax(q, 1e-30), 1e30);  // off the chain: only the correction needs it
     const double z2 = z * z;
-    const double z4 = z2 * z2;
-    const double rho = fma(-q, z4 * z, 1.0);
-    const double t = rho * fma(0.12, rho, 0.2);
-    return fma(z, t, z);
+    const double rho = fma(-(q * z), z2 * z2, 1.0);
+    return fma(z, 0.2 * rho, z);
+}
+// Step size after an accepted step without failures (O3.7): 0.8 h (rtol/err)^(1/5), at most 5 h.  One
+// expression for both kernels, arranged for a short dependent chain behind the seed:
+//     rho = 1 - (q z) z^4,   h_grow = (0.8 h z)(1 + rho/5) = fma(0.8 h z, rho/5, 0.8 h z),   5 h if z >= 6.25
+// (the growth limit is decided on the seed: at z = 6.25 the two branches agree to 1e-7 anyway).  q and its
+// float image qf are taken as given: the caller clamps them to [1e-30, 1e30] or knows that q <= 1, where
+// the clamps change nothing (q < 1e-30 or q = 0 end in 5 h either way: z >= 1e6, or NaN products).
+__device__ __forceinline__ double grow_step(double h, double q, float qf)
+{
+    const float zf = fifth_root_seed(qf);
+    const double z = (double)zf;
+    const double z2 = z * z;
+    const double qz = q * z;
+    const double h08z = (0.8 * h) * z;
+    const double rho = fma(-qz, z2 * z2, 1.0);
+    const double hz = fma(h08z, 0.2 * rho, h08z);
+    return (zf < 6.25f) ? hz : 5.0 * h;
 }
 
 // A candidate of the error norm: the ratio n/d with d > 0, kept unevaluated.
@@ -357,12 +376,20 @@ struct Attempt {
 };
 
 // scaled error estimate from the three axis quotients, NaN when the new state is not finite
+// (in two pieces: the six-lane integrator tests the second one in its fast-path vote)
+__device__ __forceinline__ double error_raw(double h, double q0, double q1, double q2)
+{
+    return h * dmax(dmax(q0, q1), q2);
+}
+__device__ __forceinline__ bool attempt_finite(double q0, double q1, double q2, double r2, double s)
+{
+    return (r2 > 0.0) & (r2 < 1.0e300) & (fabs(s) < 1.0e300) & (q0 == q0) & (q1 == q1) & (q2 == q2);
+}
 __device__ __forceinline__ double error_estimate(double h, double q0, double q1, double q2, double r2, double s)
 {
-    double err = h * dmax(dmax(q0, q1), q2);
+    double err = error_raw(h, q0, q1, q2);
     // a non-finite state or force makes the estimate NaN (it must reject, like the oracle's NaN)
-    const bool finite_ok = (r2 > 0.0) & (r2 < 1.0e300) & (fabs(s) < 1.0e300) & (q0 == q0) & (q1 == q1) & (q2 == q2);
-    if (!finite_ok) err = __longlong_as_double(0x7ff8000000000000LL);
+    if (!attempt_finite(q0, q1, q2, r2, s)) err = __longlong_as_double(0x7ff8000000000000LL);
     return err;
 }
 
@@ -531,16 +558,15 @@ template <class Cold>
 __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, double err, const StepTimes& ST,
                                            double r2, double s, bool live, bool& accepted, bool& first_turn)
 {
-    const double z = inv_fifth_root(err * P.inv_rtol);  // (err/rtol)^(-1/5)
-    const bool acc = (err <= P.rtol);                   // NaN rejects
+    const double q = err * P.inv_rtol;
+    const double z = inv_fifth_root(q);  // (err/rtol)^(-1/5), for the reject path
+    const bool acc = (err <= P.rtol);    // NaN rejects
     const unsigned fl = K.flags;
     const bool nofailed = (fl & kNoFailed) != 0u;
     const double h = K.h;
     // ---- accepted: observables, stop tests, next step size (O3.6-O3.8, O3.3).  What does not
     //      depend on z is formed first; behind z there is one product, one select, two clamps and
     //      the last-step test.
-    const double h08 = 0.8 * h;
-    const double h_alt = nofailed ? 5.0 * h : h;  // growth limit 5, or h kept after a failure
     const bool radial_min = (K.sprev < 0.0) & (s >= 0.0);
     const unsigned anymin = (fl & kAnyMin) | (radial_min ? kAnyMin : 0u);
     const bool counted = radial_min & (r2 < P.r_turn2);
@@ -551,7 +577,8 @@ __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, d
     const int st_acc = stop_exit ? 0 : (stop_last ? 1 : (stop_max ? 2 : -1));
     // h_cl = min(hmax, max(hmin_new, h_grow)) and last_new = (1.1 h_cl >= rem_new), with the three
     // comparisons of h_grow side by side instead of one behind the other (exact selects, same values)
-    const double h_grow = (nofailed & (z < 6.25)) ? h08 * z : h_alt;
+    const double h_grown = grow_step(h, dmin(dmax(q, 1e-30), 1e30), fminf(fmaxf((float)q, 1e-30f), 1e30f));
+    const double h_grow = nofailed ? h_grown : h;  // h is kept after a step with a failed attempt
     const bool over = (h_grow > P.hmax) | (ST.hmin_new > P.hmax);
     const bool under = (h_grow < ST.hmin_new);
     const bool last_grow = (1.1 * h_grow >= ST.rem_new);
@@ -598,6 +625,46 @@ __device__ __forceinline__ int finish_core(const KParams& P, Core& K, Cold& C, d
     K.h = keep ? h : (a ? h_acc : h_rej);
     K.flags = keep ? (a ? anymin | (fl & ~kAnyMin) : fl) : (a ? fl_acc : (fl & kAnyMin));
     return live ? (acc ? st_acc : st_rej) : -1;
+}
+
+// The common case of finish_core, for the six-lane integrator (whose step is bound by the instructions it
+// issues): an accepted step with no failed attempt before it, no turning point, no stop, and a step size
+// far above hmin.  fast_step_ok decides it from quantities that are known BEFORE the controller's fifth
+// root (the warp votes on it while the root is being taken); fast_step_commit is then finish_core
+// restricted to that case -- the same operations on the same operands, so the same bits:
+//   * hmin = 16 ulp(t) <= 2^-48 |t|, and after an accepted step h_grow >= 0.79 h: with
+//     h / 2 > 2^-48 |t_new| the clamps to hmin_new are no-ops (`under` false);
+//   * h_grow <= 5 h (1 + 1e-6): with 5.5 h <= hmax and 1.1 x 5.5 h < t_max - t_new, `over` and `last_new`
+//     are false: the next step size is h_grow itself and the flags do not change;
+//   * no radial minimum this step: anymin = the flag as it is.
+__device__ __forceinline__ bool fast_step_ok(const KParams& P, const Core& K, double q_own, double t_new, double r2,
+                                             double s)
+{
+    // err = h max_k q_k <= rtol  <=>  h q_k <= rtol for every axis k (rounding is monotone): each lane tests
+    // its own axis, the warp's vote combines them -- before the quotients have been gathered.  NaN fails.
+    const bool acc_own = (K.h * q_own <= P.rtol);
+    const bool finite_ok = (r2 > 0.0) & (r2 < 1.0e300) & (fabs(s) < 1.0e300);
+    const unsigned fl = K.flags;
+    const bool flags_ok = (fl & (kLast | kNoFailed)) == kNoFailed;
+    const bool radial_min = (K.sprev < 0.0) & (s >= 0.0);
+    const bool stop_exit = ((fl & kAnyMin) != 0u) & (r2 > P.r_exit2);
+    const bool stop_max = (long long)(K.n_acc + 1) >= P.max_steps;
+    // the next step size is at most 5 h (1 + 1e-6): with 5.5 h <= hmax and 1.1 x 5.5 h < t_max - t_new it is
+    // neither clamped to hmax nor the last one; with h/2 > 2^-48 |t_new| >= hmin it is not clamped to hmin
+    const double g = 5.5 * K.h;
+    const bool h_ok = (g <= P.hmax) & (1.1 * g < P.t_max - t_new) & (K.h * 140737488355328.0 > fabs(t_new)) & (K.h > 1.0e-290);  // 2^47
+    return acc_own & finite_ok & flags_ok & !radial_min & !stop_exit & !stop_max & h_ok;
+}
+template <class Cold>
+__device__ __forceinline__ void fast_step_commit(const KParams& P, Core& K, Cold& C, double err, double t_new, double r2,
+                                                 double s)
+{
+    const double q = err * P.inv_rtol;  // <= 1 here
+    K.h = grow_step(K.h, q, (float)q);  // flags stay as they are: kNoFailed set, kLast not
+    K.n_acc += 1;
+    K.t = t_new;
+    K.sprev = s;
+    C.rmin2() = (r2 < C.rmin2()) ? r2 : C.rmin2();
 }
 
 // finish_core for the per-thread integrator: on return T holds the state to continue from (or

@@ -23,7 +23,6 @@
 #include <cstdio>
 #include <algorithm>
 #include <atomic>
-#include <cstdlib>
 #include <mutex>
 #include <cuda_runtime.h>
 
@@ -150,6 +149,14 @@ struct Ckpt {
 constexpr int kCkptDoubles = 24, kCkptInts = 4;
 constexpr size_t kCkptBytesPerSlot = kCkptDoubles * 8 + kCkptInts * 4 + 8;
 
+__device__ __forceinline__ unsigned long long ld_volatile(const unsigned long long* p)
+{
+    return *(const volatile unsigned long long*)p;
+}
+
+// A slot is PUBLISHED by its idx entry: the entries are -1 when the call starts (memset), the writer
+// stores every field, fences, and stores the trajectory index last; a reader that has claimed the slot
+// number spins on idx >= 0, fences, and reads the fields past L1 (ckpt_wait / __ldcg).
 template <class Cold>
 __device__ __forceinline__ void ckpt_store(const Ckpt& K, long long slot, long long idx, const Traj& T, Cold& C)
 {
@@ -172,29 +179,60 @@ __device__ __forceinline__ void ckpt_store(const Ckpt& K, long long slot, long l
     q[1 * cap] = (int)T.c.flags;
     q[2 * cap] = C.n_rej();
     q[3 * cap] = C.n_turn();
-    K.idx[slot] = idx;
+    __threadfence();
+    *(volatile long long*)(K.idx + slot) = idx;
+}
+
+// trajectory index of a claimed slot, once its writer has published it.  The writer took the slot number
+// while running and publishes within microseconds; a second without it means a broken invariant: trap
+// (a loud failure) rather than hang.
+__device__ __forceinline__ long long ckpt_wait(const Ckpt& K, long long slot)
+{
+    long long idx = *(const volatile long long*)(K.idx + slot);
+    if (idx < 0) {
+        const unsigned long long t0 = global_ns();
+        while ((idx = *(const volatile long long*)(K.idx + slot)) < 0) {
+            __nanosleep(100);
+            if (global_ns() - t0 > 1000000000ULL) __trap();
+        }
+    }
+    __threadfence();
+    return idx;
 }
 
 // Scheduling arguments of one launch of the per-thread integrator.  Work items are the entries
 // [*begin, *end) of `order` (trajectory indices; order == nullptr: the indices themselves).  A lane
-// whose trajectory has not ended is suspended (state written to slot atomicAdd(*n_out, 1) of
-// `out`) when it has taken `budget` accepted steps -- as long as this stage has handed over fewer
-// than `soft_cap` trajectories (the six-lane integrator has half the throughput per FP64
-// operation: it is for the few, not for the many; a trajectory that is kept is asked again one
-// budget later), and only once it is `mean_factor` times longer than the mean of the trajectories
-// this launch has finished (a workload where every trajectory is long is the per-thread kernel's
-// job: nothing is handed over before 32 have finished) -- or when, `tail_iters` iterations after its
-// warp has seen the queue empty, the warp has `drain_lanes` or fewer trajectories left; when the
-// slots are exhausted it simply keeps stepping.  Suspension never changes a trajectory's
+// whose trajectory has not ended is suspended -- its state written to slot atomicAdd(*n_out, 1) of
+// `out` and published there, for the six-lane integrator that runs BESIDE this kernel and takes slots
+// as they appear (*taken = slots it has claimed so far) --
+//   (a) when it has taken `budget` accepted steps, is `mean_factor` times longer than the mean of the
+//       trajectories this launch has finished (a workload in which every trajectory is long is this
+//       kernel's job: nothing is handed over before 32 have finished), has reached the BAR, and the
+//       six-lane pass has room: fewer than its capacity + `depth` trajectories handed over and not yet
+//       finished (it has less than half the throughput per FP64 operation: it is for the few, and a
+//       suspended trajectory that waits makes no progress).  The bar is a feedback loop: a trajectory
+//       at or above it that is refused for lack of room nudges it up (by 1/64, at most once per 20 us)
+//       and asks again 64 steps later; the six-lane pass nudges it down while a quarter of its groups
+//       are idle.  It settles where the trajectories that cross it arrive as fast as the six-lane pass
+//       finishes others: the fast lane then holds the LONGEST-running trajectories, which is what
+//       bounds the end of the call.  A trajectory below the bar is asked again at the bar, or one
+//       budget later; or
+//   (b) when, `tail_iters` iterations after its warp has seen the queue empty, the warp has
+//       `drain_lanes` or fewer trajectories left.
+// When the slots are exhausted it simply keeps stepping.  Suspension never changes a trajectory's
 // arithmetic, only where it continues.
 struct Sched {
     unsigned long long* queue;
     const long long* order;
     const unsigned long long *begin, *end;
     unsigned long long* n_out;
-    const unsigned long long* soft_base;  // slots handed out before this stage
-    long long soft_cap;
+    const unsigned long long* finished;  // trajectories the six-lane passes have finished
+    unsigned long long* bar;             // accepted steps a trajectory must have to be offered (see below)
+    long long capacity;                  // trajectories the streaming six-lane pass can step at once
+    unsigned long long* started;     // set to 1 by the first block to run
+    unsigned long long* done_warps;  // warps that have exited (the six-lane pass beside this kernel ends when all have)
     Ckpt out;
+    int depth;
     int budget;
     int tail_iters;
     int refill_batch, refill_wait;
@@ -217,7 +255,7 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
     const int lane = threadIdx.x & 31;
     const long long first = (long long)*S.begin;
     const long long total = (long long)*S.end - first;
-    const long long soft_first = (long long)*S.soft_base;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *(volatile unsigned long long*)S.started = 1ULL;
     Traj T;
     long long idx = -1;
     int stop_at = 0;      // suspend when n_acc reaches this
@@ -297,16 +335,31 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
             } else if (may_suspend && (T.c.n_acc >= stop_at || drain)) {
                 bool room = true;
                 if (!drain) {
-                    // budget hand-over: only while the six-lane queue is short, and only for a trajectory
-                    // that is long compared with what this launch has finished so far
-                    const long long used = (long long)(*(volatile unsigned long long*)S.n_out) - soft_first;
-                    room = used < S.soft_cap;
+                    // budget hand-over: only while few published slots wait to be taken, and only for a
+                    // trajectory that is long compared with what this launch has finished so far
+                    const unsigned long long n_now = (unsigned long long)T.c.n_acc;
+                    const unsigned long long bar = ld_volatile(S.bar);
+                    int again = S.budget;  // steps until the next offer
+                    room = n_now >= bar;
+                    if (!room && bar - n_now < (unsigned long long)again) again = (int)(bar - n_now);
                     if (room && S.mean_factor > 0) {
                         const unsigned long long cnt = *(volatile unsigned long long*)(S.stats + 1);
                         const unsigned long long sum = *(volatile unsigned long long*)(S.stats + 0);
-                        room = (cnt >= 32ULL) && ((unsigned long long)T.c.n_acc * cnt >= (unsigned long long)S.mean_factor * sum);
+                        room = (cnt >= 32ULL) && (n_now * cnt >= (unsigned long long)S.mean_factor * sum);
                     }
-                    if (!room) stop_at += S.budget;
+                    if (room) {
+                        const unsigned long long fin = ld_volatile(S.finished), out = ld_volatile(S.n_out);
+                        room = out < fin + (unsigned long long)(S.capacity + S.depth);
+                        if (!room) {
+                            again = 64;
+                            const unsigned long long now = global_ns(), last = ld_volatile(S.bar + 1);
+                            if (now - last > 20000ULL && atomicCAS(S.bar + 1, last, now) == last) {
+                                const unsigned long long b = bar > (unsigned long long)S.budget ? bar : (unsigned long long)S.budget;
+                                *(volatile unsigned long long*)S.bar = b + (b >> 6) + 1ULL;
+                            }
+                        }
+                    }
+                    if (!room) stop_at = T.c.n_acc + again;
                 }
                 if (room) {
                     const long long slot = (long long)atomicAdd(S.n_out, 1ULL);
@@ -321,18 +374,32 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
         }
     }
     stage_end(S.timeline);
+    __threadfence();  // this warp's slots are published before it counts as done
+    if (lane == 0) atomicAdd(S.done_warps, 1ULL);
 }
 
-// ---- six lanes per trajectory: continues the slots [*begin, min(*end, cap)) of `in` to their end
-// nq queues, served in this order: the pass's own slot range first, then the ranges of the stages
-// before it (their bulk passes are complete, so their slots are too): a pass that runs out of work
-// helps drain what an earlier, smaller pass is still working through.
+// ---- six lanes per trajectory: continues published checkpoint slots to their end.  Slots are taken
+// in the order they were handed out, by whichever pass asks first (*taken is the shared queue head,
+// advanced by compare-and-swap up to the number handed out so far).  A pass either runs BESIDE the
+// per-thread integrator (streaming: it polls for new slots and ends when every warp of that kernel
+// has exited and every slot is taken) or after it (the final pass: the same code, nothing to wait for).
+// Waiting is one-sided -- the per-thread integrator never waits for this kernel -- and bounded: a
+// streaming pass that does not see the per-thread integrator START within `patience_ns` (kernels
+// serialised by a profiler, a busy device) leaves, and what it would have done is done by the final pass.
 struct SplitSched {
     unsigned long long* timeline;
-    unsigned long long* loaded;  // diagnostics: trajectories this pass has taken
-    int nq;
-    unsigned long long* queue[4];
-    const unsigned long long *begin[4], *end[4];
+    unsigned long long* loaded;            // diagnostics: trajectories this pass has taken
+    unsigned long long* taken;             // queue head: slots [0, *taken) are claimed
+    const unsigned long long* n_out;       // slots handed out so far (may overshoot the capacity)
+    const unsigned long long* started;     // != 0 once the per-thread integrator of this call runs
+    const unsigned long long* done_warps;  // warps of it that have exited ...
+    unsigned long long producer_warps;     // ... of this many
+    unsigned long long patience_ns;
+    int poll_iters;                        // a warp with idle groups looks for new slots every this many iterations
+    unsigned long long* finished;          // trajectories finished by the six-lane passes
+    unsigned long long* bar;               // the hand-over bar (Sched); lowered here while groups are idle
+    unsigned long long bar_floor;          // ... down to this (the budget)
+    long long capacity;                    // groups of the streaming pass (0: this pass does not touch the bar)
     Ckpt in;
 };
 
@@ -345,114 +412,156 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
     const int lane = threadIdx.x & 31;
     const SplitRole R = make_role(P);
     const bool leader = !R.ghost && (lane == R.base);
-    int qi = 0;  // warp-uniform: the queue being served
-    long long first = 0, total = 0;
-    auto open_queue = [&]() {
-        const unsigned long long e = *S.end[qi];
-        first = (long long)*S.begin[qi];
-        total = (long long)(e < (unsigned long long)S.in.cap ? e : (unsigned long long)S.in.cap) - first;
-    };
-    open_queue();
-    // benign state for lanes without a trajectory (they take part in every shuffle)
+    const unsigned long long cap = (unsigned long long)S.in.cap;
     SplitState Y;
-    Y.xi = 1.0 + R.k;
-    Y.xa = 101.0 + 2.0 * R.k;
-    Y.vi = Y.va = Y.a1i = Y.a1a = 0.0;
     Core K;
-    K.t = P.t0;
-    K.h = 1.0;
-    K.sprev = 0.0;
-    K.n_acc = 0;
-    K.flags = 0u;
     ColdRegs C;
     C.rmin2_ = C.t_first_ = C.t_last_ = 0.0;
     C.n_rej_ = C.n_turn_ = 0;
     long long idx = -1;
     bool live = false;
-    bool dry = false;  // warp-uniform: every queue has been seen empty
 
-    // refill: every idle group takes the next slot of the queue (one atomicAdd per warp)
-    auto refill_once = [&]() -> bool {   // returns true when another round may place more groups
+    // refill: every idle group takes the next published slot (one compare-and-swap per warp)
+    auto refill = [&]() {
         const unsigned need = __ballot_sync(FULL, leader && !live);
-        if (need == 0u || dry) return false;
-        while (total <= 0) {  // skip empty ranges
-            if (++qi >= S.nq) {
-                dry = true;
-                return false;
-            }
-            open_queue();
-        }
+        if (need == 0u) return;
         const int cnt = __popc(need);
         unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(S.queue[qi], (unsigned long long)cnt);
-        base = __shfl_sync(FULL, base, 0);
+        int got = 0;
         if (lane == 0) {
-            const long long got = total - (long long)base;
-            if (got > 0) atomicAdd(S.loaded, (unsigned long long)(got < cnt ? got : cnt));
+            for (;;) {
+                const unsigned long long head = ld_volatile(S.taken);
+                unsigned long long avail = ld_volatile(S.n_out);
+                avail = avail < cap ? avail : cap;
+                if (head >= avail) {
+                    // nothing waits.  One warp of the streaming pass nudges the bar down (by 1/64, at most once per
+                    // 20 us) while a quarter of the groups are idle (plain stores: a lost update only delays the next)
+                    if (S.capacity > 0 && blockIdx.x == 0 && threadIdx.x == 0) {
+                        const unsigned long long busy = head - ld_volatile(S.finished);
+                        const unsigned long long bar = ld_volatile(S.bar);
+                        const unsigned long long now = global_ns();
+                        if (4 * busy < 3 * (unsigned long long)S.capacity && bar > S.bar_floor && now - ld_volatile(S.bar + 1) > 20000ULL) {
+                            const unsigned long long lower = bar - (bar >> 6) - 1ULL;
+                            *(volatile unsigned long long*)S.bar = lower > S.bar_floor ? lower : S.bar_floor;
+                            *(volatile unsigned long long*)(S.bar + 1) = now;
+                        }
+                    }
+                    break;
+                }
+                const unsigned long long want = (avail - head) < (unsigned long long)cnt ? (avail - head) : (unsigned long long)cnt;
+                if (atomicCAS(S.taken, head, head + want) == head) {
+                    base = head;
+                    got = (int)want;
+                    atomicAdd(S.loaded, want);
+                    break;
+                }
+            }
         }
+        got = __shfl_sync(FULL, got, 0);
+        base = __shfl_sync(FULL, base, 0);
+        if (got == 0) return;
         if (!R.ghost && ((need >> R.base) & 1u)) {
-            const long long cand = (long long)base + __popc(need & ((1u << R.base) - 1u));
-            if (cand < total) {
-                const long long slot = first + cand;
-                const size_t cap = (size_t)S.in.cap;
+            const int rank = __popc(need & ((1u << R.base) - 1u));
+            if (rank < got) {
+                const long long slot = (long long)base + rank;
+                idx = ckpt_wait(S.in, slot);
                 const double* d = S.in.d + slot;
-                Y.xi = d[(0 + R.k) * cap];
-                Y.xa = d[(3 + R.k) * cap];
-                Y.vi = d[(6 + R.k) * cap];
-                Y.va = d[(9 + R.k) * cap];
-                Y.a1i = d[(12 + R.k) * cap];
-                Y.a1a = d[(15 + R.k) * cap];
-                K.t = d[18 * cap];
-                K.h = d[19 * cap];
-                K.sprev = d[20 * cap];
-                C.rmin2_ = d[21 * cap];
-                C.t_first_ = d[22 * cap];
-                C.t_last_ = d[23 * cap];
+                Y.xi = __ldcg(d + (0 + R.k) * cap);
+                Y.xa = __ldcg(d + (3 + R.k) * cap);
+                Y.vi = __ldcg(d + (6 + R.k) * cap);
+                Y.va = __ldcg(d + (9 + R.k) * cap);
+                Y.a1i = __ldcg(d + (12 + R.k) * cap);
+                Y.a1a = __ldcg(d + (15 + R.k) * cap);
+                K.t = __ldcg(d + 18 * cap);
+                K.h = __ldcg(d + 19 * cap);
+                K.sprev = __ldcg(d + 20 * cap);
+                C.rmin2_ = __ldcg(d + 21 * cap);
+                C.t_first_ = __ldcg(d + 22 * cap);
+                C.t_last_ = __ldcg(d + 23 * cap);
                 const int* q = S.in.i + slot;
-                K.n_acc = q[0 * cap];
-                K.flags = (unsigned)q[1 * cap];
-                C.n_rej_ = q[2 * cap];
-                C.n_turn_ = q[3 * cap];
-                idx = S.in.idx[slot];
+                K.n_acc = __ldcg(q + 0 * cap);
+                K.flags = (unsigned)__ldcg(q + 1 * cap);
+                C.n_rej_ = __ldcg(q + 2 * cap);
+                C.n_turn_ = __ldcg(q + 3 * cap);
                 live = true;
             }
         }
-        if ((long long)base + cnt >= total) {  // this range is exhausted: go on with the next one
-            if (++qi >= S.nq) {
-                dry = true;
-                return false;
-            }
-            open_queue();
-            return true;
-        }
-        return false;
-    };
-    auto refill = [&]() {
-        while (refill_once()) {
-        }
     };
 
+    // state of a group without a trajectory: it takes part in every shuffle and, in the fast loop below, steps
+    // freely (an ion alone in the trap, the atom out of reach); nothing of it is ever stored
+    auto park = [&]() {
+        Y.xi = 1.0 + R.k;
+        Y.xa = 1.0e6 * (1.0 + R.k);
+        Y.vi = Y.va = Y.a1i = Y.a1a = 0.0;
+        K.t = P.t0;
+        K.h = 1.0;
+        K.sprev = 0.0;
+        K.n_acc = 0;
+        K.flags = 0u;
+    };
+    park();
+
     stage_begin(S.timeline);
-    refill();
-    if (!__any_sync(FULL, live)) {
-        stage_end(S.timeline);
-        return;
-    }
+    const unsigned long long t_begin = global_ns();
     for (;;) {
-        // ---- kSplitUnroll attempted steps for every group (all lanes together: full-mask shuffles
-        //      inside), straight-line code up to the vote below.  Several steps per basic block
-        //      because the step-size chain of one step continues into the next: the instruction
-        //      scheduler then sees it as the long path and orders a step's bookkeeping (state
-        //      selects, observables, stop tests) behind it instead of in front of it.  A group whose
-        //      trajectory ends inside the block idles for the rest of it (st keeps the status).
-        int st = -1;
-#pragma unroll
-        for (int u = 0; u < kSplitUnroll; ++u) {
-            SplitAttempt A;
-            StepTimes ST;
-            split_attempt<TRAP>(P, R, K, Y, A, ST);
+        if (!__any_sync(FULL, live)) {
+            // ---- nothing to step: take new slots, or find out that there will be none
+            refill();
+            if (!__any_sync(FULL, live)) {
+                int leave = 0;
+                if (lane == 0) {
+                    const unsigned long long now = global_ns();
+                    if (ld_volatile(S.done_warps) >= S.producer_warps) {
+                        __threadfence();
+                        unsigned long long avail = ld_volatile(S.n_out);
+                        avail = avail < cap ? avail : cap;
+                        leave = ld_volatile(S.taken) >= avail;
+                    } else if (ld_volatile(S.started) == 0ULL) {
+                        leave = (now - t_begin > S.patience_ns);
+                    } else {
+                        leave = (now - t_begin > 120000000000ULL);  // two minutes: never in practice
+                    }
+                }
+                if (__shfl_sync(FULL, leave, 0)) break;
+                __nanosleep(500);
+                continue;
+            }
+        }
+        // ---- fast loop: one attempted step of every group per iteration (all lanes together: full-mask
+        //      shuffles inside).  As long as every trajectory of the warp takes the common case (accepted,
+        //      nothing else happens: fast_step_ok) the loop body is ONE basic block -- commit, next attempt,
+        //      vote -- so that the step-size chain of one step continues into the next and the instruction
+        //      scheduler orders the bookkeeping behind it.  Groups without a trajectory never veto.  A warp
+        //      with idle groups leaves the loop every poll_iters steps to look for new slots.
+        const bool has_idle = __any_sync(FULL, leader && !live);
+        int since_poll = 0;
+        SplitAttempt A, B;
+        split_attempt<TRAP>(P, R, K, Y, A);
+        // two steps per iteration (A, B alternate): no register moves between the steps
+        for (;;) {
+            const bool okA = (!live | fast_step_ok(P, K, A.q_own, A.t_new, A.r2, A.s)) &
+                             !(has_idle & (++since_poll > S.poll_iters));
+            if (!__all_sync(FULL, okA)) break;
+            fast_step_commit(P, K, C, A.err, A.t_new, A.r2, A.s);
+            Y = A.Y;
+            split_attempt<TRAP>(P, R, K, Y, B);
+            const bool okB = !live | fast_step_ok(P, K, B.q_own, B.t_new, B.r2, B.s);
+            if (!__all_sync(FULL, okB)) {
+                A = B;
+                break;
+            }
+            fast_step_commit(P, K, C, B.err, B.t_new, B.r2, B.s);
+            Y = B.Y;
+            split_attempt<TRAP>(P, R, K, Y, A);
+        }
+        // ---- the general case, one step: rejections, turning points, stops (finish_core)
+        int st;
+        {
+            const StepTimes ST = step_times(P, K);
+            const double err = A.finite ? A.err : __longlong_as_double(0x7ff8000000000000LL);
             bool accepted, first_turn;
-            const int s1 = finish_core(P, K, C, A.err, ST, A.r2, A.s, live & (st < 0), accepted, first_turn);
+            st = finish_core(P, K, C, err, ST, A.r2, A.s, live, accepted, first_turn);
             // once per trajectory ("position"): lane (k, 0) holds component k of the ion
             if (first_turn && R.e == 0 && O.x_turn1) O.x_turn1[R.k * N + idx] = A.Y.xi;
             Y.xi = accepted ? A.Y.xi : Y.xi;
@@ -461,10 +570,8 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
             Y.xa = accepted ? A.Y.xa : Y.xa;
             Y.va = accepted ? A.Y.va : Y.va;
             Y.a1a = accepted ? A.Y.a1a : Y.a1a;
-            st = (st < 0) ? s1 : st;
         }
         const unsigned fin = __ballot_sync(FULL, st >= 0);
-        if (fin == 0u) continue;
         // ---- a8 (rare): lanes e = 0 store component k of the final state, the group's first lane
         //      the scalars; then the group takes the next slot
         if (st >= 0) {
@@ -479,43 +586,46 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
             if (leader) {
                 const double v0[3] = {__ldg(y0 + 9 * N + idx), __ldg(y0 + 10 * N + idx), __ldg(y0 + 11 * N + idx)};
                 store_scalars(idx, K, C, st, v0, v1, O);
+                atomicAdd(S.finished, 1ULL);
             }
             live = false;
-            // benign state again: the idle group keeps stepping (untouched by finish_core) until it is refilled
-            Y.xi = 1.0 + R.k;
-            Y.xa = 101.0 + 2.0 * R.k;
-            Y.vi = Y.va = Y.a1i = Y.a1a = 0.0;
-            K.t = P.t0;
-            K.h = 1.0;
-            K.flags = 0u;
+            park();
         }
-        refill();
-        if (!__any_sync(FULL, live)) break;
+        if (fin != 0u || has_idle) refill();
     }
     stage_end(S.timeline);
 }
 
 // ---- work-queue order: the trajectories that can become long first ------------------------------
 // (1) A trajectory can only form a complex (orders of magnitude more steps) if it gets over the
-//     centrifugal barrier of the -C4/r^4 tail, i.e. if its impact parameter b is below the
-//     Langevin radius b_c = (4 C4/E)^(1/4), E = mu u^2/2 (relative motion at t0): "candidates" are
-//     those with b < kappa b_c (kappa = 1.5: the moving ion and its micromotion blur the
-//     threshold).  Polynomial form of b^4 < kappa^4 b_c^4:  |d x u|^4 mu < 8 kappa^4 C4 |u|^2.
+//     centrifugal barrier of the -C4/r^4 tail, i.e. if the atom passes the ion within the Langevin
+//     radius b_c = (4 C4/E)^(1/4), E = mu u^2/2.  With the trap on, the ion is not where it started when
+//     the atom arrives (at q = 0.4 it has moved by more than the whole range of impact parameters), so
+//     the closest approach is estimated by a PRE-FLIGHT: the atom on its straight line against the ion on
+//     its secular orbit, x_k(t) = x_k0 cos w_k t + (v_k0/w_k) sin w_k t with w_k = (Omega/2) sqrt(a_k + q_k^2/2)
+//     (PAPER.md:282), sampled at 64 times over the fly-by and refined by a parabola.  "Candidates" pass
+//     within kappa b_c + the micromotion amplitude max_k |q_k x_k| / 2 there (kappa = 1.5: the rest of the
+//     blur), with b_c from the relative speed at that moment.  Without a trap this is the impact parameter.
 // (2) Among them the slow ones take longest: the flight alone lasts ~1/u, and the complexes that
 //     survive until t_max are low-energy ones (of the 12 longest trajectories of the bench
 //     workload all have u^2 < <u^2>/2; measured).
-// Three classes, queued in this order, each a stage of the schedule:
+// Three classes, queued in this order:
 //     0: candidates with u^2 < <u^2>/2   1: the other candidates, and anything with u^2 < <u^2>/10
 //     2: the rest
-// so that the longest trajectories start their sequential run in the six-lane integrator after the
-// first few per cent of the work instead of anywhere.  Affects scheduling only, never a result.
+// so that the longest trajectories start early -- and reach the six-lane integrator a few milliseconds
+// later -- instead of anywhere.  Affects scheduling only, never a result.
 constexpr int kCntClass = 24;    // counters: trajectories per class (3)
 constexpr int kCntCursor = 28;   // counters: placement cursors (3)
 constexpr int kCntMeanU2 = 60;   // counters: <u^2> (double bits)
+constexpr int kPlanSamples = 64;
 
 struct PlanArgs {
-    double mu, c4k;  // reduced mass, 8 kappa^4 C4
+    double mu, c4;        // reduced mass, C4
+    double kappa;
     double slow0, slow1;  // class thresholds as fractions of <u^2>
+    double w[3];          // secular frequencies of the ion (0: free along that axis)
+    double hq[3];         // |q_k| / 2: relative micromotion amplitude
+    double span;          // t_max - t0
 };
 
 __device__ __forceinline__ double rel_speed2(const double* __restrict__ y0, long long N, long long i)
@@ -528,14 +638,80 @@ __device__ __forceinline__ double rel_speed2(const double* __restrict__ y0, long
 __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long long N, long long i, const PlanArgs& A,
                                           double mean_u2)
 {
-    const double d0 = y0[6 * N + i] - y0[0 * N + i], d1 = y0[7 * N + i] - y0[1 * N + i],
-                 d2 = y0[8 * N + i] - y0[2 * N + i];
-    const double u0 = y0[9 * N + i] - y0[3 * N + i], u1 = y0[10 * N + i] - y0[4 * N + i],
-                 u2 = y0[11 * N + i] - y0[5 * N + i];
-    const double c0 = d1 * u2 - d2 * u1, c1 = d2 * u0 - d0 * u2, c2 = d0 * u1 - d1 * u0;
-    const double l2 = c0 * c0 + c1 * c1 + c2 * c2;
+    double xi[3], vi[3], xa[3], va[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        xi[k] = y0[(0 + k) * N + i];
+        vi[k] = y0[(3 + k) * N + i];
+        xa[k] = y0[(6 + k) * N + i];
+        va[k] = y0[(9 + k) * N + i];
+    }
+    const double d0 = xa[0] - xi[0], d1 = xa[1] - xi[1], d2 = xa[2] - xi[2];
+    const double u0 = va[0] - vi[0], u1 = va[1] - vi[1], u2 = va[2] - vi[2];
     const double usq = u0 * u0 + u1 * u1 + u2 * u2;
-    const bool cand = (l2 * l2 * A.mu < A.c4k * usq);
+    const double dsq = d0 * d0 + d1 * d1 + d2 * d2;
+    // fly-by window: twice the time to cover the initial distance, within the time span
+    double T = A.span;
+    if (usq > 0.0) T = fmin(T, 2.0 * sqrt(dsq / usq));
+    const double dt = T / kPlanSamples;
+    // ion on its secular orbit, by the rotation recurrence: (c, s)_j = (cos, sin)(w_k j dt); free axes move linearly
+    double c[3], sn[3], cd[3], sd[3], amp[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        c[k] = 1.0;
+        sn[k] = 0.0;
+        sincos(A.w[k] * dt, &sd[k], &cd[k]);
+        amp[k] = A.w[k] > 0.0 ? vi[k] / A.w[k] : 0.0;
+    }
+    double f_prev = dsq, f_best = dsq, f_before = dsq, f_after = dsq;
+    int j_best = 0;
+    bool want_after = true;
+    for (int j = 1; j <= kPlanSamples; ++j) {
+        const double t = dt * j;
+        double f = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double cn = c[k] * cd[k] - sn[k] * sd[k];
+            sn[k] = sn[k] * cd[k] + c[k] * sd[k];
+            c[k] = cn;
+            const double xk = A.w[k] > 0.0 ? xi[k] * c[k] + amp[k] * sn[k] : xi[k] + vi[k] * t;
+            const double dk = xa[k] + va[k] * t - xk;
+            f += dk * dk;
+        }
+        if (want_after) {
+            f_after = f;
+            want_after = false;
+        }
+        if (f < f_best) {
+            f_best = f;
+            f_before = f_prev;
+            j_best = j;
+            want_after = true;
+            f_after = f;
+        }
+        f_prev = f;
+    }
+    // parabola through the best sample and its neighbours
+    const double den = f_before - 2.0 * f_best + f_after;
+    double off = 0.0;
+    if (den > 0.0 && j_best > 0 && j_best < kPlanSamples) off = fmin(fmax(0.5 * (f_before - f_after) / den, -1.0), 1.0);
+    const double dmin2 = fmax(f_best - 0.25 * (f_before - f_after) * off, 0.0);
+    const double ts = dt * (j_best + off);
+    // relative speed and micromotion amplitude at the closest approach
+    double urel2 = 0.0, mm = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        double sk, ck;
+        sincos(A.w[k] * ts, &sk, &ck);
+        const double xk = A.w[k] > 0.0 ? xi[k] * ck + amp[k] * sk : xi[k] + vi[k] * ts;
+        const double vk = A.w[k] > 0.0 ? vi[k] * ck - xi[k] * A.w[k] * sk : vi[k];
+        const double uk = va[k] - vk;
+        urel2 += uk * uk;
+        mm = fmax(mm, A.hq[k] * fabs(xk));
+    }
+    // b_c = (8 C4 / (mu u^2))^(1/4)
+    const double bc = urel2 > 0.0 ? sqrt(sqrt(8.0 * A.c4 / (A.mu * urel2))) : 1.0e300;
+    const bool cand = sqrt(dmin2) < A.kappa * bc + mm;
     if (cand && usq < A.slow0 * mean_u2) return 0;
     if (cand || usq < A.slow1 * mean_u2) return 1;
     return 2;
@@ -559,16 +735,23 @@ plan_mean_kernel(const double* __restrict__ y0, const long long N, unsigned long
     }
 }
 
-// PLACE = 0: count the classes; PLACE = 1: write order[] (cursors set by plan_bounds_kernel)
+// PLACE = 0: classify (cls[]) and count the classes; PLACE = 1: write order[] (cursors set by plan_bounds_kernel)
 template <int PLACE>
 __global__ void __launch_bounds__(256)
 plan_kernel(const double* __restrict__ y0, const long long N, const PlanArgs A, long long* __restrict__ order,
-            unsigned long long* __restrict__ counters)
+            unsigned char* __restrict__ cls_of, unsigned long long* __restrict__ counters)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned FULL = 0xffffffffu;
-    const double mean_u2 = __longlong_as_double((long long)counters[kCntMeanU2]);
-    const int cls = (i < N) ? plan_class(y0, N, i, A, mean_u2) : -1;
+    int cls = -1;
+    if (i < N) {
+        if (PLACE) {
+            cls = cls_of[i];
+        } else {
+            cls = plan_class(y0, N, i, A, __longlong_as_double((long long)counters[kCntMeanU2]));
+            cls_of[i] = (unsigned char)cls;
+        }
+    }
     const int lane = threadIdx.x & 31;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -583,29 +766,18 @@ plan_kernel(const double* __restrict__ y0, const long long N, const PlanArgs A, 
     }
 }
 
-// cursors at the class starts; bound[0..3] = the three stages' ranges of order[].  A stage is a
-// class, except that empty classes at the end are skipped so that the LAST stage (the one whose
-// six-lane pass has the whole GPU) is never empty while an earlier one is not: with a degenerate
-// input (every trajectory in one class, e.g. a fixed launch speed) all the work is in the last stage.
+// cursors at the class starts; bound[0], bound[1] = the whole of order[] (one bulk pass over the
+// class-ordered queue)
 __global__ void plan_bounds_kernel(unsigned long long* counters, int bound0, int front)
 {
-    unsigned long long start[4];
     unsigned long long acc = 0;
     for (int c = 0; c < 3; ++c) {
-        start[c] = acc;
         counters[kCntCursor + c] = acc;
         acc += counters[kCntClass + c];
         if (c == 1) counters[front] = acc;  // classes 0 and 1 (diagnostics)
     }
-    start[3] = acc;
-    int last = 2;  // last non-empty class
-    while (last > 0 && start[last + 1] == start[last]) --last;
-    const int shift = 2 - last;  // stage s holds class s - shift (stages below `shift` are empty)
-    for (int st = 0; st <= 3; ++st) {
-        const int c = st - shift;
-        counters[bound0 + st] = (c <= 0) ? 0 : start[c];
-    }
-    counters[bound0 + 3] = acc;
+    counters[bound0] = 0;
+    counters[bound0 + 1] = acc;
 }
 
 // without a plan: one stage over [0, N)
@@ -615,20 +787,13 @@ __global__ void bounds_kernel(unsigned long long* counters, int bound0, unsigned
     counters[bound0 + 1] = N;
 }
 
-// Head start for the split pass of the previous stage: it is next in ITS stream's order and must take
-// its SMs before the bulk pass of this stage (other stream) fills them; both become ready when the
-// previous bulk pass ends.  Waits until the split pass has stamped its start (or at most `ns`).
+// Head start for the six-lane pass that runs beside the per-thread integrator: it is launched first, on
+// its own stream, and must take its SMs before the per-thread integrator fills them (both become ready
+// at the same moment).  Waits until the six-lane pass has stamped its start, or at most `ns`.
 __global__ void head_start_kernel(const unsigned long long* started, unsigned long long ns)
 {
     const unsigned long long t0 = global_ns();
     while (*(volatile const unsigned long long*)started == 0ULL && global_ns() - t0 < ns) __nanosleep(500);
-}
-
-// counters[dst] = min(counters[src], cap): freezes the number of checkpoint slots written so far
-__global__ void snapshot_kernel(unsigned long long* counters, int dst, int src, unsigned long long cap)
-{
-    const unsigned long long v = counters[src];
-    counters[dst] = v < cap ? v : cap;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1038,7 +1203,7 @@ int check_params(const aig_params* p, double t_max, double rtol, double atol)
     if (!finite(p->C4) || !finite(p->C8) || !finite(p->omega_rf)) return AIG_ERR_PARAM;
     for (int k = 0; k < 3; ++k)
         if (!finite(p->a[k]) || !finite(p->q[k])) return AIG_ERR_PARAM;
-    if (p->max_steps < 1) return AIG_ERR_PARAM;
+    if (p->max_steps < 1 || p->max_steps > 2147483647LL) return AIG_ERR_PARAM;  // the step counters are int32
     if (!(p->n_att == 0 && p->n_rep == 0) && !(p->n_att >= 1 && p->n_att < p->n_rep && p->n_rep <= 32)) return AIG_ERR_PARAM;
     if (std::isnan(p->r_exit) || std::isnan(p->r_turn)) return AIG_ERR_PARAM;
     return AIG_OK;
@@ -1099,77 +1264,45 @@ KParams make_kparams(const aig_params* p, double t_max, double rtol, double atol
 bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(ptr) % a) == 0; }
 
 // ---- schedule of one aig_integrate call ------------------------------------------------------
-//   plan        order[] in three classes (plan_*_kernel), bound[] = where each class starts
-//   stage i     (i = 0, 1, 2 = class; each on its own stream, stage 0 on the caller's):
-//     bulk i    per-thread integrator over class i; what outlives `budget` accepted steps, or is
-//               still running `tail_iters` iterations after the queue ran dry, is suspended into
-//               the next free checkpoint slots
-//     split i   six-lane integrator over the slots bulk i wrote.  Stage i + 1 starts when bulk i is
-//               complete (event), so split i runs BESIDE bulk i + 1: the longest trajectories
-//               (10^2..10^3 x the mean number of steps, nearly all in class 0) start their long
-//               sequential run after a few per cent of the work.  Beside a bulk pass it takes
-//               `split_sms` SMs for itself (one 8-warp block per SM that asks for the whole shared
-//               memory, so that no bulk block can share its FP64 pipes); that bulk pass is sized
-//               for the remaining SMs and lets the split pass take its SMs first (head_start_kernel).
-//   join        the caller's stream waits for the side streams.
-// No kernel waits for another one's progress (no polling for work): every dependency is a stream
-// order or an event; head_start_kernel only delays a launch, by at most 200 us.
-// Checkpoint slots: min(N, max(2^20, N/4)).  Hand-overs are bounded by 3 stages x (soft_cap + resident lanes)
-// ~ 1.6e5, so the capacity test in the kernel is a safety net, not a working regime.
+//   plan        order[]: the work queue in three classes (plan_*_kernel), likely-long trajectories first
+//   stream      six-lane integrator on a stream of its own, on `split_sms` SMs (one 8-warp block per SM
+//               that asks for the whole shared memory, so that no bulk block shares its FP64 pipes):
+//               takes checkpoint slots as the bulk pass publishes them
+//   bulk        per-thread integrator over the whole queue on the other SMs; what outlives `budget`
+//               accepted steps (and the mean of the finished ones, several times) is suspended into
+//               the next slot as soon as the six-lane pass has room for it, and so is whatever is
+//               still running `tail_iters` iterations after the queue ran dry
+//   final       six-lane integrator on the whole GPU: shares the remaining slots with the streaming pass
+//   join        the caller's stream waits for the streaming pass.
+// The longest trajectories (10^2..10^3 x the mean number of steps) start their long sequential run
+// in the six-lane integrator a few milliseconds after they were started, whatever class they are in.
+// Waiting is one-sided and bounded (SplitSched): the bulk pass never waits for anyone.
+// Checkpoint slots: min(N, max(2^20, N/4)); the capacity test in the kernel is a safety net.
 constexpr long long kMinSlots = 1 << 20;
 
 struct SchedConfig {
     int tail_iters = 256;     // iterations a warp keeps stepping after the queue ran dry
-    int budget = 2048;        // accepted steps after which the per-thread integrator hands a trajectory over
-    int split_sms = 32;       // SMs a six-lane pass takes for itself beside a bulk pass (one 8-warp block each)
-    int split_grid_b = 8;     // last six-lane pass: one-warp blocks per SM (it has the GPU to itself)
-    int soft_cap = 16384;     // budget hand-overs per bulk stage (drain hand-overs come on top)
-    int mean_factor = 4;      // ... and only of trajectories this many times longer than the finished ones' mean
+    int budget = 2048;        // accepted steps after which the per-thread integrator offers a trajectory
+    int split_sms = 16;       // SMs the streaming six-lane pass takes for itself (one 8-warp block each)
+    int split_grid_b = 8;     // final six-lane pass: one-warp blocks per SM (it has the GPU to itself)
+    int depth = 64;           // budget hand-overs stop while this many published slots wait to be taken
+    int mean_factor = 4;      // ... and are only for trajectories this many times longer than the finished ones' mean
     int drain_lanes = 10;     // queue empty: a warp hands over what it still runs once this few lanes are alive
     double slow0 = 0.5;       // class 0: candidates with u^2 < slow0 <u^2>
     double slow1 = 0.1;       // class 1 also takes anything with u^2 < slow1 <u^2>
     int refill_batch = 8;     // idle lanes of a warp that trigger its refill ...
     int refill_wait = 16;     // ... or iterations one of them has waited
-    int plan = 1;             // 0: natural order, one bulk launch
+    int plan = 1;             // 0: natural order
     double kappa = 1.5;       // candidates: b < kappa * Langevin radius
+    int poll_iters = 32;      // six-lane warps with idle groups look for new slots every this many iterations
 };
 
 std::mutex g_sched_mutex;
-SchedConfig g_sched;          // guarded by g_sched_mutex
-bool g_sched_init = false;
+SchedConfig g_sched;          // guarded by g_sched_mutex; changed by aig_set_schedule / aig_set_schedule_ex only
 
-// the schedule in force: defaults, overridden once by AIG_SCHED="tail_iters,budget,split_sms,
-// split_grid_b,plan,kappa" (tuning aid) and at any time by aig_set_schedule()
 SchedConfig sched_config()
 {
     std::lock_guard<std::mutex> lock(g_sched_mutex);
-    if (!g_sched_init) {
-        SchedConfig c;
-        if (const char* e = std::getenv("AIG_SCHED")) {
-            int a = c.tail_iters, b = c.budget, ga = c.split_sms, gb = c.split_grid_b, pl = c.plan;
-            double kp = c.kappa;
-            const int got = std::sscanf(e, "%d,%d,%d,%d,%d,%lf", &a, &b, &ga, &gb, &pl, &kp);
-            if (got >= 1 && a >= 0) c.tail_iters = a;
-            if (got >= 2 && b >= 1) c.budget = b;
-            if (got >= 3 && ga >= 1) c.split_sms = ga;
-            if (got >= 4 && gb >= 1) c.split_grid_b = gb;
-            if (got >= 5) c.plan = pl;
-            if (got >= 6 && kp >= 0.0) c.kappa = kp;
-        }
-        if (const char* e = std::getenv("AIG_REFILL")) {  // "batch,wait,slow0,slow1,mean_factor,drain_lanes" (tuning aid)
-            int b = c.refill_batch, w = c.refill_wait, mf = c.mean_factor, dl = c.drain_lanes;
-            double s0 = c.slow0, s1 = c.slow1;
-            const int got = std::sscanf(e, "%d,%d,%lf,%lf,%d,%d", &b, &w, &s0, &s1, &mf, &dl);
-            if (got >= 5 && mf >= 0) c.mean_factor = mf;
-            if (got >= 6 && dl >= 0) c.drain_lanes = dl;
-            if (got >= 1 && b >= 1) c.refill_batch = b;
-            if (got >= 2 && w >= 0) c.refill_wait = w;
-            if (got >= 3 && s0 >= 0.0) c.slow0 = s0;
-            if (got >= 4 && s1 >= 0.0) c.slow1 = s1;
-        }
-        g_sched = c;
-        g_sched_init = true;
-    }
     return g_sched;
 }
 
@@ -1177,26 +1310,28 @@ long long slot_capacity(long long N) { return std::min(N < 1 ? 1 : N, std::max(k
 
 size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// workspace: 64 uint64 counters | order[N] (int64) | checkpoint slots
+// workspace: 64 uint64 counters | order[N] (int64) | class[N] (uint8) | checkpoint slots
 constexpr size_t kCounterBytes = 64 * sizeof(unsigned long long);
 size_t order_bytes(long long N) { return round_up((size_t)(N < 1 ? 1 : N) * sizeof(long long), 256); }
+size_t class_bytes(long long N) { return round_up((size_t)(N < 1 ? 1 : N), 256); }
 size_t ckpt_buffer_bytes(long long cap) { return round_up((size_t)cap * kCkptBytesPerSlot, 256); }
 
-// counters (uint64 each).  Stage i of the schedule: bulk pass over order[bound[i], bound[i+1]), its
-// hand-overs are the slots [snap[i], snap[i+1]).
-constexpr int kMaxStages = 4;
+// counters (uint64 each)
 enum Counter {
-    kCntFront = 0,   // plan: candidates placed (= n_front)
-    kCntZero = 2,    // constant 0
-    kCntN = 3,       // constant N
-    kCntSlots = 4,   // checkpoint slots handed out so far (may overshoot the capacity)
-    kCntBound = 5,   // bound[0 .. kMaxStages]
-    kCntSnap = 10,   // snap[0 .. kMaxStages], snap[0] = 0
-    kCntQueueBulk = 16,   // work queue of bulk pass i
-    kCntQueueSplit = 20,  // work queue of split pass i
-    kCntLoaded = 61,      // diagnostics: trajectories split pass i has taken (its own and earlier stages')
-    kCntStats = 52        // [2 i], [2 i + 1]: accepted steps / number of the trajectories bulk pass i has finished
+    kCntFront = 0,       // plan: candidates placed (classes 0 and 1)
+    kCntStarted = 2,     // the bulk pass has started
+    kCntDoneWarps = 3,   // warps of the bulk pass that have exited
+    kCntSlots = 4,       // checkpoint slots handed out so far (may overshoot the capacity)
+    kCntBound = 5,       // bound[0], bound[1]: the bulk pass's range of order[]
+    kCntTaken = 8,       // slots claimed by the six-lane passes so far
+    kCntFinished = 9,    // trajectories the six-lane passes have finished
+    kCntBar = 10,        // the hand-over bar (accepted steps), and at [11] the %globaltimer of its last change
+    kCntQueueBulk = 16,  // work queue of the bulk pass
+    kCntLoaded = 61,     // diagnostics: trajectories taken by the streaming / the final six-lane pass
+    kCntStats = 52       // accepted steps / number of the trajectories the bulk pass has finished
 };
+// stage timeline slots (kCntTime + 2 s): 0 plan (unused), 1 bulk, 2 streaming six-lane pass, 3 final six-lane pass
+constexpr int kStageBulk = 1, kStageStream = 2, kStageFinal = 3;
 
 Ckpt ckpt_at(unsigned char* base, long long cap)
 {
@@ -1222,32 +1357,28 @@ int bulk_capacity(int* blocks_per_sm, int* sm_count)
     return AIG_OK;
 }
 
-// side streams (stage i >= 1 runs on stream i - 1) and the events that chain and join them, one set
-// per device
-struct SideStreams {
-    cudaStream_t stream[kMaxStages - 1] = {};
-    cudaEvent_t done[kMaxStages] = {};   // done[i]: bulk pass i and its snapshot are complete
-    cudaEvent_t join[kMaxStages - 1] = {};
+// The side stream of the streaming six-lane pass and the two events that fork and join it, one set per
+// device.  g_enqueue_mutex is held over the whole enqueue section of a call, so every record / wait
+// pair is atomic with respect to other host threads calling aig_integrate on the same device.
+struct SideStream {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
     bool ok = false;
 };
-std::mutex g_side_mutex;
+std::mutex g_enqueue_mutex;
 
-SideStreams* side_streams()
+SideStream* side_stream()   // call with g_enqueue_mutex held
 {
-    static SideStreams side[64];
+    static SideStream side[64];
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
-    std::lock_guard<std::mutex> lock(g_side_mutex);
-    SideStreams& s = side[dev];
+    SideStream& s = side[dev];
     if (!s.ok) {
         int lo = 0, hi = 0;
         if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return nullptr;
-        for (int i = 0; i < kMaxStages - 1; ++i) {
-            if (cudaStreamCreateWithPriority(&s.stream[i], cudaStreamNonBlocking, lo) != cudaSuccess) return nullptr;
-            if (cudaEventCreateWithFlags(&s.join[i], cudaEventDisableTiming) != cudaSuccess) return nullptr;
-        }
-        for (int i = 0; i < kMaxStages; ++i)
-            if (cudaEventCreateWithFlags(&s.done[i], cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaStreamCreateWithPriority(&s.stream, cudaStreamNonBlocking, hi) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
         s.ok = true;
     }
     return &s;
@@ -1257,7 +1388,7 @@ constexpr int kSplitMinBlocks = 8;  // register cap of the split kernel: 65536 /
 #ifndef AIG_SPLIT_WARPS
 #define AIG_SPLIT_WARPS 8
 #endif
-constexpr int kSplitWarps = AIG_SPLIT_WARPS;  // warps per block of the SM-owning variant: two per scheduler (a warp issues 30 % of the
+constexpr int kSplitWarps = AIG_SPLIT_WARPS;  // warps per block of the SM-owning variant: two per scheduler (a warp issues a third of the
                                               // time, so two barely slow each other while the queue is long; at the end each is alone)
 
 template <int TRAP>
@@ -1268,12 +1399,16 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     const long long cap = slot_capacity(N);
     unsigned long long* counters = static_cast<unsigned long long*>(workspace);
     long long* order = reinterpret_cast<long long*>(static_cast<unsigned char*>(workspace) + kCounterBytes);
-    const Ckpt slots = ckpt_at(static_cast<unsigned char*>(workspace) + kCounterBytes + order_bytes(N), cap);
-    if (cudaMemsetAsync(counters, 0, kCounterBytes, st) != cudaSuccess) return AIG_ERR_CUDA;
-    const unsigned long long n64 = (unsigned long long)N;
-    if (cudaMemcpyAsync(counters + kCntN, &n64, sizeof(n64), cudaMemcpyHostToDevice, st) != cudaSuccess)
-        return AIG_ERR_CUDA;
+    unsigned char* cls_of = static_cast<unsigned char*>(workspace) + kCounterBytes + order_bytes(N);
+    const Ckpt slots = ckpt_at(cls_of + class_bytes(N), cap);
 
+    int bps = 0, sms = 0;
+    int rc = bulk_capacity<TRAP>(&bps, &sms);
+    if (rc) return rc;
+    int dev = 0, smem_optin = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        return AIG_ERR_CUDA;
     {
         // CUDA loads a kernel's code at its first launch (lazy module loading), and loading may have to
         // wait for the kernels that are running: the first call would serialise the passes that are meant
@@ -1287,33 +1422,47 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
             cudaFuncGetAttributes(&fa, plan_kernel<1>) != cudaSuccess ||
             cudaFuncGetAttributes(&fa, plan_bounds_kernel) != cudaSuccess ||
             cudaFuncGetAttributes(&fa, bounds_kernel) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, snapshot_kernel) != cudaSuccess ||
             cudaFuncGetAttributes(&fa, head_start_kernel) != cudaSuccess)
             return AIG_ERR_CUDA;
+        if (cudaFuncSetAttribute(integrate_split_kernel<TRAP, kSplitWarps, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 smem_optin) != cudaSuccess)
+            return AIG_ERR_CUDA;
     }
-    int bps = 0, sms = 0;
-    int rc = bulk_capacity<TRAP>(&bps, &sms);
-    if (rc) return rc;
-    const long long blocks = std::min((long long)bps * sms, (N + kBlock - 1) / kBlock);
     const bool plan = cfg.plan != 0 && p->C4 > 0.0 && (p->n_att == 0 || p->n_att == 4);  // the Langevin test is the r^-4 tail's
-    // stages: the three classes of the plan; without a plan one stage over [0, N)
-    const int stages = plan ? 3 : 1;
-    SideStreams* side = stages > 1 ? side_streams() : nullptr;
-    if (stages > 1 && !side) return AIG_ERR_CUDA;
+    // the streaming pass: on its own SMs when the work is large enough to fill the others
+    const long long own = std::max<long long>(1, std::min<long long>(cfg.split_sms, sms / 2));
+    const long long blocks_all = std::min((long long)bps * sms, (N + kBlock - 1) / kBlock);
+    const long long blocks = std::max<long long>(1, std::min<long long>(blocks_all, (long long)bps * (sms - own)));
+    const unsigned split_last =
+        (unsigned)std::min<long long>((long long)cfg.split_grid_b * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
 
+    std::lock_guard<std::mutex> enqueue_lock(g_enqueue_mutex);
+    SideStream* side = side_stream();
+    if (!side) return AIG_ERR_CUDA;
+
+    if (cudaMemsetAsync(counters, 0, kCounterBytes, st) != cudaSuccess) return AIG_ERR_CUDA;
+    // slot index entries = -1: "not published" (ckpt_store / ckpt_wait)
+    if (cudaMemsetAsync(slots.idx, 0xFF, (size_t)cap * sizeof(long long), st) != cudaSuccess) return AIG_ERR_CUDA;
     long long* order_arg = nullptr;
     if (plan) {
         PlanArgs A;
         A.mu = p->m_ion * p->m_atom / (p->m_ion + p->m_atom);
-        const double k2 = cfg.kappa * cfg.kappa;
-        A.c4k = 8.0 * k2 * k2 * p->C4;
+        A.c4 = p->C4;
+        A.kappa = cfg.kappa;
         A.slow0 = cfg.slow0;
         A.slow1 = cfg.slow1;
+        A.span = K.t_max - K.t0;
+        for (int k = 0; k < 3; ++k) {
+            // secular frequency (Omega/2) sqrt(a_k + q_k^2/2); not confining: free along that axis
+            const double beta2 = p->a[k] + 0.5 * p->q[k] * p->q[k];
+            A.w[k] = beta2 > 0.0 ? 0.5 * std::fabs(p->omega_rf) * std::sqrt(beta2) : 0.0;
+            A.hq[k] = 0.5 * std::fabs(p->q[k]);
+        }
         const unsigned pg = (unsigned)((N + 255) / 256);
         plan_mean_kernel<<<1, 1024, 0, st>>>(y0, N, counters);
-        plan_kernel<0><<<pg, 256, 0, st>>>(y0, N, A, order, counters);
+        plan_kernel<0><<<pg, 256, 0, st>>>(y0, N, A, order, cls_of, counters);
         plan_bounds_kernel<<<1, 1, 0, st>>>(counters, kCntBound, kCntFront);
-        plan_kernel<1><<<pg, 256, 0, st>>>(y0, N, A, order, counters);
+        plan_kernel<1><<<pg, 256, 0, st>>>(y0, N, A, order, cls_of, counters);
         g_kernel_launches += 4;
         order_arg = order;
     } else {
@@ -1321,73 +1470,63 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         g_kernel_launches++;
     }
 
-    int dev = 0, smem_optin = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
-        return AIG_ERR_CUDA;
-    if (cudaFuncSetAttribute(integrate_split_kernel<TRAP, kSplitWarps, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             smem_optin) != cudaSuccess)
-        return AIG_ERR_CUDA;
-    const long long own = std::max<long long>(1, std::min<long long>(cfg.split_sms, sms / 2));
-    const long long blocks_beside = std::max<long long>(1, std::min<long long>(blocks, (long long)bps * (sms - own)));
-    const unsigned split_last =
-        (unsigned)std::min<long long>((long long)cfg.split_grid_b * sms, (cap + kGroupsPerWarp - 1) / kGroupsPerWarp);
+    SplitSched T;
+    T.in = slots;
+    T.taken = counters + kCntTaken;
+    T.n_out = counters + kCntSlots;
+    T.started = counters + kCntStarted;
+    T.done_warps = counters + kCntDoneWarps;
+    T.producer_warps = (unsigned long long)blocks * (kBlock / 32);
+    T.poll_iters = cfg.poll_iters;
+    T.finished = counters + kCntFinished;
+    T.bar = counters + kCntBar;
+    T.bar_floor = (unsigned long long)cfg.budget;
+    T.capacity = own * kSplitWarps * kGroupsPerWarp;
 
-    // Stage i on its own stream (stage 0: the caller's): bulk pass i, snapshot, [event done_i], split pass i.
-    // Stage i + 1 waits for done_i, so bulk pass i + 1 runs beside split pass i; the split pass comes first
-    // in its own stream's order and takes its SMs before the next bulk pass (other stream, event) arrives.
-    for (int i = 0; i < stages; ++i) {
-        cudaStream_t cs = (i == 0) ? st : side->stream[i - 1];
-        if (i > 0) {
-            if (cudaStreamWaitEvent(cs, side->done[i - 1], 0) != cudaSuccess) return AIG_ERR_CUDA;
-            // split pass i - 1 stamps counters[kCntTime + 2 (2 + 2 (i - 1))] when its first block starts
-            head_start_kernel<<<1, 1, 0, cs>>>(counters + kCntTime + 2 * (2 + 2 * (i - 1)), 200000ULL);
-            g_kernel_launches++;
-        }
-        Sched S;
-        S.order = order_arg;
-        S.queue = counters + kCntQueueBulk + i;
-        S.begin = counters + kCntBound + i;
-        S.end = counters + kCntBound + i + 1;
-        S.n_out = counters + kCntSlots;
-        S.soft_base = counters + kCntSnap + i;
-        S.soft_cap = cfg.soft_cap;
-        S.out = slots;
-        S.budget = cfg.budget;
-        S.tail_iters = cfg.tail_iters;
-        S.refill_batch = cfg.refill_batch;
-        S.refill_wait = cfg.refill_wait;
-        S.drain_lanes = cfg.drain_lanes;
-        S.stats = counters + kCntStats + 2 * i;
-        S.mean_factor = cfg.mean_factor;
-        S.timeline = counters + kCntTime + 2 * (1 + 2 * i);
-        const long long grid = (i == 0) ? blocks : blocks_beside;
-        integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)grid, kBlock, 0, cs>>>(K, y0, N, O, S);
-        snapshot_kernel<<<1, 1, 0, cs>>>(counters, kCntSnap + i + 1, kCntSlots, (unsigned long long)cap);
-        g_kernel_launches += 2;
-        if (i + 1 < stages && cudaEventRecord(side->done[i], cs) != cudaSuccess) return AIG_ERR_CUDA;
-        SplitSched T;
-        T.in = slots;
-        T.timeline = counters + kCntTime + 2 * (2 + 2 * i);
-        T.loaded = counters + kCntLoaded + i;
-        T.nq = i + 1;
-        for (int j = 0; j <= i; ++j) {  // own range first, then the earlier stages'
-            T.queue[j] = counters + kCntQueueSplit + (i - j);
-            T.begin[j] = counters + kCntSnap + (i - j);
-            T.end[j] = counters + kCntSnap + (i - j) + 1;
-        }
-        if (i + 1 < stages) {
-            // beside the next bulk pass: one block per SM it owns (the dynamic shared memory request
-            // leaves no room for a bulk block next to it)
-            integrate_split_kernel<TRAP, kSplitWarps, 1><<<(unsigned)own, 32 * kSplitWarps, (size_t)smem_optin, cs>>>(K, y0, N, O, T);
-        } else {
-            integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_last, 32, 0, cs>>>(K, y0, N, O, T);
-        }
-        g_kernel_launches++;
-        if (i > 0 && cudaEventRecord(side->join[i - 1], cs) != cudaSuccess) return AIG_ERR_CUDA;
-    }
-    for (int i = 1; i < stages; ++i)
-        if (cudaStreamWaitEvent(st, side->join[i - 1], 0) != cudaSuccess) return AIG_ERR_CUDA;
+    // streaming six-lane pass on the side stream: launched first, so that it owns its SMs
+    if (cudaEventRecord(side->fork, st) != cudaSuccess || cudaStreamWaitEvent(side->stream, side->fork, 0) != cudaSuccess)
+        return AIG_ERR_CUDA;
+    T.timeline = counters + kCntTime + 2 * kStageStream;
+    T.loaded = counters + kCntLoaded;
+    T.patience_ns = 2000000ULL;  // 2 ms to see the bulk pass start
+    integrate_split_kernel<TRAP, kSplitWarps, 1><<<(unsigned)own, 32 * kSplitWarps, (size_t)smem_optin, side->stream>>>(K, y0, N, O, T);
+    g_kernel_launches++;
+    if (cudaEventRecord(side->join, side->stream) != cudaSuccess) return AIG_ERR_CUDA;
+
+    // bulk pass on the caller's stream, behind a short wait for the streaming pass to have taken its SMs
+    head_start_kernel<<<1, 1, 0, st>>>(counters + kCntTime + 2 * kStageStream, 200000ULL);
+    Sched S;
+    S.order = order_arg;
+    S.queue = counters + kCntQueueBulk;
+    S.begin = counters + kCntBound;
+    S.end = counters + kCntBound + 1;
+    S.n_out = counters + kCntSlots;
+    S.finished = counters + kCntFinished;
+    S.bar = counters + kCntBar;
+    S.capacity = own * kSplitWarps * kGroupsPerWarp;
+    S.started = counters + kCntStarted;
+    S.done_warps = counters + kCntDoneWarps;
+    S.out = slots;
+    S.depth = cfg.depth;
+    S.budget = cfg.budget;
+    S.tail_iters = cfg.tail_iters;
+    S.refill_batch = cfg.refill_batch;
+    S.refill_wait = cfg.refill_wait;
+    S.drain_lanes = cfg.drain_lanes;
+    S.stats = counters + kCntStats;
+    S.mean_factor = cfg.mean_factor;
+    S.timeline = counters + kCntTime + 2 * kStageBulk;
+    integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
+    g_kernel_launches += 2;
+
+    // final six-lane pass: the whole GPU on what is left (the bulk pass is complete: nothing to wait for)
+    T.timeline = counters + kCntTime + 2 * kStageFinal;
+    T.loaded = counters + kCntLoaded + 1;
+    T.patience_ns = 0ULL;
+    T.capacity = 0;
+    integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_last, 32, 0, st>>>(K, y0, N, O, T);
+    g_kernel_launches++;
+    if (cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) return AIG_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
 
@@ -1402,7 +1541,6 @@ uint64_t aig_kernel_launches(void) { return g_kernel_launches.load(); }
 int aig_set_schedule(int tail_iters, int budget, int split_sms, int split_grid, int plan, double kappa)
 {
     if (tail_iters < 0 || budget < 1 || split_sms < 1 || split_grid < 1 || !(kappa >= 0.0)) return AIG_ERR_PARAM;
-    (void)sched_config();  // settle the defaults / environment first
     std::lock_guard<std::mutex> lock(g_sched_mutex);
     g_sched.tail_iters = tail_iters;
     g_sched.budget = budget;
@@ -1410,6 +1548,55 @@ int aig_set_schedule(int tail_iters, int budget, int split_sms, int split_grid, 
     g_sched.split_grid_b = split_grid;
     g_sched.plan = plan;
     g_sched.kappa = kappa;
+    return AIG_OK;
+}
+
+int aig_set_schedule_ex(const aig_schedule* s)
+{
+    std::lock_guard<std::mutex> lock(g_sched_mutex);
+    if (!s) {  // back to the defaults
+        g_sched = SchedConfig();
+        return AIG_OK;
+    }
+    if (s->tail_iters < 0 || s->budget < 1 || s->split_sms < 1 || s->split_grid < 1 || !(s->kappa >= 0.0) ||
+        s->depth < 1 || s->mean_factor < 0 || s->drain_lanes < 0 || s->drain_lanes > 32 || !(s->slow0 >= 0.0) ||
+        !(s->slow1 >= 0.0) || s->refill_batch < 1 || s->refill_batch > 32 || s->refill_wait < 0 || s->poll_iters < 1)
+        return AIG_ERR_PARAM;
+    g_sched.tail_iters = s->tail_iters;
+    g_sched.budget = s->budget;
+    g_sched.split_sms = s->split_sms;
+    g_sched.split_grid_b = s->split_grid;
+    g_sched.plan = s->plan;
+    g_sched.kappa = s->kappa;
+    g_sched.depth = s->depth;
+    g_sched.mean_factor = s->mean_factor;
+    g_sched.drain_lanes = s->drain_lanes;
+    g_sched.slow0 = s->slow0;
+    g_sched.slow1 = s->slow1;
+    g_sched.refill_batch = s->refill_batch;
+    g_sched.refill_wait = s->refill_wait;
+    g_sched.poll_iters = s->poll_iters;
+    return AIG_OK;
+}
+
+int aig_get_schedule(aig_schedule* s)
+{
+    if (!s) return AIG_ERR_NULL;
+    const SchedConfig c = sched_config();
+    s->tail_iters = c.tail_iters;
+    s->budget = c.budget;
+    s->split_sms = c.split_sms;
+    s->split_grid = c.split_grid_b;
+    s->plan = c.plan;
+    s->kappa = c.kappa;
+    s->depth = c.depth;
+    s->mean_factor = c.mean_factor;
+    s->drain_lanes = c.drain_lanes;
+    s->slow0 = c.slow0;
+    s->slow1 = c.slow1;
+    s->refill_batch = c.refill_batch;
+    s->refill_wait = c.refill_wait;
+    s->poll_iters = c.poll_iters;
     return AIG_OK;
 }
 
@@ -1430,8 +1617,8 @@ const char* aig_strerror(int code)
 
 size_t aig_workspace_bytes(int64_t N)
 {
-    // counters + work-queue order (8 B per trajectory) + checkpoint slots for suspended trajectories
-    return kCounterBytes + order_bytes(N) + ckpt_buffer_bytes(slot_capacity(N));
+    // counters + work-queue order (8 B per trajectory) + class (1 B) + checkpoint slots for suspended trajectories
+    return kCounterBytes + order_bytes(N) + class_bytes(N) + ckpt_buffer_bytes(slot_capacity(N));
 }
 
 int aig_integrate(const aig_params* p, const double* y0, int64_t N, double t_max, double rtol,

@@ -72,7 +72,9 @@ __device__ __forceinline__ SplitRole make_role(const KParams& P)
 // Result of one attempted step as seen by one lane.
 struct SplitAttempt {
     SplitState Y;              // ynew (component k) and f(t_new, ynew)
-    double t_new, err, r2, s;  // as in Attempt
+    double t_new, err, r2, s;  // as in Attempt, except: err = the raw estimate, to be replaced by NaN when !finite
+    double q_own;              // this lane's axis quotient (err = h max over the three axes)
+    bool finite;
 };
 
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
@@ -152,14 +154,11 @@ __device__ __forceinline__ double level_close(const KParams& P, const SplitRole&
 // together (full-mask shuffles); lanes without a trajectory run it on benign dummy state.
 template <int TRAP>
 __device__ __forceinline__ void split_attempt(const KParams& P, const SplitRole& R, const Core& K,
-                                              const SplitState& Y, SplitAttempt& out, StepTimes& ST)
+                                              const SplitState& Y, SplitAttempt& out)
 {
     const double h = K.h;
     const double h2 = h * h;
-    ST = step_times(P, K);
-    // pin the (t, h)-only quantities here: the compiler would otherwise sink them to their use behind
-    // the error estimate, onto the step's dependent chain
-    asm volatile("" : "+d"(ST.hmin_cur), "+d"(ST.hmin_new), "+d"(ST.rem_new));
+    const double t_new = (K.flags & kLast) ? P.t_max : K.t + h;
     double Ai[7], Aa[7];
     Ai[0] = Y.a1i;
     Aa[0] = Y.a1a;
@@ -168,7 +167,7 @@ __device__ __forceinline__ void split_attempt(const KParams& P, const SplitRole&
     level_open<0>(R, Y, d0, u0, h, h2, Ai, Aa, L);
     // the cos of my stage time, inside the first level's shuffle and reciprocal latency
     double mycos = 1.0;
-    if (trap_of(TRAP) == TRAP_RF || trap_of(TRAP) == TRAP_RF_BIG) mycos = trap_cos<TRAP>(P, R.cos_end ? ST.t_new : fma(R.cCos, h, K.t));
+    if (trap_of(TRAP) == TRAP_RF || trap_of(TRAP) == TRAP_RF_BIG) mycos = trap_cos<TRAP>(P, R.cos_end ? t_new : fma(R.cCos, h, K.t));
     level_close<TRAP, 0>(P, R, L, mycos, Ai, Aa);
     level_open<1>(R, Y, d0, u0, h, h2, Ai, Aa, L);
     level_close<TRAP, 1>(P, R, L, mycos, Ai, Aa);
@@ -193,8 +192,10 @@ __device__ __forceinline__ void split_attempt(const KParams& P, const SplitRole&
     const double q0 = shfl_d(q, src), q1 = shfl_d(q, src + 2), q2 = shfl_d(q, src + 4);
     const double p0 = shfl_d(p, src), p1 = shfl_d(p, src + 2), p2 = shfl_d(p, src + 4);
     out.s = sum3(p0, p1, p2);
-    out.t_new = ST.t_new;
-    out.err = error_estimate(h, q0, q1, q2, out.r2, out.s);
+    out.t_new = t_new;
+    out.q_own = q;
+    out.err = error_raw(h, q0, q1, q2);
+    out.finite = attempt_finite(q0, q1, q2, out.r2, out.s);
     out.Y.xi = xni;
     out.Y.vi = vni;
     out.Y.a1i = Ai[6];
