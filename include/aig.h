@@ -93,7 +93,8 @@ typedef struct aig_out {
 } aig_out;
 
 /* Bin edges of the observable histograms: DEVICE pointers to strictly increasing doubles
- * (n_bins + 1 of them).  Bin j holds edges[j] <= v < edges[j+1]. */
+ * (n_bins + 1 of them).  Bin j holds edges[j] <= v < edges[j+1].  Each bin count is in 1 .. 2048
+ * (AIG_ERR_SIZE otherwise; aig_run_host checks the same). */
 typedef struct aig_hist_spec {
     const double *angle_edges;
     int32_t n_angle_bins;
@@ -247,6 +248,7 @@ typedef struct aig_schedule {
     int32_t refill_batch, refill_wait; /* idle lanes of a warp that trigger its refill (8), or iterations
                                           one of them has waited (16) */
     int32_t poll_iters;   /* six-lane warps with idle groups look for new slots every this many iterations (32) */
+    int32_t hist_blocks_per_sm; /* grid of aig_histogram's kernel: blocks of 256 threads per SM (8) */
 } aig_schedule;
 /* s = NULL restores the defaults.  AIG_ERR_PARAM for out-of-range values. */
 int aig_set_schedule_ex(const aig_schedule *s);

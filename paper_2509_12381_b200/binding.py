@@ -320,7 +320,8 @@ class Schedule(C.Structure):
     _fields_ = [("tail_iters", C.c_int32), ("budget", C.c_int32), ("split_sms", C.c_int32), ("split_grid", C.c_int32),
                 ("plan", C.c_int32), ("kappa", C.c_double), ("depth", C.c_int32), ("mean_factor", C.c_int32),
                 ("drain_lanes", C.c_int32), ("slow0", C.c_double), ("slow1", C.c_double),
-                ("refill_batch", C.c_int32), ("refill_wait", C.c_int32), ("poll_iters", C.c_int32)]
+                ("refill_batch", C.c_int32), ("refill_wait", C.c_int32), ("poll_iters", C.c_int32),
+                ("hist_blocks_per_sm", C.c_int32)]
 
 
 def get_schedule() -> dict:

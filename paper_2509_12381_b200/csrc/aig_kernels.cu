@@ -860,13 +860,15 @@ __device__ __forceinline__ int bin_of(const double* __restrict__ edges, int nb, 
     return lo;
 }
 
-// warp-aggregated increment of a shared-memory bin: lanes that hit the same bin elect one
-// leader that adds the group's population count (active lanes only).
-__device__ __forceinline__ void agg_inc(unsigned int* bins, int bin)
+// The same count, starting from a guess j0 (exact for ANY strictly increasing edges: the two loops walk to
+// the answer; with near-uniform edges and a linear guess they run at most once or twice).
+__device__ __forceinline__ int bin_from_guess(const double* __restrict__ edges, int nb, double v, int j0)
 {
-    const unsigned act = __activemask();
-    const unsigned grp = __match_any_sync(act, bin);
-    if ((threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(&bins[bin], (unsigned)__popc(grp));
+    if (v != v) return nb + 1;
+    int j = j0 < 0 ? 0 : (j0 > nb + 1 ? nb + 1 : j0);
+    while (j <= nb && edges[j] <= v) ++j;
+    while (j > 0 && edges[j - 1] > v) --j;
+    return j;
 }
 
 struct HistArgs {
@@ -878,6 +880,13 @@ struct HistArgs {
     unsigned long long *h_angle, *h_life, *h_turn, *h_status, *h_totals;
 };
 
+// HBM-bound: 33 B per trajectory (angle, lifetime, four int32, the flag).
+// Grid-stride over N, four trajectories per thread and iteration with all loads issued first; bins
+// privatised in shared memory (edges staged there too).  The 4-valued status and the small n_turn values
+// (0..3: all but a few per mille) are counted in registers and folded once per warp at the end; the
+// angle takes a linear guess of its bin, corrected against the edges (exact for any edges), and a plain
+// run-length cached shared-memory atomic; lifetimes (complexes only) a binary search.
+constexpr int kHistUnroll = 2;
 __global__ void __launch_bounds__(256)
 histogram_kernel(const HistArgs a, const long long N)
 {
@@ -893,36 +902,113 @@ histogram_kernel(const HistArgs a, const long long N)
     for (int i = threadIdx.x; i <= a.nl; i += blockDim.x) s_le[i] = a.life_edges[i];
     for (int i = threadIdx.x; i < nbins_total; i += blockDim.x) s_angle[i] = 0u;
     __syncthreads();
+    const double e0 = s_ae[0];
+    const double span = s_ae[a.na] - e0;
+    const double scale = (span > 0.0 && span < 1.0e300) ? (double)a.na / span : 0.0;
 
-    unsigned long long sum_acc = 0, sum_rej = 0, n_cplx = 0, n_traj = 0;
+    unsigned long long sum_acc = 0, sum_rej = 0;
+    unsigned n_cplx = 0, n_traj = 0;
+    unsigned c_status[4] = {0u, 0u, 0u, 0u}, c_turn[4] = {0u, 0u, 0u, 0u};
+    const bool turn_regs = a.nt >= 4;
+    int run_bin = 0;
+    unsigned run_len = 0u;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
-        agg_inc(s_angle, bin_of(s_ae, a.na, a.angle[i]));
-        const bool cplx = a.complex_flag[i] != 0;
-        if (cplx) agg_inc(s_life, bin_of(s_le, a.nl, a.lifetime[i]));
-        const int nt = a.n_turn[i];
-        agg_inc(s_turn, nt < 0 ? 0 : (nt >= a.nt ? a.nt - 1 : nt));
-        agg_inc(s_status, a.status[i] & 3);
-        sum_acc += (unsigned long long)a.n_acc[i];
-        sum_rej += (unsigned long long)a.n_rej[i];
-        n_cplx += cplx ? 1u : 0u;
-        n_traj += 1u;
+    // software pipeline: the loads of the next kHistUnroll trajectories are in flight while the current ones
+    // are binned (the kernel is bound by memory latency, not by instructions)
+    struct Batch {
+        double ang[kHistUnroll], life[kHistUnroll];
+        int nt[kHistUnroll], st[kHistUnroll], na[kHistUnroll], nr[kHistUnroll];
+        unsigned char fl[kHistUnroll];
+    };
+    auto load = [&](Batch& B, long long i0) {
+#pragma unroll
+        for (int u = 0; u < kHistUnroll; ++u) {
+            const long long i = i0 + u * stride;
+            const bool in = i < N;
+            B.ang[u] = in ? __ldcs(a.angle + i) : 0.0;
+            B.life[u] = in ? __ldcs(a.lifetime + i) : 0.0;  // for every trajectory: a load behind the flag would expose its latency
+            B.fl[u] = in ? __ldcs(a.complex_flag + i) : (unsigned char)0;
+            B.nt[u] = in ? __ldcs(a.n_turn + i) : 0;
+            B.st[u] = in ? __ldcs(a.status + i) : 0;
+            B.na[u] = in ? __ldcs(a.n_acc + i) : 0;
+            B.nr[u] = in ? __ldcs(a.n_rej + i) : 0;
+        }
+    };
+    Batch cur, nxt;
+    long long i0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i0 < N) load(cur, i0);
+    for (; i0 < N; i0 += kHistUnroll * stride) {
+        const long long i_next = i0 + kHistUnroll * stride;
+        if (i_next < N) load(nxt, i_next);
+#pragma unroll
+        for (int u = 0; u < kHistUnroll; ++u) {
+            const long long i = i0 + u * stride;
+            if (i >= N) break;
+            const double v = cur.ang[u];
+            const double g = fmin(fmax((v - e0) * scale, -1.0), (double)a.na + 1.0);
+            const int ba = bin_from_guess(s_ae, a.na, v, (v == v) ? (int)g + 1 : 0);
+            // run-length cache: the angle distribution is sharply peaked (most atoms are barely deflected), so
+            // consecutive trajectories of a thread mostly hit the same bin: one atomic per run, not per trajectory
+            if (ba == run_bin) {
+                ++run_len;
+            } else {
+                if (run_len) atomicAdd(&s_angle[run_bin], run_len);
+                run_bin = ba;
+                run_len = 1u;
+            }
+            const bool cplx = cur.fl[u] != 0;
+            if (cplx) atomicAdd(&s_life[bin_of(s_le, a.nl, cur.life[u])], 1u);
+            const int b = cur.nt[u] < 0 ? 0 : (cur.nt[u] >= a.nt ? a.nt - 1 : cur.nt[u]);
+            if (turn_regs && b < 4) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) c_turn[k] += (b == k) ? 1u : 0u;
+            } else {
+                atomicAdd(&s_turn[b], 1u);
+            }
+            const int sb = cur.st[u] & 3;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) c_status[k] += (sb == k) ? 1u : 0u;
+            sum_acc += (unsigned long long)cur.na[u];
+            sum_rej += (unsigned long long)cur.nr[u];
+            n_cplx += cplx ? 1u : 0u;
+            n_traj += 1u;
+        }
+        cur = nxt;
     }
-    // totals: warp shuffle reduction, one global atomic per warp and quantity
+    // the last run of every thread, aggregated over the lanes that end in the same bin
+    const unsigned FULL = 0xffffffffu;
+    {
+        const unsigned grp = __match_any_sync(FULL, run_bin);
+        const unsigned tot = __reduce_add_sync(grp, run_len);
+        if ((threadIdx.x & 31) == __ffs(grp) - 1 && tot) atomicAdd(&s_angle[run_bin], tot);
+    }
+    // register counters: one reduction per warp, one shared-memory atomic per warp and value
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const unsigned cs = __reduce_add_sync(FULL, c_status[k]);
+        const unsigned ct = __reduce_add_sync(FULL, c_turn[k]);
+        if ((threadIdx.x & 31) == 0) {
+            if (cs) atomicAdd(&s_status[k], cs);
+            if (ct) atomicAdd(&s_turn[k], ct);
+        }
+    }
+    const unsigned w_cplx = __reduce_add_sync(FULL, n_cplx), w_traj = __reduce_add_sync(FULL, n_traj);
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
-        sum_acc += __shfl_down_sync(0xffffffffu, sum_acc, off);
-        sum_rej += __shfl_down_sync(0xffffffffu, sum_rej, off);
-        n_cplx += __shfl_down_sync(0xffffffffu, n_cplx, off);
-        n_traj += __shfl_down_sync(0xffffffffu, n_traj, off);
+        sum_acc += __shfl_down_sync(FULL, sum_acc, off);
+        sum_rej += __shfl_down_sync(FULL, sum_rej, off);
     }
+    __shared__ unsigned long long s_tot[4];
+    if (threadIdx.x < 4) s_tot[threadIdx.x] = 0ULL;
+    __syncthreads();
     if ((threadIdx.x & 31) == 0) {
-        if (sum_acc) atomicAdd(&a.h_totals[0], sum_acc);
-        if (sum_rej) atomicAdd(&a.h_totals[1], sum_rej);
-        if (n_cplx) atomicAdd(&a.h_totals[2], n_cplx);
-        if (n_traj) atomicAdd(&a.h_totals[3], n_traj);
+        if (sum_acc) atomicAdd(&s_tot[0], sum_acc);
+        if (sum_rej) atomicAdd(&s_tot[1], sum_rej);
+        if (w_cplx) atomicAdd(&s_tot[2], (unsigned long long)w_cplx);
+        if (w_traj) atomicAdd(&s_tot[3], (unsigned long long)w_traj);
     }
     __syncthreads();
+    if (threadIdx.x < 4 && s_tot[threadIdx.x]) atomicAdd(&a.h_totals[threadIdx.x], s_tot[threadIdx.x]);
     for (int i = threadIdx.x; i < a.na + 2; i += blockDim.x)
         if (s_angle[i]) atomicAdd(&a.h_angle[i], (unsigned long long)s_angle[i]);
     for (int i = threadIdx.x; i < a.nl + 2; i += blockDim.x)
@@ -1295,6 +1381,7 @@ struct SchedConfig {
     int plan = 1;             // 0: natural order
     double kappa = 1.5;       // candidates: b < kappa * Langevin radius
     int poll_iters = 32;      // six-lane warps with idle groups look for new slots every this many iterations
+    int hist_blocks_per_sm = 8;  // grid of histogram_kernel
 };
 
 std::mutex g_sched_mutex;
@@ -1560,7 +1647,8 @@ int aig_set_schedule_ex(const aig_schedule* s)
     }
     if (s->tail_iters < 0 || s->budget < 1 || s->split_sms < 1 || s->split_grid < 1 || !(s->kappa >= 0.0) ||
         s->depth < 1 || s->mean_factor < 0 || s->drain_lanes < 0 || s->drain_lanes > 32 || !(s->slow0 >= 0.0) ||
-        !(s->slow1 >= 0.0) || s->refill_batch < 1 || s->refill_batch > 32 || s->refill_wait < 0 || s->poll_iters < 1)
+        !(s->slow1 >= 0.0) || s->refill_batch < 1 || s->refill_batch > 32 || s->refill_wait < 0 || s->poll_iters < 1 ||
+        s->hist_blocks_per_sm < 1 || s->hist_blocks_per_sm > 64)
         return AIG_ERR_PARAM;
     g_sched.tail_iters = s->tail_iters;
     g_sched.budget = s->budget;
@@ -1576,6 +1664,7 @@ int aig_set_schedule_ex(const aig_schedule* s)
     g_sched.refill_batch = s->refill_batch;
     g_sched.refill_wait = s->refill_wait;
     g_sched.poll_iters = s->poll_iters;
+    g_sched.hist_blocks_per_sm = s->hist_blocks_per_sm;
     return AIG_OK;
 }
 
@@ -1597,6 +1686,7 @@ int aig_get_schedule(aig_schedule* s)
     s->refill_batch = c.refill_batch;
     s->refill_wait = c.refill_wait;
     s->poll_iters = c.poll_iters;
+    s->hist_blocks_per_sm = c.hist_blocks_per_sm;
     return AIG_OK;
 }
 
@@ -1728,8 +1818,12 @@ int aig_histogram(const aig_out* obs, int64_t N, const aig_hist_spec* spec, cons
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return AIG_ERR_CUDA;
     const size_t smem = sizeof(double) * (a.na + 1 + a.nl + 1) +
                         sizeof(unsigned) * ((a.na + 2) + (a.nl + 2) + a.nt + 4);
-    long long blocks = (N + 255) / 256;
-    const long long cap = (long long)sms * 8;
+    // up to 2048 bins each: 57 KB of dynamic shared memory, above the 48 KB a kernel gets without opting in
+    if (smem > 48 * 1024 &&
+        cudaFuncSetAttribute(histogram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return AIG_ERR_CUDA;
+    long long blocks = (N + 256 * kHistUnroll - 1) / (256 * kHistUnroll);
+    const long long cap = (long long)sms * sched_config().hist_blocks_per_sm;
     if (blocks > cap) blocks = cap;
     histogram_kernel<<<(unsigned)blocks, 256, smem, st>>>(a, N);
     g_kernel_launches++;
@@ -1842,6 +1936,7 @@ int aig_run_host(const aig_params* p, const double* y0_host, int64_t N, double t
     size_t hist_words = 0, edge_words = 0;
     if (hs) {
         if (hs->n_angle_bins < 1 || hs->n_life_bins < 1 || hs->n_turn_bins < 1) return AIG_ERR_SIZE;
+        if (hs->n_angle_bins > 2048 || hs->n_life_bins > 2048 || hs->n_turn_bins > 2048) return AIG_ERR_SIZE;
         if (!hs->angle_edges || !hs->life_edges) return AIG_ERR_NULL;
         hist_words = (size_t)(hs->n_angle_bins + 2) + (hs->n_life_bins + 2) + hs->n_turn_bins + 4 + 4;
         edge_words = (size_t)(hs->n_angle_bins + 1) + (hs->n_life_bins + 1);

@@ -296,6 +296,105 @@ def test_schedule_invariance(aig):
         aig.set_schedule(budget=0)
 
 
+def test_sanitizer_scenario(aig):
+    """Every kernel of the path on a small input with a schedule that exercises all queues (plan, tiny
+    budget, streaming and final six-lane pass, drain), then the reductions.  Also the command line of the
+    compute-sanitizer runs recorded in profiles/ (memcheck, racecheck, synccheck)."""
+    import torch
+    w = inputs.config(2).replace(N=8229)
+    y0 = inputs.generate_y0(w)
+    p = aig.make_params(**w.params())
+    y0d = _dev(y0)
+    ref = _host(aig.aig_integrate(p, y0d, w.t_max, w.rtol, w.atol, out=aig.alloc_out(w.N, "cuda", position=True)))
+    try:
+        aig.set_schedule(plan=1, budget=40, tail_iters=3, split_sms=5, mean_factor=0, depth=4, poll_iters=2)
+        out = aig.aig_integrate(p, y0d, w.t_max, w.rtol, w.atol, out=aig.alloc_out(w.N, "cuda", position=True))
+        g = _host(out)
+    finally:
+        aig.set_schedule()
+    for k in ref:
+        assert np.array_equal(ref[k].view(np.uint8), g[k].view(np.uint8)), k
+    ae, le = inputs.histogram_edges()
+    H = aig.hist_to_numpy(aig.aig_histogram(out, _dev(ae), _dev(le), 64))
+    want = orc.histogram(g, ae, le, 64)
+    for k in want:
+        assert np.array_equal(H[k], want[k]), k
+    extra = aig.aig_observables(p, y0d, out)
+    res = aig.aig_outliers(out, extra).cpu().numpy()
+    allobs = dict(g)
+    allobs.update({k: v.cpu().numpy() for k, v in extra.items()})
+    wo = orc.outliers(allobs)
+    for r, k in enumerate(aig.OUTLIER_KEYS):
+        assert (int(res[r, 0]), int(res[r, 1])) == wo[k], k
+    t, y, n = aig.aig_trace(p, y0d[:, 0].contiguous(), w.t_max, w.rtol, w.atol, cap=4096)
+    torch.cuda.synchronize()
+
+
+def test_guard_bands_no_out_of_bounds_write(aig):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds WRITES are looked for directly: every
+    buffer of a call (outputs, first-bounce record, workspace, histogram, observables, outlier scratch) is
+    carved out of one arena with 4 KiB guard bands of a sentinel pattern around it; after the whole path has
+    run with the all-queues schedule of test_sanitizer_scenario the guard bands must be untouched, for
+    several sizes including N = 1 and a size that is not a multiple of anything."""
+    import torch
+    GUARD = 4096
+
+    class Arena:
+        def __init__(self, nbytes):
+            self.buf = torch.full((nbytes,), 0xA5, dtype=torch.uint8, device="cuda")
+            self.pos = GUARD
+            self.spans = []
+
+        def take(self, shape, dtype):
+            n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+            start = (self.pos + 255) // 256 * 256
+            t = self.buf[start:start + n].view(dtype).view(*shape)
+            self.spans.append((start, start + n))
+            self.pos = start + n + GUARD
+            assert self.pos <= self.buf.numel()
+            return t
+
+        def check(self):
+            mask = torch.ones(self.buf.numel(), dtype=torch.bool, device="cuda")
+            for a, b in self.spans:
+                mask[a:b] = False
+            assert bool((self.buf[mask] == 0xA5).all()), "a guard band was written"
+
+    ae, le = inputs.histogram_edges()
+    for n in (1, 257, 8229):
+        w = inputs.config(2).replace(N=n)
+        y0 = inputs.generate_y0(w)
+        p = aig.make_params(**w.params())
+        ws_bytes = aig.workspace_bytes(n)
+        A = Arena(64 * GUARD + 400 * n + ws_bytes + 64 * 1024)
+        f64, i32 = torch.float64, torch.int32
+        y0d = A.take((12, n), f64)
+        y0d.copy_(torch.from_numpy(y0))
+        out = {"y_final": A.take((12, n), f64), "t_final": A.take((n,), f64), "lifetime": A.take((n,), f64),
+               "angle": A.take((n,), f64), "r_min": A.take((n,), f64), "n_acc": A.take((n,), i32),
+               "n_rej": A.take((n,), i32), "n_turn": A.take((n,), i32), "status": A.take((n,), i32),
+               "complex_flag": A.take((n,), torch.uint8), "x_turn1": A.take((3, n), f64)}
+        ws = A.take((ws_bytes,), torch.uint8)
+        try:
+            aig.set_schedule(plan=1, budget=40, tail_iters=3, split_sms=5, mean_factor=0, depth=4, poll_iters=2)
+            aig.aig_integrate(p, y0d, w.t_max, w.rtol, w.atol, out=out, workspace=ws)
+        finally:
+            aig.set_schedule()
+        aed, led = A.take((len(ae),), f64), A.take((len(le),), f64)
+        aed.copy_(torch.from_numpy(ae))
+        led.copy_(torch.from_numpy(le))
+        hist = {"angle": A.take((len(ae) + 1,), torch.int64), "lifetime": A.take((len(le) + 1,), torch.int64),
+                "n_turn": A.take((64,), torch.int64), "status": A.take((4,), torch.int64), "totals": A.take((4,), torch.int64)}
+        for v in hist.values():
+            v.zero_()
+        aig.aig_histogram(out, aed, led, 64, hist=hist)
+        extra = {k: A.take((n,), f64) for k in ("dist", "KE", "transfer", "position")}
+        aig.aig_observables(p, y0d, out, extra=extra)
+        torch.cuda.synchronize()
+        A.check()
+        assert int(hist["totals"][3].item()) == n and bool((out["status"] <= 1).all())
+
+
 def test_config1_two_body_physics(aig):
     """Trap off, N = 65,536: parity on a prefix + physics at full size."""
     w = inputs.config(1)
@@ -774,6 +873,20 @@ def test_histogram_exact(aig):
     H3 = aig.hist_to_numpy(aig.aig_histogram(dev, _dev(ae), _dev(le), 64))
     ref3 = orc.histogram(obs, ae, le, 64)
     assert all(np.array_equal(H3[k], ref3[k]) for k in ref3)
+    # the largest bin counts the ABI accepts (2048 each: more shared memory than a kernel gets by default),
+    # edges that are far from uniform (the angle's bin is found from a linear guess: exact for any edges),
+    # +-inf, fewer than four n_turn bins, and one more than the limit
+    ae2 = np.sort(np.concatenate([[-0.1], rng.uniform(0.0, 0.3, 1000), rng.uniform(3.0, 3.3, 1047), [3.5]]))
+    le2 = np.geomspace(1e3, 1e14, 2049)
+    assert len(ae2) == 2049 and np.all(np.diff(ae2) > 0)
+    obs["angle"][5:8] = [np.inf, -np.inf, ae2[1024]]
+    dev = {**dev, "angle": _dev(obs["angle"])}
+    for nt_bins in (2048, 3, 1):
+        H4 = aig.hist_to_numpy(aig.aig_histogram(dev, _dev(ae2), _dev(le2), nt_bins))
+        ref4 = orc.histogram(obs, ae2, le2, nt_bins)
+        assert all(np.array_equal(H4[k], ref4[k]) for k in ref4), nt_bins
+    with pytest.raises(Exception):
+        aig.aig_histogram(dev, _dev(np.linspace(0, 1, 2050)), _dev(le2), 64)
 
 
 def test_run_host_end_to_end(aig):
