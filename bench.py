@@ -473,6 +473,14 @@ def main() -> int:
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1:
+        # python bench.py --gpus N: become N ranks (one process per GPU) of this node
+        import torch
+        from paper_2509_12381_b200 import sharding
+        return sharding.launch_ranks(os.path.abspath(__file__), sys.argv[1:], args.gpus, torch.cuda.device_count())
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but launched with WORLD_SIZE={world_env}")
     return run_ours(args)
 
 

@@ -10,6 +10,11 @@ This module holds no arithmetic of the method and works on CPU tensors with the 
 """
 from __future__ import annotations
 
+import os
+import socket
+import subprocess
+import sys
+
 import numpy as np
 
 from . import inputs
@@ -79,3 +84,28 @@ def sum_over_ranks(x: int, device="cpu", group=None) -> int:
     t = torch.tensor([int(x)], dtype=torch.int64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
     return int(t.item())
+
+
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_ranks(script: str, script_args: list[str], n_ranks: int, n_devices: int, env: dict | None = None) -> int:
+    """One process per GPU ("distributed evenly across the ncores cores", one worker per GPU):
+    re-launch ``script`` as ``n_ranks`` ranks of one node through ``torch.distributed.run`` (rendezvous on
+    127.0.0.1, a free port) and return its exit code.  Fails loudly, without launching anything, when the node has
+    fewer devices than ranks: a run must never report fewer GPUs than it was asked for.  Rank r then owns the index
+    range ``shard_y0(..., r, n_ranks)`` of the seeded stream; only rank 0 prints."""
+    if n_ranks < 1:
+        raise SystemExit(f"--gpus {n_ranks}: need at least one rank")
+    if n_devices < n_ranks:
+        raise SystemExit(f"--gpus {n_ranks}: this node has only {n_devices} CUDA device(s); refusing to run "
+                         f"{n_ranks} ranks on fewer GPUs (no rank may share a device)")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_ranks}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), script, *script_args]
+    e = dict(os.environ if env is None else env)
+    e.setdefault("NCCL_DEBUG", "INFO")   # one "Init COMPLETE" line per rank on stderr: the ranks can be counted
+    e.setdefault("OMP_NUM_THREADS", "1")
+    return subprocess.call(cmd, env=e)

@@ -395,6 +395,49 @@ def test_guard_bands_no_out_of_bounds_write(aig):
         assert int(hist["totals"][3].item()) == n and bool((out["status"] <= 1).all())
 
 
+def test_concurrent_calls_two_threads(aig):
+    """include/aig.h: aig_integrate may be called from several host threads at once (own streams, outputs and
+    workspaces).  Two threads, two streams, one device, several calls each: every result byte-identical to
+    the same call made alone."""
+    import threading
+    import torch
+    w = inputs.config(2).replace(N=6000 + 11)
+    y0 = inputs.generate_y0(w)
+    p = aig.make_params(**w.params())
+    halves = [np.ascontiguousarray(y0[:, :3000]), np.ascontiguousarray(y0[:, 3000:])]
+    ref = [_host(aig.aig_integrate(p, _dev(h), w.t_max, w.rtol, w.atol)) for h in halves]
+    results, errors = [None, None], []
+
+    def work(k):
+        try:
+            torch.cuda.set_device(0)
+            stream = torch.cuda.Stream()
+            yd = _dev(halves[k])
+            n = halves[k].shape[1]
+            keep = []   # every buffer stays allocated until the stream has run
+            for _ in range(6):
+                out = aig.alloc_out(n, "cuda")
+                ws = torch.zeros(aig.workspace_bytes(n), dtype=torch.uint8, device="cuda")
+                stream.wait_stream(torch.cuda.current_stream())
+                keep.append(aig.aig_integrate(p, yd, w.t_max, w.rtol, w.atol, out=out, workspace=ws, stream=stream))
+            stream.synchronize()
+            for o in keep:   # all six calls, not only the last
+                g = {kk: v.cpu().numpy() for kk, v in o.items() if not kk.startswith("_")}
+                for key in ref[k]:
+                    assert np.array_equal(ref[k][key].view(np.uint8), g[key].view(np.uint8)), (k, key)
+            results[k] = g
+        except Exception as e:  # pragma: no cover
+            errors.append(e)
+
+    threads = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    [t.start() for t in threads]
+    [t.join() for t in threads]
+    assert not errors, errors
+    for k in range(2):
+        for key in ref[k]:
+            assert np.array_equal(ref[k][key].view(np.uint8), results[k][key].view(np.uint8)), (k, key)
+
+
 def test_config1_two_body_physics(aig):
     """Trap off, N = 65,536: parity on a prefix + physics at full size."""
     w = inputs.config(1)

@@ -114,3 +114,37 @@ def test_world_size_2_gloo(tmp_path, per_rank):
             assert np.array_equal(r["h_" + k].view(np.uint64), ref[k]), k
         assert int(r["h_totals"][3]) == n_all
         assert float(r["t_max"]) == float(world) and int(r["n_sum"]) == n_all
+
+
+def test_launch_ranks_refuses_more_ranks_than_devices():
+    # what `python bench.py --gpus 2` does on a node with fewer GPUs: fail loudly, launch nothing
+    with pytest.raises(SystemExit) as e:
+        sharding.launch_ranks("unused.py", [], 2, 1)
+    assert "only 1 CUDA device" in str(e.value)
+    with pytest.raises(SystemExit):
+        sharding.launch_ranks("unused.py", [], 8, 0)
+
+
+def test_bench_gpus_2_fails_loudly_without_two_gpus():
+    import subprocess
+    import torch
+    if torch.cuda.device_count() >= 2:
+        pytest.skip("needs a node with fewer than two GPUs")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0"],
+                       capture_output=True, text=True, env={k: v for k, v in os.environ.items() if k != "WORLD_SIZE"})
+    assert r.returncode != 0 and "--gpus 2" in r.stderr and "n_gpus" not in r.stdout
+
+
+def test_launch_ranks_gloo(capfd):
+    """The spawn path of `bench.py --gpus N` (sharding.launch_ranks -> torch.distributed.run -> one process per
+    rank), driven with a CPU rank program over gloo: two ranks, each owns 96 trajectories of the stream."""
+    import json
+    here = os.path.dirname(os.path.abspath(__file__))
+    rc = sharding.launch_ranks(os.path.join(here, "gloo_rank_worker.py"), ["96"], 2, 2)
+    assert rc == 0
+    out = capfd.readouterr().out
+    line = json.loads([l for l in out.splitlines() if l.startswith("{")][-1])
+    w = inputs.config(0)
+    want = sum(int(abs(sharding.shard_y0(w, r, 2, per_rank=96)[0]).sum() * 1e6) for r in range(2))
+    assert line == {"n_gpus": 2, "trajectories": 192, "max_over_ranks": 2.0, "checksum": want}
