@@ -225,7 +225,7 @@ uint64_t aig_kernel_launches(void);
  *               queue ran dry before it hands its trajectories over (default 256)
  *   budget      accepted steps after which a trajectory is offered to the six-lane integrator
  *               (default 2048)
- *   split_sms   SMs the six-lane pass owns while the bulk pass runs beside it (16)
+ *   split_sms   SMs the six-lane pass owns while the bulk pass runs beside it (12)
  *   split_grid  one-warp blocks per SM of the final six-lane pass (8)
  *   plan        0: natural order; 1: three classes, slow capture candidates first (default)
  *   kappa       candidates are trajectories with impact parameter < kappa Langevin radii (1.5)

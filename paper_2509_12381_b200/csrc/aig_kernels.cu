@@ -638,44 +638,47 @@ __device__ __forceinline__ double rel_speed2(const double* __restrict__ y0, long
 __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long long N, long long i, const PlanArgs& A,
                                           double mean_u2)
 {
-    double xi[3], vi[3], xa[3], va[3];
+    // single precision throughout: a scheduling estimate (positions ~1e3 a0 to 1e-4 a0, far below the ~1e2 a0
+    // it decides on), on the FP32 pipes instead of the FP64 pipe the integrators need
+    float xi[3], vi[3], xa[3], va[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        xi[k] = y0[(0 + k) * N + i];
-        vi[k] = y0[(3 + k) * N + i];
-        xa[k] = y0[(6 + k) * N + i];
-        va[k] = y0[(9 + k) * N + i];
+        xi[k] = (float)y0[(0 + k) * N + i];
+        vi[k] = (float)y0[(3 + k) * N + i];
+        xa[k] = (float)y0[(6 + k) * N + i];
+        va[k] = (float)y0[(9 + k) * N + i];
     }
-    const double d0 = xa[0] - xi[0], d1 = xa[1] - xi[1], d2 = xa[2] - xi[2];
-    const double u0 = va[0] - vi[0], u1 = va[1] - vi[1], u2 = va[2] - vi[2];
-    const double usq = u0 * u0 + u1 * u1 + u2 * u2;
-    const double dsq = d0 * d0 + d1 * d1 + d2 * d2;
+    const float d0 = xa[0] - xi[0], d1 = xa[1] - xi[1], d2 = xa[2] - xi[2];
+    const float u0 = va[0] - vi[0], u1 = va[1] - vi[1], u2 = va[2] - vi[2];
+    const float usq = u0 * u0 + u1 * u1 + u2 * u2;
+    const float dsq = d0 * d0 + d1 * d1 + d2 * d2;
     // fly-by window: twice the time to cover the initial distance, within the time span
-    double T = A.span;
-    if (usq > 0.0) T = fmin(T, 2.0 * sqrt(dsq / usq));
-    const double dt = T / kPlanSamples;
+    float T = (float)A.span;
+    if (usq > 0.0f) T = fminf(T, 2.0f * sqrtf(dsq / usq));
+    const float dt = T / kPlanSamples;
     // ion on its secular orbit, by the rotation recurrence: (c, s)_j = (cos, sin)(w_k j dt); free axes move linearly
-    double c[3], sn[3], cd[3], sd[3], amp[3];
+    float c[3], sn[3], cd[3], sd[3], amp[3], w[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        c[k] = 1.0;
-        sn[k] = 0.0;
-        sincos(A.w[k] * dt, &sd[k], &cd[k]);
-        amp[k] = A.w[k] > 0.0 ? vi[k] / A.w[k] : 0.0;
+        w[k] = (float)A.w[k];
+        c[k] = 1.0f;
+        sn[k] = 0.0f;
+        sincosf(w[k] * dt, &sd[k], &cd[k]);
+        amp[k] = w[k] > 0.0f ? vi[k] / w[k] : 0.0f;
     }
-    double f_prev = dsq, f_best = dsq, f_before = dsq, f_after = dsq;
+    float f_prev = dsq, f_best = dsq, f_before = dsq, f_after = dsq;
     int j_best = 0;
     bool want_after = true;
     for (int j = 1; j <= kPlanSamples; ++j) {
-        const double t = dt * j;
-        double f = 0.0;
+        const float t = dt * j;
+        float f = 0.0f;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const double cn = c[k] * cd[k] - sn[k] * sd[k];
+            const float cn = c[k] * cd[k] - sn[k] * sd[k];
             sn[k] = sn[k] * cd[k] + c[k] * sd[k];
             c[k] = cn;
-            const double xk = A.w[k] > 0.0 ? xi[k] * c[k] + amp[k] * sn[k] : xi[k] + vi[k] * t;
-            const double dk = xa[k] + va[k] * t - xk;
+            const float xk = w[k] > 0.0f ? xi[k] * c[k] + amp[k] * sn[k] : xi[k] + vi[k] * t;
+            const float dk = xa[k] + va[k] * t - xk;
             f += dk * dk;
         }
         if (want_after) {
@@ -692,28 +695,28 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
         f_prev = f;
     }
     // parabola through the best sample and its neighbours
-    const double den = f_before - 2.0 * f_best + f_after;
-    double off = 0.0;
-    if (den > 0.0 && j_best > 0 && j_best < kPlanSamples) off = fmin(fmax(0.5 * (f_before - f_after) / den, -1.0), 1.0);
-    const double dmin2 = fmax(f_best - 0.25 * (f_before - f_after) * off, 0.0);
-    const double ts = dt * (j_best + off);
+    const float den = f_before - 2.0f * f_best + f_after;
+    float off = 0.0f;
+    if (den > 0.0f && j_best > 0 && j_best < kPlanSamples) off = fminf(fmaxf(0.5f * (f_before - f_after) / den, -1.0f), 1.0f);
+    const float dmin2 = fmaxf(f_best - 0.25f * (f_before - f_after) * off, 0.0f);
+    const float ts = dt * (j_best + off);
     // relative speed and micromotion amplitude at the closest approach
-    double urel2 = 0.0, mm = 0.0;
+    float urel2 = 0.0f, mm = 0.0f;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        double sk, ck;
-        sincos(A.w[k] * ts, &sk, &ck);
-        const double xk = A.w[k] > 0.0 ? xi[k] * ck + amp[k] * sk : xi[k] + vi[k] * ts;
-        const double vk = A.w[k] > 0.0 ? vi[k] * ck - xi[k] * A.w[k] * sk : vi[k];
-        const double uk = va[k] - vk;
+        float sk, ck;
+        sincosf(w[k] * ts, &sk, &ck);
+        const float xk = w[k] > 0.0f ? xi[k] * ck + amp[k] * sk : xi[k] + vi[k] * ts;
+        const float vk = w[k] > 0.0f ? vi[k] * ck - xi[k] * w[k] * sk : vi[k];
+        const float uk = va[k] - vk;
         urel2 += uk * uk;
-        mm = fmax(mm, A.hq[k] * fabs(xk));
+        mm = fmaxf(mm, (float)A.hq[k] * fabsf(xk));
     }
     // b_c = (8 C4 / (mu u^2))^(1/4)
-    const double bc = urel2 > 0.0 ? sqrt(sqrt(8.0 * A.c4 / (A.mu * urel2))) : 1.0e300;
-    const bool cand = sqrt(dmin2) < A.kappa * bc + mm;
-    if (cand && usq < A.slow0 * mean_u2) return 0;
-    if (cand || usq < A.slow1 * mean_u2) return 1;
+    const float bc = urel2 > 0.0f ? sqrtf(sqrtf((float)(8.0 * A.c4 / A.mu) / urel2)) : 3.0e38f;
+    const bool cand = sqrtf(dmin2) < (float)A.kappa * bc + mm;
+    if (cand && usq < (float)(A.slow0 * mean_u2)) return 0;
+    if (cand || usq < (float)(A.slow1 * mean_u2)) return 1;
     return 2;
 }
 
@@ -1369,7 +1372,7 @@ constexpr long long kMinSlots = 1 << 20;
 struct SchedConfig {
     int tail_iters = 256;     // iterations a warp keeps stepping after the queue ran dry
     int budget = 2048;        // accepted steps after which the per-thread integrator offers a trajectory
-    int split_sms = 16;       // SMs the streaming six-lane pass takes for itself (one 8-warp block each)
+    int split_sms = 12;       // SMs the streaming six-lane pass takes for itself (one 8-warp block each)
     int split_grid_b = 8;     // final six-lane pass: one-warp blocks per SM (it has the GPU to itself)
     int depth = 64;           // budget hand-overs stop while this many published slots wait to be taken
     int mean_factor = 4;      // ... and are only for trajectories this many times longer than the finished ones' mean
