@@ -112,7 +112,7 @@ typedef struct aig_hist {
     uint64_t *angle, *lifetime, *n_turn, *status, *totals;
 } aig_hist;
 
-/* Bytes of DEVICE scratch aig_integrate needs for N trajectories: 64 uint64 counters (work
+/* Bytes of DEVICE scratch aig_integrate needs for N trajectories: 256 uint64 counters (work
  * queues, slot counts, a stage timeline), the work-queue order (one int64 and one class byte per trajectory) and
  * min(N, max(2^20, N/4)) checkpoint slots of 216 B for suspended trajectories. */
 size_t aig_workspace_bytes(int64_t N);

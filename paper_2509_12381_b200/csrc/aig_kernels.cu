@@ -610,14 +610,20 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
 //     survive until t_max are low-energy ones (of the 12 longest trajectories of the bench
 //     workload all have u^2 < <u^2>/2; measured).
 // Three classes, queued in this order:
-//     0: candidates with u^2 < <u^2>/2   1: the other candidates, and anything with u^2 < <u^2>/10
+//     0: candidates with u^2 < <u^2>/2, and anything with u^2 < <u^2>/10   1: the other candidates
 //     2: the rest
 // so that the longest trajectories start early -- and reach the six-lane integrator a few milliseconds
 // later -- instead of anywhere.  Affects scheduling only, never a result.
-constexpr int kCntClass = 24;    // counters: trajectories per class (3)
-constexpr int kCntCursor = 28;   // counters: placement cursors (3)
+constexpr int kCntClass = 24;    // counters: trajectories per class (3; diagnostics)
 constexpr int kCntMeanU2 = 60;   // counters: <u^2> (double bits)
 constexpr int kPlanSamples = 64;
+// Inside a class the queue is ordered by slowness as well: kPlanSub buckets of u^2 / <u^2>, 1/8 wide, the
+// slowest first (the long trajectories of EVERY class are its slow ones, the unpredicted ones of class 2 too).
+// Bucket = class * kPlanSub + sub; their counts and placement cursors sit behind the first 64 counters.
+constexpr int kPlanSub = 16;
+constexpr int kPlanBuckets = 3 * kPlanSub;
+constexpr int kCntBucket = 64;                  // counters: trajectories per bucket
+constexpr int kCntCursor = 64 + kPlanBuckets;   // counters: placement cursors
 
 struct PlanArgs {
     double mu, c4;        // reduced mass, C4
@@ -715,9 +721,10 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
     // b_c = (8 C4 / (mu u^2))^(1/4)
     const float bc = urel2 > 0.0f ? sqrtf(sqrtf((float)(8.0 * A.c4 / A.mu) / urel2)) : 3.0e38f;
     const bool cand = sqrtf(dmin2) < (float)A.kappa * bc + mm;
-    if (cand && usq < (float)(A.slow0 * mean_u2)) return 0;
-    if (cand || usq < (float)(A.slow1 * mean_u2)) return 1;
-    return 2;
+    const float r = usq / (float)mean_u2;
+    const int cls = ((cand && r < (float)A.slow0) || r < (float)A.slow1) ? 0 : (cand ? 1 : 2);
+    const int sub = (int)fminf(8.0f * r, (float)(kPlanSub - 1));
+    return cls * kPlanSub + sub;
 }
 
 // <u^2> over the first min(N, 65536) trajectories (a sample is enough for a scheduling threshold)
@@ -755,29 +762,30 @@ plan_kernel(const double* __restrict__ y0, const long long N, const PlanArgs A, 
             cls_of[i] = (unsigned char)cls;
         }
     }
+    // lanes of the same bucket: one atomic per bucket and warp
     const int lane = threadIdx.x & 31;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const unsigned m = __ballot_sync(FULL, cls == c);
-        if (m == 0u) continue;
+    const unsigned m = __match_any_sync(FULL, cls);
+    if (cls >= 0) {
+        const int leader = __ffs(m) - 1;
         unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(&counters[(PLACE ? kCntCursor : kCntClass) + c], (unsigned long long)__popc(m));
+        if (lane == leader) base = atomicAdd(&counters[(PLACE ? kCntCursor : kCntBucket) + cls], (unsigned long long)__popc(m));
         if (PLACE) {
-            base = __shfl_sync(FULL, base, 0);
-            if (cls == c) order[base + __popc(m & ((1u << lane) - 1u))] = i;
+            base = __shfl_sync(m, base, leader);
+            order[base + __popc(m & ((1u << lane) - 1u))] = i;
         }
     }
 }
 
-// cursors at the class starts; bound[0], bound[1] = the whole of order[] (one bulk pass over the
-// class-ordered queue)
+// cursors at the bucket starts; bound[0], bound[1] = the whole of order[] (one bulk pass over the ordered queue)
 __global__ void plan_bounds_kernel(unsigned long long* counters, int bound0, int front)
 {
     unsigned long long acc = 0;
-    for (int c = 0; c < 3; ++c) {
-        counters[kCntCursor + c] = acc;
-        acc += counters[kCntClass + c];
-        if (c == 1) counters[front] = acc;  // classes 0 and 1 (diagnostics)
+    for (int b = 0; b < kPlanBuckets; ++b) {
+        counters[kCntCursor + b] = acc;
+        const unsigned long long n = counters[kCntBucket + b];
+        acc += n;
+        counters[kCntClass + b / kPlanSub] += n;
+        if (b == 2 * kPlanSub - 1) counters[front] = acc;  // classes 0 and 1 (diagnostics)
     }
     counters[bound0] = 0;
     counters[bound0 + 1] = acc;
@@ -1400,8 +1408,8 @@ long long slot_capacity(long long N) { return std::min(N < 1 ? 1 : N, std::max(k
 
 size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// workspace: 64 uint64 counters | order[N] (int64) | class[N] (uint8) | checkpoint slots
-constexpr size_t kCounterBytes = 64 * sizeof(unsigned long long);
+// workspace: 256 uint64 counters (64 of the schedule + the plan's buckets) | order[N] (int64) | bucket[N] (uint8) | checkpoint slots
+constexpr size_t kCounterBytes = 256 * sizeof(unsigned long long);
 size_t order_bytes(long long N) { return round_up((size_t)(N < 1 ? 1 : N) * sizeof(long long), 256); }
 size_t class_bytes(long long N) { return round_up((size_t)(N < 1 ? 1 : N), 256); }
 size_t ckpt_buffer_bytes(long long cap) { return round_up((size_t)cap * kCkptBytesPerSlot, 256); }
