@@ -1484,7 +1484,7 @@ SideStream* side_stream()   // call with g_enqueue_mutex held
 
 constexpr int kSplitMinBlocks = 8;  // register cap of the split kernel: 65536 / (8 x 32) = 256
 #ifndef AIG_SPLIT_WARPS
-#define AIG_SPLIT_WARPS 8
+#define AIG_SPLIT_WARPS 4
 #endif
 constexpr int kSplitWarps = AIG_SPLIT_WARPS;  // warps per block of the SM-owning variant: two per scheduler (a warp issues a third of the
                                               // time, so two barely slow each other while the queue is long; at the end each is alone)
