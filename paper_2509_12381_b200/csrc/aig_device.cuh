@@ -12,12 +12,15 @@
 //     branch-free (own reciprocal and cos), so the scheduler interleaves the two chains of a
 //     level: FP64 latency is 8 cycles at 2 cycles issue per warp on sm_100a, a lone dependent
 //     chain leaves 3/4 of the pipe idle;
+//   * the relative position d = x_ion - x_atom has a stage chain of its own (the r^-9 wall would see
+//     the rounding of a difference of two lab-frame positions): "Stage positions" below;
 //   * (dV/dr)/r = 4 C4/r^6 - 8 C8/r^10 needs even powers of r only: no square root;
-//     1/r^2 = MUFU.RCP64H seed + one cubic and one Newton correction (no slow-path branch);
+//     1/r^2 = MUFU.RCP64H seed + one cubic correction (three FMAs, no slow-path branch);
 //   * cos(Omega t): Cody-Waite reduction + Taylor kernel (trig_constants.inc), five per attempt
 //     (c6 = c7 = 1 share one, k1 is FSAL), all issued up front;
 //   * the error norm is a maximum of ratios found by cross-multiplication in a fixed binary
-//     tree and divided once; the controller's fifth root is a float seed + one cubic correction.
+//     tree and divided once; the controller's fifth root is a float seed + one Newton-type correction
+//     folded into the new step size (grow_step).
 // Every product-sum is an explicit fma() and the library is compiled with -fmad=false, so the
 // arithmetic of a trajectory does not depend on which kernel executes it: the per-thread
 // integrator below and the six-lanes-per-trajectory one (aig_split.cuh) call the same scalar
@@ -356,8 +359,8 @@ struct Traj {
 };
 
 // The rarely touched part of a trajectory's state (observables and counters).  The per-thread
-// integrator keeps it in shared memory (ColdShared in aig_kernels.cu: one slot per thread, SoA)
-// to stay within 168 registers at three blocks per SM; ColdRegs is the same thing in registers.
+// integrator keeps it in shared memory (ColdShared in aig_kernels.cu: one slot per thread, SoA:
+// it runs at 246 registers, two blocks of 128 threads per SM); ColdRegs is the same thing in registers.
 struct ColdRegs {
     static constexpr bool kInRegisters = true;
     double rmin2_, t_first_, t_last_;
