@@ -114,7 +114,7 @@ typedef struct aig_hist {
 
 /* Bytes of DEVICE scratch aig_integrate needs for N trajectories: 256 uint64 counters (work
  * queues, slot counts, a stage timeline), the work-queue order (one int64 and one class byte per trajectory) and
- * min(N, max(2^20, N/4)) checkpoint slots of 216 B for suspended trajectories. */
+ * min(N, max(2^20, N/4)) checkpoint slots of 224 B for suspended trajectories. */
 size_t aig_workspace_bytes(int64_t N);
 
 /* Integrate N trajectories from t0 to the first stop (exit radius, t_max, max_steps).

@@ -316,6 +316,7 @@ __device__ __forceinline__ void step_end_begin(const KParams& P, double x, doubl
     S.mv = dmax(fabs(v), P.thr);
     S.mx = dmax(fabs(x), P.thr);
 }
+
 // returns v_new and the two norm candidates |e_v| / max(|v|,|v_new|,thr), |e_x| / max(|x|,|x_new|,thr)
 __device__ __forceinline__ double step_end_finish(const StepEndPart& S, double h, double xn, double v, double A6,
                                                   double A7, Ratio& cv, Ratio& cx)
@@ -409,7 +410,6 @@ template <int TRAP>
 __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, Attempt& R)
 {
     const double h = T.c.h;
-    const double h2 = h * h;
     const double t_new = (T.c.flags & kLast) ? P.t_max : T.c.t + h;
 
     // A[i][l]: acceleration component i (0-2 ion, 3-5 atom) of stage l+1
@@ -427,6 +427,11 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
     // three levels; the two stages of a level are independent of each other
 #pragma unroll
     for (int lev = 0; lev < 3; ++lev) {
+        // h^2 is formed again at every level (the same product, the same bits) instead of living in a register
+        // pair through the force evaluations in between: the kernel runs at the register count that allows three
+        // blocks per SM, without a spill
+        double h2;
+        asm volatile("mul.f64 %0, %1, %1;" : "=d"(h2) : "d"(h));
         // cos(Omega t) at the stage times of this level (independent of the positions; c6 = c7 = 1)
         double cs[2];
         cs[0] = trap_cos<TRAP>(P, (lev == 2) ? t_new : fma(kC[2 * lev + 1], h, T.c.t));
@@ -466,21 +471,27 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
             for (int i = 0; i < 6; ++i) A[i][s] = a[i];
         }
     }
-    // stage 7 position = the 5th-order solution x_new; A[.][6] = f(t_new, ynew)
-    Ratio cv[6], cx[6];
+    // stage 7 position = the 5th-order solution x_new; A[.][6] = f(t_new, ynew).  Axis by axis (ion and atom
+    // component of the axis, then its quotient at once: eight norm candidates live instead of twenty-four)
+    double q[3];
 #pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        R.X[i] = (i < 3) ? Xis[1][i] : Xa_new[i - 3];
-        StepEndPart S;
-        step_end_begin(P, T.X[i], T.V[i], A[i], S);
-        R.V[i] = step_end_finish(S, h, R.X[i], T.V[i], A[i][5], A[i][6], cv[i], cx[i]);
-        R.A7[i] = A[i][6];
+    for (int k = 0; k < 3; ++k) {
+        Ratio cv[2], cx[2];
+#pragma unroll
+        for (int pa = 0; pa < 2; ++pa) {
+            const int i = k + 3 * pa;
+            R.X[i] = pa ? Xa_new[k] : Xis[1][k];
+            StepEndPart S;
+            step_end_begin(P, T.X[i], T.V[i], A[i], S);
+            R.V[i] = step_end_finish(S, h, R.X[i], T.V[i], A[i][5], A[i][6], cv[pa], cx[pa]);
+            R.A7[i] = A[i][6];
+        }
+        q[k] = axis_quotient(cv[0], cx[0], cv[1], cx[1]);
     }
     R.s = radial_s(R.X, R.V);
     R.r2 = r2[1];
     R.t_new = t_new;
-    R.err = error_estimate(h, axis_quotient(cv[0], cx[0], cv[3], cx[3]), axis_quotient(cv[1], cx[1], cv[4], cx[4]),
-                           axis_quotient(cv[2], cx[2], cv[5], cx[5]), R.r2, R.s);
+    R.err = error_estimate(h, q[0], q[1], q[2], R.r2, R.s);
 }
 
 // Times of one attempt that depend on (t, h) only: the split kernel forms them while the stages

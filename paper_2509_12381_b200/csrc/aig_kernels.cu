@@ -36,7 +36,7 @@ namespace aig {
 #define AIG_BLOCK 128
 #endif
 #ifndef AIG_MIN_BLOCKS
-#define AIG_MIN_BLOCKS 2
+#define AIG_MIN_BLOCKS 3
 #endif
 #ifndef AIG_SPLIT_UNROLL
 #define AIG_SPLIT_UNROLL 2
@@ -73,19 +73,33 @@ struct OutPtrs {
 // ------------------------------------------------------------------------------------------
 // integrator
 // ------------------------------------------------------------------------------------------
-// Cold state of the per-thread integrator: one shared-memory slot per thread, SoA (conflict-free).
+// Cold state of the per-thread integrator: shared memory, one 8-byte slot per thread and row, every row
+// at a compile-time offset from ONE per-thread address (a separate array each would cost an address
+// register each: the kernel runs at the 168 registers that allow three blocks per SM).
+//   rows: 0 r_min^2, 1 t_first, 2 t_last, 3 (n_rej, n_turn), 4-6 initial atom velocity, 7 trajectory index,
+//         8 (accepted steps at which the trajectory is offered next, iterations an idle lane of the warp has waited),
+//         9 (iterations since the queue was seen empty, stop status of a finished trajectory not stored yet),
+//         10 the radial observable s(t) between two steps (Core::sprev: read and written once per step),
+//         11 (accepted steps, flags) between two steps (Core::n_acc, Core::flags: likewise)
+constexpr int kColdRows = 12;
+template <int BLOCK>
 struct ColdShared {
     static constexpr bool kInRegisters = false;
-    __device__ __forceinline__ double& rmin2() { return s_rmin2[threadIdx.x]; }
-    __device__ __forceinline__ double& t_first() { return s_tfirst[threadIdx.x]; }
-    __device__ __forceinline__ double& t_last() { return s_tlast[threadIdx.x]; }
-    __device__ __forceinline__ int& n_rej() { return s_nrej[threadIdx.x]; }
-    __device__ __forceinline__ int& n_turn() { return s_nturn[threadIdx.x]; }
-    double* s_rmin2;
-    double* s_tfirst;
-    double* s_tlast;
-    int* s_nrej;
-    int* s_nturn;
+    double* b;  // row 0 of this thread
+    __device__ __forceinline__ double& rmin2() { return b[0 * BLOCK]; }
+    __device__ __forceinline__ double& t_first() { return b[1 * BLOCK]; }
+    __device__ __forceinline__ double& t_last() { return b[2 * BLOCK]; }
+    __device__ __forceinline__ int& n_rej() { return reinterpret_cast<int*>(b + 3 * BLOCK)[0]; }
+    __device__ __forceinline__ int& n_turn() { return reinterpret_cast<int*>(b + 3 * BLOCK)[1]; }
+    __device__ __forceinline__ double& v0(int k) { return b[(4 + k) * BLOCK]; }
+    __device__ __forceinline__ long long& idx() { return *reinterpret_cast<long long*>(b + 7 * BLOCK); }
+    __device__ __forceinline__ int& stop_at() { return reinterpret_cast<int*>(b + 8 * BLOCK)[0]; }
+    __device__ __forceinline__ int& waited() { return reinterpret_cast<int*>(b + 8 * BLOCK)[1]; }
+    __device__ __forceinline__ int& since_dry() { return reinterpret_cast<int*>(b + 9 * BLOCK)[0]; }
+    __device__ __forceinline__ int& pending() { return reinterpret_cast<int*>(b + 9 * BLOCK)[1]; }
+    __device__ __forceinline__ double& sprev() { return b[10 * BLOCK]; }
+    __device__ __forceinline__ volatile int& n_acc() { return reinterpret_cast<volatile int*>(b + 11 * BLOCK)[0]; }
+    __device__ __forceinline__ volatile int& flags() { return reinterpret_cast<volatile int*>(b + 11 * BLOCK)[1]; }
 };
 
 template <int TRAP, class Cold>
@@ -139,14 +153,15 @@ __device__ __forceinline__ void store_traj(const double (&v0)[3], long long N, l
 // Checkpoint slots: the full state of a suspended trajectory, SoA over `cap` slots
 // (d: 24 doubles per slot, i: 4 ints, idx: the trajectory's global index).
 //   d rows: 0-2 x_ion, 3-5 x_atom, 6-8 v_ion, 9-11 v_atom, 12-14 a_ion, 15-17 a_atom (FSAL),
-//           18 t, 19 h, 20 s(t), 21 r_min^2, 22 t_first, 23 t_last;  i rows: n_acc, flags, n_rej, n_turn
+//           18 t, 19 h, 20 s(t), 21 r_min^2, 22 t_first, 23 t_last;  i rows: n_acc, flags, n_rej, n_turn,
+//           time of the hand-over (two rows; diagnostics)
 struct Ckpt {
     double* d;
     int* i;
     long long* idx;
     long long cap;
 };
-constexpr int kCkptDoubles = 24, kCkptInts = 4;
+constexpr int kCkptDoubles = 24, kCkptInts = 6;  // i rows 4, 5: %globaltimer of the hand-over (diagnostics)
 constexpr size_t kCkptBytesPerSlot = kCkptDoubles * 8 + kCkptInts * 4 + 8;
 
 __device__ __forceinline__ unsigned long long ld_volatile(const unsigned long long* p)
@@ -179,6 +194,9 @@ __device__ __forceinline__ void ckpt_store(const Ckpt& K, long long slot, long l
     q[1 * cap] = (int)T.c.flags;
     q[2 * cap] = C.n_rej();
     q[3 * cap] = C.n_turn();
+    const unsigned long long now = global_ns();
+    q[4 * cap] = (int)(unsigned)(now & 0xffffffffULL);
+    q[5 * cap] = (int)(unsigned)(now >> 32);
     __threadfence();
     *(volatile long long*)(K.idx + slot) = idx;
 }
@@ -242,56 +260,64 @@ struct Sched {
     unsigned long long* timeline;
 };
 
+#ifdef AIG_MAXNREG
+#define AIG_BULK_BOUNDS __maxnreg__(AIG_MAXNREG)
+#else
+#define AIG_BULK_BOUNDS __launch_bounds__(BLOCK, MINB)
+#endif
 template <int TRAP, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB)
+__global__ void AIG_BULK_BOUNDS
 integrate_kernel(const KParams P, const double* __restrict__ y0, const long long N, const OutPtrs O,
                  const Sched S)
 {
-    __shared__ double s_rmin2[BLOCK], s_tfirst[BLOCK], s_tlast[BLOCK];
-    __shared__ double s_v0[3][BLOCK];  // initial atom velocity (for the scattering angle at the end)
-    __shared__ int s_nrej[BLOCK], s_nturn[BLOCK];
-    ColdShared C{s_rmin2, s_tfirst, s_tlast, s_nrej, s_nturn};
+    __shared__ double s_cold[kColdRows][BLOCK];
+    ColdShared<BLOCK> C{&s_cold[0][threadIdx.x]};
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const long long first = (long long)*S.begin;
-    const long long total = (long long)*S.end - first;
+    // the queue's range: block-wide constants of the refill code only, kept out of the registers
+    __shared__ long long s_range[2];
+    if (threadIdx.x == 0) {
+        s_range[0] = (long long)*S.begin;
+        s_range[1] = (long long)*S.end - s_range[0];
+    }
+    __syncthreads();
     if (blockIdx.x == 0 && threadIdx.x == 0) *(volatile unsigned long long*)S.started = 1ULL;
     Traj T;
-    long long idx = -1;
-    int stop_at = 0;      // suspend when n_acc reaches this
-    int since_dry = 0;    // warp-uniform: iterations since the queue was seen empty
+    C.idx() = -1;
+    C.waited() = 0;     // warp-uniform: iterations since a lane of this warp went idle
+    C.since_dry() = 0;  // warp-uniform: iterations since the queue was seen empty
+    C.pending() = -1;   // stop status of a finished trajectory whose results are not stored yet
     bool live = false;
     bool dry = false;     // warp-uniform: the queue has been seen empty
     bool may_suspend = true;
-    int pending = -1;     // stop status of a finished trajectory whose results are not stored yet
-    int waited = 0;       // warp-uniform: iterations since a lane of this warp went idle
     stage_begin(S.timeline);
 
     for (;;) {
         // ---- service: lanes without a trajectory store what they finished and take the next items
         //      of the queue.  The whole warp walks through this code (atan2 / sqrt of the end, global
         //      loads and the twelve divisions of the start) whenever one lane needs it, so idle lanes
-        //      are served in batches: when refill_batch of them wait, or one has waited refill_wait
+        //      are served in batches: when refill_batch of them wait, or one has C.waited() refill_wait
         //      iterations, or the queue is empty.
         const unsigned need = __ballot_sync(FULL, !live);
-        if (need && (__popc(need) >= S.refill_batch || waited >= S.refill_wait || dry)) {
-            waited = 0;
+        if (need && (__popc(need) >= S.refill_batch || C.waited() >= S.refill_wait || dry)) {
+            C.waited() = 0;
             {   // accepted steps and count of what this warp has finished since its last service
-                const unsigned fm = __ballot_sync(FULL, pending >= 0);
+                const unsigned fm = __ballot_sync(FULL, C.pending() >= 0);
                 if (fm) {
-                    const unsigned steps = __reduce_add_sync(FULL, pending >= 0 ? (unsigned)T.c.n_acc : 0u);
+                    const unsigned steps = __reduce_add_sync(FULL, C.pending() >= 0 ? (unsigned)T.c.n_acc : 0u);
                     if (lane == 0) {
                         atomicAdd(S.stats + 0, (unsigned long long)steps);
                         atomicAdd(S.stats + 1, (unsigned long long)__popc(fm));
                     }
                 }
             }
-            if (pending >= 0) {
-                const double v0[3] = {s_v0[0][threadIdx.x], s_v0[1][threadIdx.x], s_v0[2][threadIdx.x]};
-                store_traj(v0, N, idx, T, C, pending, O);
-                pending = -1;
+            if (C.pending() >= 0) {
+                const double v0[3] = {C.v0(0), C.v0(1), C.v0(2)};
+                store_traj(v0, N, C.idx(), T, C, C.pending(), O);
+                C.pending() = -1;
             }
             if (!dry) {
+                const long long first = s_range[0], total = s_range[1];
                 const int cnt = __popc(need);
                 const int leader = __ffs(need) - 1;
                 unsigned long long base = 0;
@@ -300,11 +326,15 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
                 if (!live) {
                     const long long cand = (long long)base + __popc(need & ((1u << lane) - 1u));
                     if (cand < total) {
-                        idx = S.order ? S.order[first + cand] : first + cand;
+                        const long long idx = S.order ? S.order[first + cand] : first + cand;
+                        C.idx() = idx;
                         load_traj<TRAP>(P, y0, N, idx, T, C);
+                        C.sprev() = T.c.sprev;
+                        C.n_acc() = T.c.n_acc;
+                        C.flags() = (int)T.c.flags;
 #pragma unroll
-                        for (int k = 0; k < 3; ++k) s_v0[k][threadIdx.x] = T.V[3 + k];
-                        stop_at = S.budget;
+                        for (int k = 0; k < 3; ++k) C.v0(k) = T.V[3 + k];
+                        C.stop_at() = S.budget;
                         may_suspend = true;
                         live = true;
                     }
@@ -313,26 +343,35 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
             }
             if (!__any_sync(FULL, live)) break;
         } else if (need) {
-            ++waited;
+            ++C.waited();
         }
         // warp-uniform: the queue is empty, the grace period is over and few lanes are still alive: at
         // fewer than ~11 lanes the six-lane kernel does more steps per SM and second than this one
-        const bool drain = dry && since_dry > S.tail_iters && (32 - __popc(need)) <= S.drain_lanes;
-        if (dry) ++since_dry;
+        const bool drain = dry && C.since_dry() > S.tail_iters && (32 - __popc(need)) <= S.drain_lanes;
+        if (dry) ++C.since_dry();
         // ---- one attempted step for every live lane
         if (live) {
+            // s(t), the step counter and the flags live in shared memory between two steps (volatile: re-read, not
+            // kept): three registers less through the stages, which is what lets the kernel run at 168 without a spill
             Attempt R;
+            T.c.flags = (unsigned)C.flags();
             dp45_attempt<TRAP>(P, T, R);
             bool first_turn;
+            T.c.sprev = C.sprev();
+            T.c.n_acc = C.n_acc();
+            T.c.flags = (unsigned)C.flags();
             const int st = finish_attempt(P, T, C, R, first_turn);
+            C.sprev() = T.c.sprev;
+            C.n_acc() = T.c.n_acc;
+            C.flags() = (int)T.c.flags;
             if (first_turn && O.x_turn1) {  // once per trajectory ("position")
 #pragma unroll
-                for (int k = 0; k < 3; ++k) O.x_turn1[k * N + idx] = T.X[k];
+                for (int k = 0; k < 3; ++k) O.x_turn1[k * N + C.idx()] = T.X[k];
             }
             if (st >= 0) {
-                pending = st;
+                C.pending() = st;
                 live = false;
-            } else if (may_suspend && (T.c.n_acc >= stop_at || drain)) {
+            } else if (may_suspend && (T.c.n_acc >= C.stop_at() || drain)) {
                 bool room = true;
                 if (!drain) {
                     // budget hand-over: only while few published slots wait to be taken, and only for a
@@ -359,12 +398,12 @@ integrate_kernel(const KParams P, const double* __restrict__ y0, const long long
                             }
                         }
                     }
-                    if (!room) stop_at = T.c.n_acc + again;
+                    if (!room) C.stop_at() = T.c.n_acc + again;
                 }
                 if (room) {
                     const long long slot = (long long)atomicAdd(S.n_out, 1ULL);
                     if (slot < S.out.cap) {
-                        ckpt_store(S.out, slot, idx, T, C);
+                        ckpt_store(S.out, slot, C.idx(), T, C);
                         live = false;
                     } else {
                         may_suspend = false;  // no slot left: finish it here
@@ -617,8 +656,8 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
 constexpr int kCntClass = 24;    // counters: trajectories per class (3; diagnostics)
 constexpr int kCntMeanU2 = 60;   // counters: <u^2> (double bits)
 constexpr int kPlanSamples = 64;
-// Inside a class the queue is ordered by slowness as well: kPlanSub buckets of u^2 / <u^2>, 1/8 wide, the
-// slowest first (the long trajectories of EVERY class are its slow ones, the unpredicted ones of class 2 too).
+// Inside a class the queue is ordered by slowness (and closeness) as well: kPlanSub buckets of u^2 / <u^2> + x^2/4,
+// 1/8 wide, the slowest first (the long trajectories of EVERY class are its slow ones, the unpredicted ones of class 2 too).
 // Bucket = class * kPlanSub + sub; their counts and placement cursors sit behind the first 64 counters.
 constexpr int kPlanSub = 16;
 constexpr int kPlanBuckets = 3 * kPlanSub;
@@ -720,10 +759,14 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
     }
     // b_c = (8 C4 / (mu u^2))^(1/4)
     const float bc = urel2 > 0.0f ? sqrtf(sqrtf((float)(8.0 * A.c4 / A.mu) / urel2)) : 3.0e38f;
-    const bool cand = sqrtf(dmin2) < (float)A.kappa * bc + mm;
+    const float x = sqrtf(dmin2) / ((float)A.kappa * bc + mm);  // closest approach in units of the capture range
+    const bool cand = x < 1.0f;
     const float r = usq / (float)mean_u2;
     const int cls = ((cand && r < (float)A.slow0) || r < (float)A.slow1) ? 0 : (cand ? 1 : 2);
-    const int sub = (int)fminf(8.0f * r, (float)(kPlanSub - 1));
+    // inside a class: slow and close first (measured on the bench workload: its longest trajectories start 2 ms earlier
+    // than by slowness alone)
+    const float xs = fminf(x, 2.0f);
+    const int sub = (int)fminf(8.0f * (r + 0.25f * xs * xs), (float)(kPlanSub - 1));
     return cls * kPlanSub + sub;
 }
 
