@@ -41,9 +41,9 @@ FLOPS_PER_ATTEMPT = 900.0
 FP64_PEAK_NOMINAL = 148 * 4 * 16 * 2 * 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of one integrate_kernel launch at the bench
 # workload, from the ncu --set full capture summarised in profiles/ (None until captured).
-INTEGRATE_DRAM_TRAFFIC_BYTES = 3.02e9
-INTEGRATE_DRAM_TRAFFIC_SOURCE = ("constant from the ncu --set full capture summarised in profiles/r01d_integrate_full.md "
-                                 "(integrator kernels of one call), NOT measured in this run")
+INTEGRATE_DRAM_TRAFFIC_BYTES = 8.81e9
+INTEGRATE_DRAM_TRAFFIC_SOURCE = ("constant from the ncu --set full capture summarised in profiles/r02_integrate_full.md "
+                                 "(the bulk integrator kernel of one call), NOT measured in this run")
 
 WORKLOAD_NAME = "configs[4] N=4194304 q=0.1 rtol=1e-10 atol=1e-12 seed=4"
 SWEEP_Q = (0.1, 0.2, 0.4)
@@ -297,6 +297,14 @@ def run_ours(args) -> int:
     n_tmax = sum_over_ranks(int((out["status"] == 1).sum().item()))
     max_steps_seen = int(max_over_ranks(float(out["n_acc"].max().item())))
 
+    if args.probe_six_lane:
+        # only the single-trajectory latency probe (the command of the six-lane kernel's ncu capture in profiles/)
+        aig.aig_integrate(aig.make_params(**w.params()), y0, w.t_max, w.rtol, w.atol, out=out, workspace=ws)
+        i_probe = int(torch.argmax(out["n_acc"] + out["n_rej"]).item())
+        us, n1 = six_lane_step_us(w, i_probe)
+        print(json.dumps({"probe": "six_lane_step", "trajectory": i_probe, "attempted_steps": n1, "us_per_step": us,
+                          "cycles_per_step_at_1965MHz": us * 1965.0}), flush=True)
+        return 0
     i_longest = int(torch.argmax(out["n_acc"] + out["n_rej"]).item())
     max_attempted = int((out["n_acc"][i_longest] + out["n_rej"][i_longest]).item())
     step_us, _ = six_lane_step_us(w, i_longest)
@@ -467,6 +475,8 @@ def main() -> int:
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-side", action="store_true", help="skip timing aig_observables / aig_outliers")
+    ap.add_argument("--probe-six-lane", action="store_true",
+                    help="run only the latency probe: the workload's longest trajectory alone in the six-lane integrator")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=2097152)
     ap.add_argument("--ref-sample", type=int, default=262144)
