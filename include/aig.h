@@ -204,6 +204,23 @@ int aig_run_host(const aig_params *p, const double *y0_host, int64_t N, double t
                  double atol, const aig_out *out_host, const aig_hist_spec *hist_spec_host,
                  const aig_hist *hist_out_host);
 
+/* NEXT-2: an observable against the launch direction (the paper's heatmaps).
+ * The direction of trajectory i is that of x_atom - x_ion at t0 (rows 6-8 minus rows 0-2 of y0): u = (1 - cos theta)/2
+ * in [0, 1] (equal steps of u are equal solid angles, eq. (12)-(13) at PAPER.md:92-98) and phi = atan2(dy, dx) brought
+ * into [0, 2 pi).  Cells are given by explicit edges (DEVICE pointers, strictly increasing, n + 1 of them, n in 1..4096
+ * each): cell (a, b) holds u_edges[a] <= u < u_edges[a+1], phi_edges[b] <= phi < phi_edges[b+1].  For every trajectory
+ * inside the window whose value is not NaN: count[a * n_phi + b] += 1, sum[a * n_phi + b] += value[i] (DEVICE arrays
+ * of n_u * n_phi, ACCUMULATED into: the caller zeroes them; sum / count is the map).  On a "uniform" grid workload
+ * with edges half-way between the grid directions the map is the value array reshaped to [ntheta][nphi]. */
+typedef struct aig_map_spec {
+    const double *u_edges;
+    int32_t n_u;
+    const double *phi_edges;
+    int32_t n_phi;
+} aig_map_spec;
+int aig_map2d(const double *y0, int64_t N, const double *value, const aig_map_spec *spec, uint64_t *count,
+              double *sum, void *cuda_stream);
+
 /* Measurement aid: run a register-resident FP64 FMA chain kernel on every SM and return the
  * achieved non-tensor FP64 rate in FLOP/s through *flops_per_s (blocking; used by bench.py as
  * the measured ALU roofline denominator). ilp in [1, 16] independent chains per thread. */

@@ -316,3 +316,28 @@ def outliers(obs: dict) -> dict:
                 hi = i
         out[k] = (lo, hi)
     return out
+
+
+def map2d(y0, value, u_edges, phi_edges):
+    """PAPER.md:483, :517 (an observable against the launch direction), as a definition: the direction of
+    trajectory i is that of x_atom - x_ion at t0; u = (1 - cos theta)/2, phi = atan2(dy, dx) in [0, 2 pi); cell
+    (a, b) holds u_edges[a] <= u < u_edges[a+1], phi_edges[b] <= phi < phi_edges[b+1].  Returns (count, sum) of the
+    non-NaN values inside the window, [n_u][n_phi].  Plain loop."""
+    y0 = np.asarray(y0, dtype=np.float64)
+    ue, pe = np.asarray(u_edges, dtype=np.float64), np.asarray(phi_edges, dtype=np.float64)
+    nu, nph = len(ue) - 1, len(pe) - 1
+    count = np.zeros((nu, nph), dtype=np.int64)
+    total = np.zeros((nu, nph), dtype=np.float64)
+    d = y0[6:9] - y0[0:3]
+    r = np.sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2])
+    u = 0.5 * (1.0 - d[2] / r)
+    phi = np.arctan2(d[1], d[0])
+    phi = np.where(phi < 0.0, phi + 2.0 * np.pi, phi)
+    a = np.searchsorted(ue, u, side="right")
+    b = np.searchsorted(pe, phi, side="right")
+    for i in range(y0.shape[1]):
+        v = value[i]
+        if 1 <= a[i] <= nu and 1 <= b[i] <= nph and v == v:
+            count[a[i] - 1, b[i] - 1] += 1
+            total[a[i] - 1, b[i] - 1] += v
+    return count, total

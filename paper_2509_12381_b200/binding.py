@@ -19,7 +19,7 @@ _lib = None
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
            "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_set_schedule", "aig_strerror",
            "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes", "aig_trace",
-           "aig_set_schedule_ex", "aig_get_schedule"]
+           "aig_set_schedule_ex", "aig_get_schedule", "aig_map2d"]
 
 
 class AigError(RuntimeError):
@@ -236,6 +236,33 @@ def aig_outliers(obs, extra, stream=None):
     _check(L.aig_outliers(C.byref(o), C.byref(e), N, res.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "aig_outliers")
     res._ws = ws  # keep the scratch alive until the stream has run
     return res
+
+
+class MapSpec(C.Structure):
+    _fields_ = [("u_edges", C.c_void_p), ("n_u", C.c_int32), ("phi_edges", C.c_void_p), ("n_phi", C.c_int32)]
+
+
+def aig_map2d(y0, value, u_edges, phi_edges, count=None, total=None, stream=None):
+    """An observable against the launch direction (include/aig.h: aig_map2d): returns (count [n_u, n_phi] int64,
+    sum [n_u, n_phi] float64) CUDA tensors, accumulated into when given."""
+    torch = _torch()
+    N = y0.shape[1]
+    assert y0.is_cuda and y0.dtype == torch.float64 and y0.shape[0] == 12 and y0.is_contiguous()
+    assert value.is_cuda and value.dtype == torch.float64 and value.numel() == N and value.is_contiguous()
+    for e in (u_edges, phi_edges):
+        assert e.is_cuda and e.dtype == torch.float64 and e.is_contiguous() and e.numel() >= 2
+    nu, nph = u_edges.numel() - 1, phi_edges.numel() - 1
+    if count is None:
+        count = torch.zeros((nu, nph), dtype=torch.int64, device=y0.device)
+    if total is None:
+        total = torch.zeros((nu, nph), dtype=torch.float64, device=y0.device)
+    spec = MapSpec(u_edges.data_ptr(), nu, phi_edges.data_ptr(), nph)
+    L = lib()
+    L.aig_map2d.restype = C.c_int
+    L.aig_map2d.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    _check(L.aig_map2d(y0.data_ptr(), N, value.data_ptr(), C.byref(spec), count.data_ptr(), total.data_ptr(),
+                       _stream_ptr(stream)), "aig_map2d")
+    return count, total
 
 
 def aig_trace(params: Params, y0, t_max, rtol, atol, cap: int = 1 << 20, stream=None):

@@ -410,6 +410,7 @@ template <int TRAP>
 __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, Attempt& R)
 {
     const double h = T.c.h;
+    const double h2 = h * h;
     const double t_new = (T.c.flags & kLast) ? P.t_max : T.c.t + h;
 
     // A[i][l]: acceleration component i (0-2 ion, 3-5 atom) of stage l+1
@@ -427,11 +428,6 @@ __device__ __forceinline__ void dp45_attempt(const KParams& P, const Traj& T, At
     // three levels; the two stages of a level are independent of each other
 #pragma unroll
     for (int lev = 0; lev < 3; ++lev) {
-        // h^2 is formed again at every level (the same product, the same bits) instead of living in a register
-        // pair through the force evaluations in between: the kernel runs at the register count that allows three
-        // blocks per SM, without a spill
-        double h2;
-        asm volatile("mul.f64 %0, %1, %1;" : "=d"(h2) : "d"(h));
         // cos(Omega t) at the stage times of this level (independent of the positions; c6 = c7 = 1)
         double cs[2];
         cs[0] = trap_cos<TRAP>(P, (lev == 2) ? t_new : fma(kC[2 * lev + 1], h, T.c.t));

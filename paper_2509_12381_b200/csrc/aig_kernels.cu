@@ -38,10 +38,6 @@ namespace aig {
 #ifndef AIG_MIN_BLOCKS
 #define AIG_MIN_BLOCKS 3
 #endif
-#ifndef AIG_SPLIT_UNROLL
-#define AIG_SPLIT_UNROLL 2
-#endif
-constexpr int kSplitUnroll = AIG_SPLIT_UNROLL;  // steps per basic block of the six-lane integrator
 constexpr int kBlock = AIG_BLOCK;             // threads per block of the integrator
 constexpr int kBlocksPerSM = AIG_MIN_BLOCKS;  // resident blocks per SM the register budget is sized for
 
@@ -260,13 +256,8 @@ struct Sched {
     unsigned long long* timeline;
 };
 
-#ifdef AIG_MAXNREG
-#define AIG_BULK_BOUNDS __maxnreg__(AIG_MAXNREG)
-#else
-#define AIG_BULK_BOUNDS __launch_bounds__(BLOCK, MINB)
-#endif
 template <int TRAP, int BLOCK, int MINB>
-__global__ void AIG_BULK_BOUNDS
+__global__ void __launch_bounds__(BLOCK, MINB)
 integrate_kernel(const KParams P, const double* __restrict__ y0, const long long N, const OutPtrs O,
                  const Sched S)
 {
@@ -1298,6 +1289,34 @@ outliers_kernel(const OutlierArgs a, const long long N)
 }
 
 // ------------------------------------------------------------------------------------------
+// NEXT-2: an observable against the launch direction
+// ------------------------------------------------------------------------------------------
+// HBM-bound: 56 B read per trajectory; one global atomic pair per trajectory inside the window (thousands of
+// cells: little contention).  Edges are searched in global memory (L1-resident: a few KB).
+__global__ void __launch_bounds__(256)
+map2d_kernel(const double* __restrict__ y0, const long long N, const double* __restrict__ value,
+             const double* __restrict__ u_edges, const int n_u, const double* __restrict__ phi_edges, const int n_phi,
+             unsigned long long* __restrict__ count, double* __restrict__ sum)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+        const double v = value[i];
+        const double dx = y0[6 * N + i] - y0[0 * N + i], dy = y0[7 * N + i] - y0[1 * N + i],
+                     dz = y0[8 * N + i] - y0[2 * N + i];
+        const double r = sqrt(sum3(dx * dx, dy * dy, dz * dz));
+        const double u = 0.5 * (1.0 - dz / r);
+        double phi = atan2(dy, dx);
+        if (phi < 0.0) phi += 6.283185307179586;
+        const int a = bin_of(u_edges, n_u, u), b = bin_of(phi_edges, n_phi, phi);  // 0 / n + 1: outside (NaN too)
+        if (a >= 1 && a <= n_u && b >= 1 && b <= n_phi && v == v) {
+            const long long cell = (long long)(a - 1) * n_phi + (b - 1);
+            atomicAdd(count + cell, 1ULL);
+            atomicAdd(sum + cell, v);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // FP64 roofline probe: ILP independent FMA chains per thread, all in registers
 // ------------------------------------------------------------------------------------------
 template <int ILP>
@@ -1928,6 +1947,29 @@ int aig_observables(const aig_params* p, const double* y0, const aig_out* out, i
     const long long blocks = std::min<long long>((N + 255) / 256, (long long)sms * 8);
     observables_kernel<<<(unsigned)blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
         y0, out->y_final, N, p->m_ion, p->m_atom, extra->dist, extra->KE, extra->transfer, out->x_turn1, extra->position);
+    g_kernel_launches++;
+    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
+}
+
+int aig_map2d(const double* y0, int64_t N, const double* value, const aig_map_spec* spec, uint64_t* count, double* sum,
+              void* cuda_stream)
+{
+    if (!spec) return AIG_ERR_NULL;
+    if (N < 0 || N > (1LL << 40)) return AIG_ERR_SIZE;
+    if (spec->n_u < 1 || spec->n_phi < 1 || spec->n_u > 4096 || spec->n_phi > 4096) return AIG_ERR_SIZE;
+    if (!spec->u_edges || !spec->phi_edges || !count || !sum) return AIG_ERR_NULL;
+    if (N == 0) return AIG_OK;
+    if (!y0 || !value) return AIG_ERR_NULL;
+    if (!aligned(y0, 8) || !aligned(value, 8) || !aligned(spec->u_edges, 8) || !aligned(spec->phi_edges, 8) ||
+        !aligned(count, 8) || !aligned(sum, 8))
+        return AIG_ERR_ALIGN;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AIG_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return AIG_ERR_CUDA;
+    const long long blocks = std::min<long long>((N + 255) / 256, (long long)sms * 8);
+    map2d_kernel<<<(unsigned)blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        y0, N, value, spec->u_edges, spec->n_u, spec->phi_edges, spec->n_phi,
+        reinterpret_cast<unsigned long long*>(count), sum);
     g_kernel_launches++;
     return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }

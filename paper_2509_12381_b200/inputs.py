@@ -250,6 +250,22 @@ def grid_angles(w: Workload):
     return np.arccos(1.0 - 2.0 * u), np.linspace(p0, p1, nph)
 
 
+def map_edges(w: Workload, n_u: int | None = None, n_phi: int | None = None):
+    """Cell edges (u_edges, phi_edges) for a map of an observable against the launch direction (aig_map2d) over the
+    (theta, phi) window of a "grid" workload, u = (1 - cos theta)/2.  Defaults: one cell per grid direction, edges
+    half-way between neighbouring directions (the outer ones half a spacing beyond the window), so that on a
+    "uniform" grid the map is the value array reshaped; for random directions pass the cell counts: equal steps of u
+    (equal solid angles) and of phi inside the window."""
+    (t0, t1), (p0, p1) = w.notes["theta"], w.notes["phi"]
+    u0, u1 = (1.0 - math.cos(t0)) / 2.0, (1.0 - math.cos(t1)) / 2.0
+    if n_u is None and n_phi is None:
+        nt, nph = w.notes["ntheta"], w.notes["nphi"]
+        du = (u1 - u0) / max(nt - 1, 1)
+        dp = (p1 - p0) / max(nph - 1, 1)
+        return (u0 - du / 2 + du * np.arange(nt + 1), p0 - dp / 2 + dp * np.arange(nph + 1))
+    return np.linspace(u0, u1, int(n_u) + 1), np.linspace(p0, p1, int(n_phi) + 1)
+
+
 PAPER_DRAWS = 16  # uniforms per trajectory of a "grid" workload: 0-1 direction, 2-15 seven Box-Muller pairs
 
 

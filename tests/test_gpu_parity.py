@@ -944,3 +944,41 @@ def test_run_host_end_to_end(aig):
     assert np.array_equal(res["x_turn1"].view(np.uint64), dev["x_turn1"].view(np.uint64))
     ref = orc.histogram(dev, ae, le, 64)
     assert all(np.array_equal(res["hist"][k], ref[k]) for k in ref)
+
+
+def test_map2d_observable_against_launch_direction(aig):
+    """NEXT-2: aig_map2d against its definition (oracle.map2d) -- counts exact, sums to rounding
+    (the order of the atomic additions is free) -- for random launch directions of the paper's workload, with the
+    integrator's scattering angle as the observable, several blocks and a ragged tail; the grid workload maps onto
+    its own reshape; NaN values and directions outside the window are skipped; N = 0."""
+    import torch
+    w = inputs.paper_workload(ntheta=173, nphi=71, theta=(0.2, 2.4), phi=(0.3, 5.1), positions="random", t_max=2.0e11)
+    y0 = inputs.generate_y0(w)
+    y0d = _dev(y0)
+    out = aig.aig_integrate(aig.make_params(**w.params()), y0d, w.t_max, w.rtol, w.atol)
+    val = out["angle"].clone()
+    val[::97] = float("nan")
+    ue, pe = inputs.map_edges(w, 24, 40)
+    ue, pe = ue[2:-3].copy(), pe[1:-4].copy()           # a window smaller than the data: some directions fall outside
+    d = y0[6:9] - y0[0:3]
+    u = 0.5 * (1 - d[2] / np.linalg.norm(d, axis=0))
+    phi = np.mod(np.arctan2(d[1], d[0]), 2 * math.pi)
+    assert np.min(np.abs(u[:, None] - ue[None, :])) > 1e-12 and np.min(np.abs(phi[:, None] - pe[None, :])) > 1e-12
+    count, total = aig.aig_map2d(y0d, val, _dev(ue), _dev(pe))
+    c_ref, t_ref = orc.map2d(y0, val.cpu().numpy(), ue, pe)
+    assert np.array_equal(count.cpu().numpy(), c_ref) and 0 < c_ref.sum() < w.N * 0.9
+    assert np.allclose(total.cpu().numpy(), t_ref, rtol=1e-12, atol=1e-12)
+    aig.aig_map2d(y0d, val, _dev(ue), _dev(pe), count=count, total=total)       # accumulates
+    assert np.array_equal(count.cpu().numpy(), 2 * c_ref)
+    # grid workload: the map is the reshape
+    wg = inputs.paper_workload(ntheta=12, nphi=17, theta=(0.3, 1.4), phi=(0.2, 1.3))
+    yg = inputs.generate_y0(wg)
+    vg = np.arange(wg.N, dtype=float) + 0.25
+    ueg, peg = inputs.map_edges(wg)
+    cg, tg = aig.aig_map2d(_dev(yg), _dev(vg), _dev(ueg), _dev(peg))
+    assert np.array_equal(cg.cpu().numpy(), np.ones((12, 17), dtype=np.int64))
+    assert np.array_equal(tg.cpu().numpy(), vg.reshape(12, 17))
+    # N = 0
+    e12 = torch.empty((12, 0), dtype=torch.float64, device="cuda")
+    c0, _ = aig.aig_map2d(e12, torch.empty(0, dtype=torch.float64, device="cuda"), _dev(ueg), _dev(peg))
+    assert int(c0.sum().item()) == 0

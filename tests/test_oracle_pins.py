@@ -907,3 +907,50 @@ def test_lennard_jones_6_12_conserves_energy_and_angular_momentum():
     assert np.max(np.abs(E1 - E0)) <= 1e-7 * De
     assert np.max(np.abs(L1 - L0)) <= 1e-8 * np.max(np.abs(L0))
     assert np.all(o["status"] <= 1) and o["n_turn"].max() >= 1
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-2: an observable against the launch direction
+# ------------------------------------------------------------------------------------------
+
+def test_map2d_hand_directions_and_grid_reshape():
+    # six axis directions: +z is u = 0, -z is u = 1, the equator u = 1/2 with phi = 0, pi/2, pi, 3 pi/2
+    y0 = np.zeros((12, 6))
+    y0[0:3] = np.array([[1.0, 2.0, 3.0]]).T                      # the ion is not at the origin: the direction is relative
+    for i, d in enumerate([(0, 0, 1), (0, 0, -1), (1, 0, 0), (0, 1, 0), (-1, 0, 0), (0, -1, 0)]):
+        y0[6:9, i] = y0[0:3, i] + 7.0 * np.array(d)
+    ue = np.array([0.0, 0.25, 0.75, 1.0 + 1e-12])
+    pe = np.array([0.0, 1.0, 2.0, 4.0, 2 * math.pi])
+    val = np.array([1.0, 2.0, 4.0, 8.0, 16.0, float("nan")])
+    count, total = orc.map2d(y0, val, ue, pe)
+    want = np.zeros((3, 4))
+    want[0, 0] = 1.0      # +z: u = 0, phi = atan2(0, 0) = 0
+    want[2, 0] = 2.0      # -z
+    want[1, 0] = 4.0      # +x: phi = 0
+    want[1, 1] = 8.0      # +y: phi = pi/2 in [1, 2)
+    want[1, 2] = 16.0     # -x: phi = pi in [2, 4)
+    assert np.array_equal(total, want) and count.sum() == 5     # -y (phi = 3 pi/2) holds the NaN: skipped
+    # the paper's grid (eq. 12-13): with edges half-way between the grid directions the map IS the reshape
+    w = inputs.paper_workload(ntheta=7, nphi=9, theta=(0.3, 1.4), phi=(0.2, 1.3))
+    y0 = inputs.generate_y0(w)
+    val = np.arange(w.N, dtype=float) + 0.5
+    ue, pe = inputs.map_edges(w)
+    count, total = orc.map2d(y0, val, ue, pe)
+    assert np.array_equal(count, np.ones((7, 9), dtype=np.int64)) and np.array_equal(total, val.reshape(7, 9))
+
+
+def test_map2d_equal_solid_angle_cells_fill_uniformly():
+    # isotropic directions (config 0's generator) on an equal-u x equal-phi grid: every cell the same expectation
+    w = inputs.config(0).replace(N=40000)
+    y0 = inputs.generate_y0(w)
+    ue, pe = np.linspace(0.0, 1.0 + 1e-12, 9), np.linspace(0.0, 2 * math.pi, 11)
+    count, total = orc.map2d(y0, np.ones(w.N), ue, pe)
+    assert count.sum() == w.N and np.array_equal(total, count.astype(float))
+    expect = w.N / count.size
+    chi2 = float(((count - expect) ** 2 / expect).sum())
+    assert chi2 < 130.0, chi2          # 79 degrees of freedom: mean 79, 99.9 % quantile 124
+    # equal steps of THETA instead would not: the polar caps would be nearly empty
+    te = 0.5 * (1 - np.cos(np.linspace(0, math.pi, 9)))
+    te[-1] += 1e-12
+    c2, _ = orc.map2d(y0, np.ones(w.N), te, pe)
+    assert c2[0].sum() < 0.5 * c2[4].sum()
