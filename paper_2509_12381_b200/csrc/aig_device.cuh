@@ -341,6 +341,29 @@ __device__ __forceinline__ double axis_quotient(const Ratio cvi, const Ratio cxi
     return m.n * rcp_nr(m.d);
 }
 
+// The same quotient with the four reciprocals taken BEFORE the maximum is known (the six-lane kernel: three more
+// reciprocals issued, four fewer operations on the dependent chain).  The reciprocal travels with its ratio through
+// the same cross-multiplication tree, so the result is m.n * rcp_nr(m.d) of the same m: the same bits.
+struct RatioR {
+    double n, d, r;
+};
+__device__ __forceinline__ RatioR ratio_max_r(const RatioR a, const RatioR b)
+{
+    const bool gt = b.n * a.d > a.n * b.d;
+    RatioR m;
+    m.n = gt ? b.n : a.n;
+    m.d = gt ? b.d : a.d;
+    m.r = gt ? b.r : a.r;
+    return m;
+}
+__device__ __forceinline__ double axis_quotient_early_rcp(const Ratio cvi, const Ratio cxi, const Ratio cva, const Ratio cxa)
+{
+    const RatioR a{cvi.n, cvi.d, rcp_nr(cvi.d)}, b{cxi.n, cxi.d, rcp_nr(cxi.d)}, c{cva.n, cva.d, rcp_nr(cva.d)},
+        d{cxa.n, cxa.d, rcp_nr(cxa.d)};
+    const RatioR m = ratio_max_r(ratio_max_r(a, b), ratio_max_r(c, d));
+    return m.n * m.r;
+}
+
 // Controller state of one trajectory: time, step size, radial observable at t, accepted-step
 // count and flags.  The split kernel keeps a copy on each of a trajectory's six lanes.
 struct Core {

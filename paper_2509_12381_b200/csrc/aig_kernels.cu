@@ -631,14 +631,14 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
 //     centrifugal barrier of the -C4/r^4 tail, i.e. if the atom passes the ion within the Langevin
 //     radius b_c = (4 C4/E)^(1/4), E = mu u^2/2.  With the trap on, the ion is not where it started when
 //     the atom arrives (at q = 0.4 it has moved by more than the whole range of impact parameters), so
-//     the closest approach is estimated by a PRE-FLIGHT: the atom on its straight line against the ion on
-//     its secular orbit, x_k(t) = x_k0 cos w_k t + (v_k0/w_k) sin w_k t with w_k = (Omega/2) sqrt(a_k + q_k^2/2)
-//     (PAPER.md:282), sampled at 64 times over the fly-by and refined by a parabola.  "Candidates" pass
-//     within kappa b_c + the micromotion amplitude max_k |q_k x_k| / 2 there (kappa = 1.5: the rest of the
-//     blur), with b_c from the relative speed at that moment.  Without a trap this is the impact parameter.
+//     the closest approach is estimated by a PRE-FLIGHT: the atom on its straight line against the ion
+//     moving in the trap alone -- eq. (4)-(6) without the atom, integrated by classical RK4 in 96 steps
+//     over the fly-by, in single precision (a secular-orbit formula is off by 15-40 % of the orbit at the
+//     trap strengths of the configs: as much as b_c itself) -- and refined by a parabola through the
+//     three samples around the minimum.  "Candidates" pass within kappa b_c (kappa = 1.5), b_c from the
+//     relative speed at that moment.  Without a trap this is the impact parameter.
 // (2) Among them the slow ones take longest: the flight alone lasts ~1/u, and the complexes that
-//     survive until t_max are low-energy ones (of the 12 longest trajectories of the bench
-//     workload all have u^2 < <u^2>/2; measured).
+//     survive until t_max are low-energy ones.
 // Three classes, queued in this order:
 //     0: candidates with u^2 < <u^2>/2, and anything with u^2 < <u^2>/10   1: the other candidates
 //     2: the rest
@@ -646,7 +646,7 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
 // later -- instead of anywhere.  Affects scheduling only, never a result.
 constexpr int kCntClass = 24;    // counters: trajectories per class (3; diagnostics)
 constexpr int kCntMeanU2 = 60;   // counters: <u^2> (double bits)
-constexpr int kPlanSamples = 64;
+constexpr int kPlanSamples = 96;
 // Inside a class the queue is ordered by slowness (and closeness) as well: kPlanSub buckets of u^2 / <u^2> + x^2/4,
 // 1/8 wide, the slowest first (the long trajectories of EVERY class are its slow ones, the unpredicted ones of class 2 too).
 // Bucket = class * kPlanSub + sub; their counts and placement cursors sit behind the first 64 counters.
@@ -659,8 +659,8 @@ struct PlanArgs {
     double mu, c4;        // reduced mass, C4
     double kappa;
     double slow0, slow1;  // class thresholds as fractions of <u^2>
-    double w[3];          // secular frequencies of the ion (0: free along that axis)
-    double hq[3];         // |q_k| / 2: relative micromotion amplitude
+    float wa[3], wb[3];   // trap stiffness of the ion: w_k(t) = wa_k + wb_k cos(Omega t)  (eq. (4)-(6))
+    float omega, phase0;  // Omega, Omega t0 reduced to [0, 2 pi)
     double span;          // t_max - t0
 };
 
@@ -691,32 +691,34 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
     // fly-by window: twice the time to cover the initial distance, within the time span
     float T = (float)A.span;
     if (usq > 0.0f) T = fminf(T, 2.0f * sqrtf(dsq / usq));
-    const float dt = T / kPlanSamples;
-    // ion on its secular orbit, by the rotation recurrence: (c, s)_j = (cos, sin)(w_k j dt); free axes move linearly
-    float c[3], sn[3], cd[3], sd[3], amp[3], w[3];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        w[k] = (float)A.w[k];
-        c[k] = 1.0f;
-        sn[k] = 0.0f;
-        sincosf(w[k] * dt, &sd[k], &cd[k]);
-        amp[k] = w[k] > 0.0f ? vi[k] / w[k] : 0.0f;
-    }
-    float f_prev = dsq, f_best = dsq, f_before = dsq, f_after = dsq;
+    const float h = T / kPlanSamples, hh = 0.5f * h, h6 = h * (1.0f / 6.0f);
+    // the ion in the trap alone: x_k'' = -w_k(t) x_k, classical RK4; the phase Omega t is advanced directly
+    float x[3] = {xi[0], xi[1], xi[2]}, v[3] = {vi[0], vi[1], vi[2]};
+    const float dph = A.omega * h;
+    float c0 = __cosf(A.phase0);
+    float f_prev = dsq, f_best = dsq, f_before = dsq, f_after = dsq, u_best = usq;
     int j_best = 0;
     bool want_after = true;
     for (int j = 1; j <= kPlanSamples; ++j) {
-        const float t = dt * j;
-        float f = 0.0f;
+        const float ph = A.phase0 + dph * (float)(j - 1);
+        const float ch = __cosf(ph + 0.5f * dph), c1 = __cosf(ph + dph);
+        const float t = h * (float)j;
+        float f = 0.0f, us = 0.0f;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const float cn = c[k] * cd[k] - sn[k] * sd[k];
-            sn[k] = sn[k] * cd[k] + c[k] * sd[k];
-            c[k] = cn;
-            const float xk = w[k] > 0.0f ? xi[k] * c[k] + amp[k] * sn[k] : xi[k] + vi[k] * t;
-            const float dk = xa[k] + va[k] * t - xk;
-            f += dk * dk;
+            const float w0 = fmaf(A.wb[k], c0, A.wa[k]), wh = fmaf(A.wb[k], ch, A.wa[k]), w1 = fmaf(A.wb[k], c1, A.wa[k]);
+            const float k1x = v[k], k1v = -w0 * x[k];
+            const float k2x = fmaf(hh, k1v, v[k]), k2v = -wh * fmaf(hh, k1x, x[k]);
+            const float k3x = fmaf(hh, k2v, v[k]), k3v = -wh * fmaf(hh, k2x, x[k]);
+            const float k4x = fmaf(h, k3v, v[k]), k4v = -w1 * fmaf(h, k3x, x[k]);
+            x[k] = fmaf(h6, (k1x + k4x) + 2.0f * (k2x + k3x), x[k]);
+            v[k] = fmaf(h6, (k1v + k4v) + 2.0f * (k2v + k3v), v[k]);
+            const float dk = fmaf(va[k], t, xa[k]) - x[k];
+            const float uk = va[k] - v[k];
+            f = fmaf(dk, dk, f);
+            us = fmaf(uk, uk, us);
         }
+        c0 = c1;
         if (want_after) {
             f_after = f;
             want_after = false;
@@ -725,6 +727,7 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
             f_best = f;
             f_before = f_prev;
             j_best = j;
+            u_best = us;
             want_after = true;
             f_after = f;
         }
@@ -735,28 +738,16 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
     float off = 0.0f;
     if (den > 0.0f && j_best > 0 && j_best < kPlanSamples) off = fminf(fmaxf(0.5f * (f_before - f_after) / den, -1.0f), 1.0f);
     const float dmin2 = fmaxf(f_best - 0.25f * (f_before - f_after) * off, 0.0f);
-    const float ts = dt * (j_best + off);
-    // relative speed and micromotion amplitude at the closest approach
-    float urel2 = 0.0f, mm = 0.0f;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        float sk, ck;
-        sincosf(w[k] * ts, &sk, &ck);
-        const float xk = w[k] > 0.0f ? xi[k] * ck + amp[k] * sk : xi[k] + vi[k] * ts;
-        const float vk = w[k] > 0.0f ? vi[k] * ck - xi[k] * w[k] * sk : vi[k];
-        const float uk = va[k] - vk;
-        urel2 += uk * uk;
-        mm = fmaxf(mm, (float)A.hq[k] * fabsf(xk));
-    }
+    const float urel2 = u_best;  // relative speed at the sample of the closest approach
     // b_c = (8 C4 / (mu u^2))^(1/4)
     const float bc = urel2 > 0.0f ? sqrtf(sqrtf((float)(8.0 * A.c4 / A.mu) / urel2)) : 3.0e38f;
-    const float x = sqrtf(dmin2) / ((float)A.kappa * bc + mm);  // closest approach in units of the capture range
-    const bool cand = x < 1.0f;
+    const float xc = sqrtf(dmin2) / ((float)A.kappa * bc);  // closest approach in units of the capture range
+    const bool cand = xc < 1.0f;
     const float r = usq / (float)mean_u2;
     const int cls = ((cand && r < (float)A.slow0) || r < (float)A.slow1) ? 0 : (cand ? 1 : 2);
     // inside a class: slow and close first (measured on the bench workload: its longest trajectories start 2 ms earlier
     // than by slowness alone)
-    const float xs = fminf(x, 2.0f);
+    const float xs = fminf(xc, 2.0f);
     const int sub = (int)fminf(8.0f * (r + 0.25f * xs * xs), (float)(kPlanSub - 1));
     return cls * kPlanSub + sub;
 }
@@ -1612,12 +1603,13 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         A.slow0 = cfg.slow0;
         A.slow1 = cfg.slow1;
         A.span = K.t_max - K.t0;
+        const double W = 0.25 * p->omega_rf * p->omega_rf;
         for (int k = 0; k < 3; ++k) {
-            // secular frequency (Omega/2) sqrt(a_k + q_k^2/2); not confining: free along that axis
-            const double beta2 = p->a[k] + 0.5 * p->q[k] * p->q[k];
-            A.w[k] = beta2 > 0.0 ? 0.5 * std::fabs(p->omega_rf) * std::sqrt(beta2) : 0.0;
-            A.hq[k] = 0.5 * std::fabs(p->q[k]);
+            A.wa[k] = (float)(p->a[k] * W);
+            A.wb[k] = (float)(2.0 * p->q[k] * W);
         }
+        A.omega = (float)p->omega_rf;
+        A.phase0 = (float)std::fmod(p->omega_rf * p->t0, 6.283185307179586);
         const unsigned pg = (unsigned)((N + 255) / 256);
         plan_mean_kernel<<<1, 1024, 0, st>>>(y0, N, counters);
         plan_kernel<0><<<pg, 256, 0, st>>>(y0, N, A, order, cls_of, counters);

@@ -20,6 +20,10 @@
 #pragma once
 #include "aig_device.cuh"
 
+#ifndef AIG_SPLIT_EARLY_RCP
+#define AIG_SPLIT_EARLY_RCP 1
+#endif
+
 namespace aig {
 
 constexpr int kGroupLanes = 6;                     // lanes per trajectory
@@ -186,7 +190,7 @@ __device__ __forceinline__ void split_attempt(const KParams& P, const SplitRole&
     Ratio cvi, cxi, cva, cxa;
     const double vni = step_end_finish(Si, h, xni, Y.vi, Ai[5], Ai[6], cvi, cxi);
     const double vna = step_end_finish(Sa, h, xna, Y.va, Aa[5], Aa[6], cva, cxa);
-    const double q = axis_quotient(cvi, cxi, cva, cxa);
+    const double q = AIG_SPLIT_EARLY_RCP ? axis_quotient_early_rcp(cvi, cxi, cva, cxa) : axis_quotient(cvi, cxi, cva, cxa);
     const double p = (xna - xni) * (vna - vni);
     const int src = R.base + R.e;
     const double q0 = shfl_d(q, src), q1 = shfl_d(q, src + 2), q2 = shfl_d(q, src + 4);
