@@ -632,7 +632,7 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
 //     radius b_c = (4 C4/E)^(1/4), E = mu u^2/2.  With the trap on, the ion is not where it started when
 //     the atom arrives (at q = 0.4 it has moved by more than the whole range of impact parameters), so
 //     the closest approach is estimated by a PRE-FLIGHT: the atom on its straight line against the ion
-//     moving in the trap alone -- eq. (4)-(6) without the atom, integrated by classical RK4 in 96 steps
+//     moving in the trap alone -- eq. (4)-(6) without the atom, integrated by classical RK4 in 64 steps
 //     over the fly-by, in single precision (a secular-orbit formula is off by 15-40 % of the orbit at the
 //     trap strengths of the configs: as much as b_c itself) -- and refined by a parabola through the
 //     three samples around the minimum.  "Candidates" pass within kappa b_c (kappa = 1.5), b_c from the
@@ -646,7 +646,7 @@ integrate_split_kernel(const KParams P, const double* __restrict__ y0, const lon
 // later -- instead of anywhere.  Affects scheduling only, never a result.
 constexpr int kCntClass = 24;    // counters: trajectories per class (3; diagnostics)
 constexpr int kCntMeanU2 = 60;   // counters: <u^2> (double bits)
-constexpr int kPlanSamples = 96;
+constexpr int kPlanSamples = 64;
 // Inside a class the queue is ordered by slowness (and closeness) as well: kPlanSub buckets of u^2 / <u^2> + x^2/4,
 // 1/8 wide, the slowest first (the long trajectories of EVERY class are its slow ones, the unpredicted ones of class 2 too).
 // Bucket = class * kPlanSub + sub; their counts and placement cursors sit behind the first 64 counters.
@@ -752,21 +752,24 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
     return cls * kPlanSub + sub;
 }
 
-// <u^2> over the first min(N, 65536) trajectories (a sample is enough for a scheduling threshold)
+// <u^2> over the first min(N, 65536) trajectories (a sample is enough for a scheduling threshold): 64 blocks add
+// their partial sums into counters[kCntMeanU2] (a double, zero from the call's memset); the readers divide by n
+constexpr long long kPlanMeanSample = 65536;
 __global__ void __launch_bounds__(1024)
 plan_mean_kernel(const double* __restrict__ y0, const long long N, unsigned long long* __restrict__ counters)
 {
     __shared__ double part[32];
-    const long long n = N < 65536 ? N : 65536;
+    const long long n = N < kPlanMeanSample ? N : kPlanMeanSample;
     double s = 0.0;
-    for (long long i = threadIdx.x; i < n; i += blockDim.x) s += rel_speed2(y0, N, i);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        s += rel_speed2(y0, N, i);
     for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
     if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
     __syncthreads();
     if (threadIdx.x < 32) {
         s = (threadIdx.x < (blockDim.x >> 5)) ? part[threadIdx.x] : 0.0;
         for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
-        if (threadIdx.x == 0) counters[kCntMeanU2] = (unsigned long long)__double_as_longlong(s / (double)n);
+        if (threadIdx.x == 0) atomicAdd(reinterpret_cast<double*>(counters + kCntMeanU2), s);
     }
 }
 
@@ -783,7 +786,8 @@ plan_kernel(const double* __restrict__ y0, const long long N, const PlanArgs A, 
         if (PLACE) {
             cls = cls_of[i];
         } else {
-            cls = plan_class(y0, N, i, A, __longlong_as_double((long long)counters[kCntMeanU2]));
+            const long long n_mean = N < kPlanMeanSample ? N : kPlanMeanSample;
+            cls = plan_class(y0, N, i, A, __longlong_as_double((long long)counters[kCntMeanU2]) / (double)n_mean);
             cls_of[i] = (unsigned char)cls;
         }
     }
@@ -1553,31 +1557,47 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     unsigned char* cls_of = static_cast<unsigned char*>(workspace) + kCounterBytes + order_bytes(N);
     const Ckpt slots = ckpt_at(cls_of + class_bytes(N), cap);
 
-    int bps = 0, sms = 0;
-    int rc = bulk_capacity<TRAP>(&bps, &sms);
-    if (rc) return rc;
-    int dev = 0, smem_optin = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
-        return AIG_ERR_CUDA;
+    // Per device and kernel family, once: resident blocks of the bulk kernel, the shared-memory opt-in of the
+    // streaming block, and a touch of every kernel of the schedule.  (CUDA loads a kernel's code at its first
+    // launch -- lazy module loading -- and loading may have to wait for the kernels that are running: the first
+    // call would serialise the passes that are meant to overlap.)  Later calls find the answers cached: a dozen
+    // runtime queries would otherwise sit in front of every call's first launch.
+    struct Setup {
+        bool done = false;
+        int bps = 0, sms = 0, smem_optin = 0;
+    };
+    static Setup setup_of[64];
+    static std::mutex setup_mutex;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return AIG_ERR_CUDA;
+    int bps = 0, sms = 0, smem_optin = 0;
     {
-        // CUDA loads a kernel's code at its first launch (lazy module loading), and loading may have to
-        // wait for the kernels that are running: the first call would serialise the passes that are meant
-        // to overlap.  Touch every kernel of the schedule before anything is enqueued.
-        cudaFuncAttributes fa;
-        if (cudaFuncGetAttributes(&fa, integrate_kernel<TRAP, kBlock, kBlocksPerSM>) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, integrate_split_kernel<TRAP, kSplitWarps, 1>) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, integrate_split_kernel<TRAP, 1, kSplitMinBlocks>) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, plan_mean_kernel) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, plan_kernel<0>) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, plan_kernel<1>) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, plan_bounds_kernel) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, bounds_kernel) != cudaSuccess ||
-            cudaFuncGetAttributes(&fa, head_start_kernel) != cudaSuccess)
-            return AIG_ERR_CUDA;
-        if (cudaFuncSetAttribute(integrate_split_kernel<TRAP, kSplitWarps, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 smem_optin) != cudaSuccess)
-            return AIG_ERR_CUDA;
+        std::lock_guard<std::mutex> lock(setup_mutex);
+        Setup& su = setup_of[dev];
+        if (!su.done) {
+            const int rc = bulk_capacity<TRAP>(&su.bps, &su.sms);
+            if (rc) return rc;
+            if (cudaDeviceGetAttribute(&su.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+                return AIG_ERR_CUDA;
+            cudaFuncAttributes fa;
+            if (cudaFuncGetAttributes(&fa, integrate_kernel<TRAP, kBlock, kBlocksPerSM>) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, integrate_split_kernel<TRAP, kSplitWarps, 1>) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, integrate_split_kernel<TRAP, 1, kSplitMinBlocks>) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, plan_mean_kernel) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, plan_kernel<0>) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, plan_kernel<1>) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, plan_bounds_kernel) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, bounds_kernel) != cudaSuccess ||
+                cudaFuncGetAttributes(&fa, head_start_kernel) != cudaSuccess)
+                return AIG_ERR_CUDA;
+            if (cudaFuncSetAttribute(integrate_split_kernel<TRAP, kSplitWarps, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     su.smem_optin) != cudaSuccess)
+                return AIG_ERR_CUDA;
+            su.done = true;
+        }
+        bps = su.bps;
+        sms = su.sms;
+        smem_optin = su.smem_optin;
     }
     const bool plan = cfg.plan != 0 && p->C4 > 0.0 && (p->n_att == 0 || p->n_att == 4);  // the Langevin test is the r^-4 tail's
     // the streaming pass: on its own SMs when the work is large enough to fill the others
@@ -1611,7 +1631,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         A.omega = (float)p->omega_rf;
         A.phase0 = (float)std::fmod(p->omega_rf * p->t0, 6.283185307179586);
         const unsigned pg = (unsigned)((N + 255) / 256);
-        plan_mean_kernel<<<1, 1024, 0, st>>>(y0, N, counters);
+        plan_mean_kernel<<<(unsigned)std::min<long long>(64, (N + 1023) / 1024), 1024, 0, st>>>(y0, N, counters);
         plan_kernel<0><<<pg, 256, 0, st>>>(y0, N, A, order, cls_of, counters);
         plan_bounds_kernel<<<1, 1, 0, st>>>(counters, kCntBound, kCntFront);
         plan_kernel<1><<<pg, 256, 0, st>>>(y0, N, A, order, cls_of, counters);
