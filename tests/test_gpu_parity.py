@@ -267,6 +267,23 @@ def test_config0_trajectories(aig):
     assert abs(int(g["complex_flag"].sum()) - int(o["complex_flag"].sum())) <= 3
 
 
+def test_static_trap_trajectories(aig):
+    """The static-trap kernels (q = 0: no cos in the loop; PAPER.md:432 runs a harmonic trap this way) over whole
+    trajectories, through the plan, the bulk pass and both six-lane passes: the config-0 system with a = 0.001, q = 0."""
+    w = inputs.config(0, q_trap=0.0, a_trap=0.001).replace(N=1500 + 3)
+    assert all(x == 0 for x in w.q) and any(x != 0 for x in w.a)
+    y0 = inputs.generate_y0(w)
+    g, o = run_gpu(aig, w, y0), run_orc(w, y0)
+    _compare_direct(w, y0, g, o)
+    try:
+        aig.set_schedule(plan=1, budget=30, tail_iters=2, split_sms=3, mean_factor=0, depth=4, poll_iters=2)
+        g2 = run_gpu(aig, w, y0)
+    finally:
+        aig.set_schedule()
+    for k in g:
+        assert np.array_equal(g[k].view(np.uint8), g2[k].view(np.uint8)), k
+
+
 def test_schedule_invariance(aig):
     """Where a trajectory is integrated (per-thread kernel, six-lane kernel, before or after a
     suspension, queued first or last) never changes its result: every output array is bit-identical
