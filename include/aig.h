@@ -45,6 +45,7 @@ extern "C" {
 #define AIG_ERR_PARAM (-5)     /* masses <= 0, max_steps < 1, non-finite parameter */
 #define AIG_ERR_ALIGN (-6)     /* device pointer not aligned to its element size */
 #define AIG_ERR_CUDA (-7)      /* CUDA runtime error (no device, launch failure, out of memory) */
+#define AIG_ERR_STATIC_LIMIT (-8) /* aig_outliers_static only: N is beyond what its built-in scratch is stated for */
 
 /* status[i] of one trajectory */
 #define AIG_STATUS_EXIT 0      /* r > r_exit after the first radial minimum */
@@ -175,6 +176,34 @@ int aig_observables(const aig_params *p, const double *y0, const aig_out *out, i
 size_t aig_outliers_workspace_bytes(void);
 int aig_outliers(const aig_out *out, const aig_obs_extra *extra, int64_t N, int64_t *result,
                  void *workspace, void *cuda_stream);
+
+/* ---- aig_outliers without a workspace: for callers that must not allocate device memory -------------
+ * Some users of this library run where device memory is not theirs to ask for: an analysis hook inside a
+ * long ensemble run whose host program handed out all of the GPU's memory at start-up and wants no
+ * cudaMalloc afterwards (it synchronises the whole device and can fail hours into a run), a plug-in of a
+ * framework that owns the allocator, a service with a fixed memory plan.  They can pass the observable
+ * arrays they already hold and an [8][2] result, but have nowhere to take aig_outliers' workspace from.
+ * aig_outliers_static is aig_outliers (same kernel, same result rows, same tie and NaN rules,
+ * PAPER.md:521) with the scratch -- one ticket counter and the per-block partial extrema -- kept in an
+ * array that is part of the library itself: AIG_OUTLIERS_STATIC_SCRATCH_BYTES (131,328) bytes of device
+ * memory on every GPU that loads libaig, held until the process exits, enough for a grid of 512 blocks.
+ *   - The call itself allocates and frees nothing (no cudaMalloc / cudaFree, no library routine that
+ *     does); it enqueues one 256-byte memset and one kernel on `cuda_stream`.
+ *   - Limit: N <= AIG_OUTLIERS_STATIC_MAX_N (2^28 trajectories, 64 times the largest ensemble of
+ *     BASELINE.json); a larger N returns AIG_ERR_STATIC_LIMIT before anything touches the device -- use
+ *     aig_outliers with a workspace of your own for that.  N = 0 is valid (every row -1, -1).
+ *   - The first call on each device looks up the array's device address (once per device, with that device
+ *     current, kept afterwards).  Make that first call outside any stream capture.
+ *   - All calls on a device share the one array, and it keeps what the previous call left in it; each call
+ *     zeroes the counter it needs, in stream order.  Two calls whose kernels can overlap on the GPU
+ *     (different streams, or different host threads on different streams) race on it and give wrong
+ *     indices: keep calls on one device in one stream order.  aig_outliers has no such restriction.
+ * out, extra, result: as for aig_outliers (HOST structs of DEVICE pointers; result DEVICE int64 [8][2]). */
+#define AIG_OUTLIERS_STATIC_MAX_N (1LL << 28)
+#define AIG_OUTLIERS_STATIC_SCRATCH_BYTES 131328
+int64_t aig_outliers_static_max_n(void);
+int aig_outliers_static(const aig_out *out, const aig_obs_extra *extra, int64_t N, int64_t *result,
+                        void *cuda_stream);
 
 /* ---- NEXT-3: replay of one trajectory, every accepted step recorded ---------------
  * the paper simulates its longest-lived (or a custom) trajectory again "with

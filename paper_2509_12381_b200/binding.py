@@ -19,7 +19,7 @@ _lib = None
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
            "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_set_schedule", "aig_strerror",
            "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes", "aig_trace",
-           "aig_set_schedule_ex", "aig_get_schedule", "aig_map2d"]
+           "aig_set_schedule_ex", "aig_get_schedule", "aig_map2d", "aig_outliers_static", "aig_outliers_static_max_n"]
 
 
 class AigError(RuntimeError):
@@ -236,6 +236,31 @@ def aig_outliers(obs, extra, stream=None):
     _check(L.aig_outliers(C.byref(o), C.byref(e), N, res.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "aig_outliers")
     res._ws = ws  # keep the scratch alive until the stream has run
     return res
+
+
+def aig_outliers_static(obs, extra, result, stream=None):
+    """aig_outliers through the library's built-in scratch (include/aig.h): nothing is allocated here or in the
+    library, so the caller passes ``result``, an int64 CUDA tensor [8, 2] of its own, and gets it back.  For callers
+    that hold their arrays already and may not ask for more device memory.  Calls on one device must not overlap
+    (one shared scratch); raises for N beyond aig_outliers_static_max_n()."""
+    torch = _torch()
+    N = obs["angle"].numel()
+    assert result.is_cuda and result.dtype == torch.int64 and tuple(result.shape) == (len(OUTLIER_KEYS), 2)
+    assert result.is_contiguous()
+    L = lib()
+    L.aig_outliers_static.restype = C.c_int
+    L.aig_outliers_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    e = _extra_struct(extra)
+    o = _out_struct(obs)
+    _check(L.aig_outliers_static(C.byref(o), C.byref(e), N, result.data_ptr(), _stream_ptr(stream)),
+           "aig_outliers_static")
+    return result
+
+
+def aig_outliers_static_max_n() -> int:
+    L = lib()
+    L.aig_outliers_static_max_n.restype = C.c_int64
+    return int(L.aig_outliers_static_max_n())
 
 
 class MapSpec(C.Structure):

@@ -1784,6 +1784,9 @@ const char* aig_strerror(int code)
         case AIG_ERR_PARAM: return "invalid physical parameter";
         case AIG_ERR_ALIGN: return "misaligned device pointer";
         case AIG_ERR_CUDA: return "CUDA runtime error (no device, launch failure or out of memory)";
+        case AIG_ERR_STATIC_LIMIT:
+            return "N exceeds AIG_OUTLIERS_STATIC_MAX_N, the stated limit of aig_outliers_static's built-in scratch "
+                   "(use aig_outliers with a caller workspace)";
         default: return "unknown error code";
     }
 }
@@ -2190,6 +2193,93 @@ int aig_kernel_info(int* sm_count, int* blocks_per_sm, int* threads_per_block, i
     if (regs_per_thread) *regs_per_thread = fa.numRegs;
     if (local_bytes_per_thread) *local_bytes_per_thread = (int)fa.localSizeBytes;
     return AIG_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// aig_outliers_static: the arg-min / arg-max pass for callers that may not allocate (include/aig.h)
+// ------------------------------------------------------------------------------------------
+// The per-block partial extrema and the ticket counter of outliers_kernel live in an array that is part of
+// the library image instead of a caller workspace.  Every device that loads libaig holds these bytes from
+// module load until the process exits; every call on a device uses the same bytes.
+namespace {
+
+constexpr int kOutlierStaticBlocks = 512;  // grid cap of the static variant (aig_outliers itself: 1024)
+constexpr size_t kOutlierStaticBytes = 256 + (size_t)kOutlierStaticBlocks * kOutlierObs * 2 * sizeof(Extreme);  // 131,328
+static_assert(kOutlierStaticBytes == AIG_OUTLIERS_STATIC_SCRATCH_BYTES, "include/aig.h states the size of the static scratch");
+
+static __device__ __align__(256) unsigned char g_outlier_scratch[kOutlierStaticBytes];
+
+// In host code `g_outlier_scratch` names a host-side shadow of the array, not memory a kernel can use: the
+// device address has to be asked for, separately on every device (each holds its own copy).  Looked up at the
+// first call on a device, with that device current, and kept.
+unsigned char* outlier_static_scratch(int* rc)
+{
+    static unsigned char* ptr_of[64];
+    static std::mutex lookup_mutex;
+    int dev = 0;
+    *rc = AIG_ERR_CUDA;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(lookup_mutex);
+    if (!ptr_of[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_outlier_scratch) != cudaSuccess || !p) {
+            (void)cudaGetLastError();
+            return nullptr;
+        }
+        ptr_of[dev] = static_cast<unsigned char*>(p);
+    }
+    *rc = AIG_OK;
+    return ptr_of[dev];
+}
+
+}  // namespace
+
+extern "C" {
+
+int64_t aig_outliers_static_max_n(void) { return AIG_OUTLIERS_STATIC_MAX_N; }
+
+int aig_outliers_static(const aig_out* out, const aig_obs_extra* extra, int64_t N, int64_t* result, void* cuda_stream)
+{
+    if (!result) return AIG_ERR_NULL;
+    if (N < 0) return AIG_ERR_SIZE;
+    if (N > AIG_OUTLIERS_STATIC_MAX_N) return AIG_ERR_STATIC_LIMIT;
+    if (!aligned(result, 8)) return AIG_ERR_ALIGN;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (N > 0) {
+        if (!out || !extra) return AIG_ERR_NULL;
+        if (!out->angle || !out->lifetime || !out->n_turn || !out->n_acc || !extra->dist || !extra->KE || !extra->transfer)
+            return AIG_ERR_NULL;
+    }
+    int rc = AIG_OK;
+    unsigned char* scratch = outlier_static_scratch(&rc);  // first call on this device: the address look-up
+    if (!scratch) return rc;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AIG_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return AIG_ERR_CUDA;
+    // the array still holds the previous call's ticket count and partials: the ticket must start at zero (the
+    // partials of the blocks of this launch are all rewritten before the last block reads them)
+    if (cudaMemsetAsync(scratch, 0, 256, st) != cudaSuccess) return AIG_ERR_CUDA;
+    OutlierArgs a;
+    a.angle = N ? out->angle : nullptr;
+    a.lifetime = N ? out->lifetime : nullptr;
+    a.n_turn = N ? out->n_turn : nullptr;
+    a.n_acc = N ? out->n_acc : nullptr;
+    a.transfer = N ? extra->transfer : nullptr;
+    a.dist = N ? extra->dist : nullptr;
+    a.ke = N ? extra->KE : nullptr;
+    a.position = N ? extra->position : nullptr;
+    a.ticket = reinterpret_cast<unsigned int*>(scratch);
+    a.partial = reinterpret_cast<Extreme*>(scratch + 256);
+    a.result = reinterpret_cast<long long*>(result);
+    int occ = 0;  // one wave of resident blocks, as in aig_outliers, and never more than the array has room for
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, outliers_kernel, 256, 0) != cudaSuccess || occ < 1) return AIG_ERR_CUDA;
+    const long long blocks = std::min<long long>(std::max<long long>(1, (N + 255) / 256),
+                                                 std::min<long long>((long long)sms * occ, kOutlierStaticBlocks));
+    outliers_kernel<<<(unsigned)blocks, 256, 0, st>>>(a, N);
+    g_kernel_launches++;
+    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
 }
 
 }  // extern "C"
