@@ -883,6 +883,25 @@ def test_degenerate_inputs(aig):
     g3, o3 = run_gpu(aig, w3, y0[:, :1].copy()), run_orc(w3, y0[:, :1].copy(), threads=1)
     assert g3["status"][0] == 1 and g3["t_final"][0] == 3e10 and o3["status"][0] == 1
     assert block_rel(g3["y_final"], o3["y_final"]).max() < 1e-6
+    # an atom that starts at R0 moving AWAY from the ion in free motion never has a radial minimum: the exit radius
+    # must not stop it (BASELINE.json configs[0]: "after the first inner turning point"); it runs to t_max exactly,
+    # no turning point, r_min = the distance at t0, the straight line, ode45's x5 step sequence (same count as the
+    # oracle, whose own pin is tests/test_oracle_pins.py::test_receding_atom_never_exits_before_a_radial_minimum)
+    kw = dict(m_ion=138 * inputs.AMU, m_atom=87 * inputs.AMU, C4=0.0, C8=0.0, a=(0, 0, 0), q=(0, 0, 0), omega_rf=0.0,
+              r_exit=5050.0)
+    yr = np.array([0, 0, 0, 1e-8, -2e-8, 5e-9, 4000.0, 3000.0, 0.0, 2.4e-7, 1.6e-7, 1e-8]).reshape(12, 1)
+    yr = np.concatenate([yr, yr], axis=1)
+    yr[9:12, 1] = [-2.4e-7, -1.6e-7, 1e-8]          # the same start moving inwards: stops beyond r_exit after its minimum
+    t_max, rtol, atol = 2e11, 1e-10, 1e-12
+    gr = _host(aig.aig_integrate(aig.make_params(**kw), _dev(yr), t_max, rtol, atol))
+    orr = orc.integrate(orc.make_params(**kw), yr, t_max, rtol, atol)
+    assert gr["status"][0] == 1 and gr["t_final"][0] == t_max and gr["n_turn"][0] == 0 and gr["r_min"][0] == 5000.0
+    assert gr["complex_flag"][0] == 0 and gr["lifetime"][0] == 0.0 and gr["n_rej"][0] == 0
+    assert gr["n_acc"][0] == orr["n_acc"][0] and gr["n_acc"][1] == orr["n_acc"][1]
+    d_end = (yr[6:9, 0] - yr[0:3, 0]) + (yr[9:12, 0] - yr[3:6, 0]) * t_max
+    assert np.max(np.abs((gr["y_final"][6:9, 0] - gr["y_final"][0:3, 0]) - d_end)) <= 1e-12 * np.linalg.norm(d_end)
+    assert gr["status"][1] == 0 and gr["n_turn"][1] == 1 and gr["t_final"][1] == orr["t_final"][1]
+    assert block_rel(gr["y_final"], orr["y_final"]).max() < 1e-12
 
 
 def test_argument_errors(aig):

@@ -395,6 +395,49 @@ def test_free_motion_exact_and_step_sequence():
     assert o["t_final"][0] == tt[-1]
 
 
+def test_receding_atom_never_exits_before_a_radial_minimum():
+    """BASELINE.json configs[0]: stop when r > 1.01 R0 "after the first inner turning point".  An atom that starts
+    at R0 already moving AWAY from the ion (d.u > 0 at t0) in free motion has no radial minimum at all: it must
+    not be stopped when it crosses r_exit but run to t_max exactly (status 1), with no turning point, r_min equal
+    to the distance at t0 (the smallest it ever is), the straight-line final state, and ode45's hand-computable
+    step sequence (h0 from the initial-step rule, x5 per accepted step, capped at hmax, the last step stretched
+    to land on t_max)."""
+    p = orc.make_params(138 * inputs.AMU, 87 * inputs.AMU, 0.0, 0.0, (0, 0, 0), (0, 0, 0), 0.0, r_exit=5050.0)
+    y0 = np.array([0, 0, 0, 1e-8, -2e-8, 5e-9, 4000.0, 3000.0, 0.0, 2.4e-7, 1.6e-7, 1e-8])
+    d0, u = y0[6:9] - y0[0:3], y0[9:12] - y0[3:6]
+    assert d0 @ u > 0 and np.linalg.norm(d0) == 5000.0
+    t_max, rtol, atol = 2e11, 1e-10, 1e-12
+    o = orc.integrate(p, y0.reshape(12, 1), t_max, rtol, atol)
+    tt, yy, st = orc.integrate_trace(p, y0, t_max, rtol, atol)
+    assert st == 1 and o["status"][0] == 1 and o["t_final"][0] == t_max and tt[-1] == t_max
+    assert o["n_turn"][0] == 0 and o["complex_flag"][0] == 0 and o["lifetime"][0] == 0.0 and o["n_rej"][0] == 0
+    assert o["r_min"][0] == 5000.0
+    d_end = d0 + u * t_max
+    assert np.linalg.norm(d_end) > 10 * 5050.0          # far beyond the exit radius, and still not stopped
+    got = o["y_final"][6:9, 0] - o["y_final"][0:3, 0]
+    assert np.max(np.abs(got - d_end)) <= 1e-12 * np.linalg.norm(d_end)
+    assert o["angle"][0] < 1e-15
+    thr = atol / rtol
+    f0 = np.concatenate([y0[3:6], np.zeros(3), y0[9:12], np.zeros(3)])
+    rho = np.max(np.abs(f0) / np.maximum(np.abs(y0), thr)) / (0.8 * rtol**0.2)
+    h, hmax, t, times = 1.0 / rho, 0.1 * t_max, 0.0, []
+    while True:
+        h = min(h, hmax)
+        if 1.1 * h >= t_max - t:
+            times.append(t_max)
+            break
+        t = t + h
+        times.append(t)
+        h = 5.0 * h
+    assert len(times) == len(tt) == o["n_acc"][0]
+    assert np.allclose(tt, times, rtol=1e-12)
+    # the same start moving inwards does stop, at the first step end beyond r_exit after its closest approach
+    yin = y0.copy()
+    yin[9:12] = [-2.4e-7, -1.6e-7, 1e-8]
+    oi = orc.integrate(p, yin.reshape(12, 1), t_max, rtol, atol)
+    assert oi["status"][0] == 0 and oi["t_final"][0] < t_max and oi["n_turn"][0] == 1
+
+
 # ------------------------------------------------------------------------------------------
 # trap term: the paper's harmonic recipe (PAPER.md:432) and Mathieu theory
 # ------------------------------------------------------------------------------------------
@@ -548,6 +591,45 @@ def test_deflection_angle_matches_quadrature():
         assert o["r_min"][i] >= rmin - 1e-9 and o["r_min"][i] < rmin * 1.05
         checked += 1
     assert checked >= 10
+
+
+def test_angle_is_the_atoms_lab_frame_deflection_ion_at_rest():
+    """`angle` is "the scattering angle of the atom": the turn of the ATOM's velocity in the frame
+    the state is given in, not the ion's and not the relative velocity's.  Config 1 runs in the centre-of-mass
+    frame, where both particles turn by the same angle, so it cannot tell them apart.  Here the same collisions
+    are boosted to the frame in which the ion starts AT REST (trap off: Galilean invariance).  With u = v_atom -
+    v_ion turned by chi (quadrature) and |u_f|^2 = |u_0|^2 + 2 (V(R0) - V(r_f)) / mu, the atom's velocity is
+    v_cm + (m_i / M) u with v_cm = (m_a / M) u_0, hence
+        angle = atan2(|u_f| sin chi, |u_f| cos chi + (m_a / m_i) |u_0|).
+    The ion's own velocity starts at zero (angle 0 by atan2(0, 0)) and the relative velocity turns by chi: an
+    oracle that took either fails by O(1) rad."""
+    w = inputs.config(1)
+    n = 64
+    p = orc.make_params(**w.params())
+    y0 = inputs.generate_y0(w, n=n).copy()
+    v_ion0 = y0[3:6].copy()
+    y0[3:6] -= v_ion0
+    y0[9:12] -= v_ion0
+    assert np.all(y0[3:6] == 0.0)
+    o = orc.integrate(p, y0, w.t_max, w.rtol, w.atol)
+    b = inputs.impact_parameters(w, n=n)
+    bc = (4 * w.C4 / w.E_coll) ** 0.25
+    mu = w.m_ion * w.m_atom / (w.m_ion + w.m_atom)
+    V = lambda r: -w.C4 / r**4 + w.C8 / r**8
+    checked, apart = 0, 0
+    for i in range(n):
+        if b[i] < 1.01 * bc:
+            continue
+        assert o["status"][i] == 0
+        rf = np.linalg.norm(o["y_final"][6:9, i] - o["y_final"][0:3, i])
+        chi, _ = _deflection_quadrature(w, b[i], rf)
+        u0 = np.linalg.norm(y0[9:12, i])
+        uf = math.sqrt(u0 * u0 + 2.0 * (V(w.R0) - V(rf)) / mu)
+        want = math.atan2(uf * math.sin(chi), uf * math.cos(chi) + (w.m_atom / w.m_ion) * u0)
+        assert abs(o["angle"][i] - want) < 1e-8, (i, b[i], o["angle"][i], want, chi)
+        apart += abs(want - chi) > 1e-3 and want > 1e-3     # the three candidate angles really differ here
+        checked += 1
+    assert checked >= 10 and apart >= 10
 
 
 def test_captured_deflection_converges_with_tolerance():
