@@ -233,14 +233,22 @@ int aig_run_host(const aig_params *p, const double *y0_host, int64_t N, double t
                  double atol, const aig_out *out_host, const aig_hist_spec *hist_spec_host,
                  const aig_hist *hist_out_host);
 
-/* NEXT-2: an observable against the launch direction (the paper's heatmaps).
- * The direction of trajectory i is that of x_atom - x_ion at t0 (rows 6-8 minus rows 0-2 of y0): u = (1 - cos theta)/2
- * in [0, 1] (equal steps of u are equal solid angles, eq. (12)-(13) at PAPER.md:92-98) and phi = atan2(dy, dx) brought
- * into [0, 2 pi).  Cells are given by explicit edges (DEVICE pointers, strictly increasing, n + 1 of them, n in 1..4096
- * each): cell (a, b) holds u_edges[a] <= u < u_edges[a+1], phi_edges[b] <= phi < phi_edges[b+1].  For every trajectory
- * inside the window whose value is not NaN: count[a * n_phi + b] += 1, sum[a * n_phi + b] += value[i] (DEVICE arrays
- * of n_u * n_phi, ACCUMULATED into: the caller zeroes them; sum / count is the map).  On a "uniform" grid workload
- * with edges half-way between the grid directions the map is the value array reshaped to [ntheta][nphi]. */
+/* NEXT-2: an observable against the launch direction (the paper's heatmaps, PAPER.md:483, :517:
+ * "as a function of the spherical angles theta and phi", the "(theta, phi) for the initial conditions of the atom").
+ * The direction of trajectory i is that of the ATOM's position at t0, rows 6-8 of y0 alone (about the trap centre; a
+ * thermally displaced ion does not shift the cells): u = (1 - cos theta)/2 in [0, 1] (equal steps of u are equal solid
+ * angles, eq. (12)-(13) at PAPER.md:92-98) and phi = atan2(y, x) brought into [phi_edges[0], phi_edges[0] + 2 pi), so a
+ * window may straddle phi = 0 (edges from -0.5 to 0.5, say); the edges must span at most one turn.  Cells are given by
+ * explicit edges (DEVICE pointers, strictly increasing, n + 1 of them, n in 1..4096 each): cell (a, b) holds
+ * u_edges[a] <= u < u_edges[a+1], phi_edges[b] <= phi < phi_edges[b+1].  For every trajectory inside the window whose
+ * value is not NaN: count[a * n_phi + b] += 1, sum[a * n_phi + b] += value[i] (DEVICE arrays of n_u * n_phi,
+ * ACCUMULATED into: the caller zeroes them; sum / count is the map).  An atom AT the origin has no direction and is
+ * skipped.  At a pole (theta = 0 or pi) phi is undefined and read as 0: on a "uniform" grid whose theta window
+ * starts at 0 (the paper's default octant) the nphi trajectories of that row are one and the same launch point and all
+ * land in the cell that holds phi = 0.  Such a grid is index-ordered (i = theta index * nphi + phi index), so its map
+ * is simply the value array viewed as [ntheta][nphi], which is what the paper does; aig_map2d is for "random"
+ * positions and for re-binning.  Away from the poles, with edges half-way between the grid directions, the map of a
+ * grid workload equals that view (head-on or "thermal"). */
 typedef struct aig_map_spec {
     const double *u_edges;
     int32_t n_u;

@@ -319,20 +319,25 @@ def outliers(obs: dict) -> dict:
 
 
 def map2d(y0, value, u_edges, phi_edges):
-    """PAPER.md:483, :517 (an observable against the launch direction), as a definition: the direction of
-    trajectory i is that of x_atom - x_ion at t0; u = (1 - cos theta)/2, phi = atan2(dy, dx) in [0, 2 pi); cell
-    (a, b) holds u_edges[a] <= u < u_edges[a+1], phi_edges[b] <= phi < phi_edges[b+1].  Returns (count, sum) of the
-    non-NaN values inside the window, [n_u][n_phi].  Plain loop."""
+    """PAPER.md:483, :517 (an observable "as a function of the spherical angles theta and phi", the "(theta, phi) for
+    the initial conditions of the atom"), as a definition: the direction of trajectory i is that of the ATOM's
+    position at t0 (rows 6-8 alone, about the trap centre; the ion's thermal displacement does not enter);
+    u = (1 - cos theta)/2, phi = atan2(y, x) brought into [phi_edges[0], phi_edges[0] + 2 pi) (a window may straddle
+    phi = 0; at a pole x = y = 0 and phi = atan2(0, 0) = 0); cell (a, b) holds u_edges[a] <= u < u_edges[a+1],
+    phi_edges[b] <= phi < phi_edges[b+1].  Returns (count, sum) of the non-NaN values inside the window,
+    [n_u][n_phi].  Plain loop."""
     y0 = np.asarray(y0, dtype=np.float64)
     ue, pe = np.asarray(u_edges, dtype=np.float64), np.asarray(phi_edges, dtype=np.float64)
     nu, nph = len(ue) - 1, len(pe) - 1
     count = np.zeros((nu, nph), dtype=np.int64)
     total = np.zeros((nu, nph), dtype=np.float64)
-    d = y0[6:9] - y0[0:3]
+    d = y0[6:9]
     r = np.sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2])
-    u = 0.5 * (1.0 - d[2] / r)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        u = 0.5 * (1.0 - d[2] / r)
     phi = np.arctan2(d[1], d[0])
-    phi = np.where(phi < 0.0, phi + 2.0 * np.pi, phi)
+    two_pi = 2.0 * np.pi
+    phi = phi - two_pi * np.floor((phi - pe[0]) / two_pi)
     a = np.searchsorted(ue, u, side="right")
     b = np.searchsorted(pe, phi, side="right")
     for i in range(y0.shape[1]):

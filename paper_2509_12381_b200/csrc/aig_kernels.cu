@@ -1284,7 +1284,7 @@ outliers_kernel(const OutlierArgs a, const long long N)
 // ------------------------------------------------------------------------------------------
 // NEXT-2: an observable against the launch direction
 // ------------------------------------------------------------------------------------------
-// HBM-bound: 56 B read per trajectory; one global atomic pair per trajectory inside the window (thousands of
+// HBM-bound: 32 B read per trajectory; one global atomic pair per trajectory inside the window (thousands of
 // cells: little contention).  Edges are searched in global memory (L1-resident: a few KB).
 __global__ void __launch_bounds__(256)
 map2d_kernel(const double* __restrict__ y0, const long long N, const double* __restrict__ value,
@@ -1292,14 +1292,15 @@ map2d_kernel(const double* __restrict__ y0, const long long N, const double* __r
              unsigned long long* __restrict__ count, double* __restrict__ sum)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
+    const double two_pi = 6.283185307179586, phi0 = phi_edges[0];
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
         const double v = value[i];
-        const double dx = y0[6 * N + i] - y0[0 * N + i], dy = y0[7 * N + i] - y0[1 * N + i],
-                     dz = y0[8 * N + i] - y0[2 * N + i];
+        // the spherical angles of the atom's initial position; r = 0 gives u = NaN: skipped
+        const double dx = y0[6 * N + i], dy = y0[7 * N + i], dz = y0[8 * N + i];
         const double r = sqrt(sum3(dx * dx, dy * dy, dz * dz));
         const double u = 0.5 * (1.0 - dz / r);
-        double phi = atan2(dy, dx);
-        if (phi < 0.0) phi += 6.283185307179586;
+        double phi = atan2(dy, dx);  // a pole (dx = dy = 0) reads phi = 0
+        phi = phi - two_pi * floor((phi - phi0) / two_pi);  // into [phi0, phi0 + 2 pi): a window may straddle 0
         const int a = bin_of(u_edges, n_u, u), b = bin_of(phi_edges, n_phi, phi);  // 0 / n + 1: outside (NaN too)
         if (a >= 1 && a <= n_u && b >= 1 && b <= n_phi && v == v) {
             const long long cell = (long long)(a - 1) * n_phi + (b - 1);

@@ -996,7 +996,7 @@ def test_map2d_observable_against_launch_direction(aig):
     val[::97] = float("nan")
     ue, pe = inputs.map_edges(w, 24, 40)
     ue, pe = ue[2:-3].copy(), pe[1:-4].copy()           # a window smaller than the data: some directions fall outside
-    d = y0[6:9] - y0[0:3]
+    d = y0[6:9]                                          # the atom's own position
     u = 0.5 * (1 - d[2] / np.linalg.norm(d, axis=0))
     phi = np.mod(np.arctan2(d[1], d[0]), 2 * math.pi)
     assert np.min(np.abs(u[:, None] - ue[None, :])) > 1e-12 and np.min(np.abs(phi[:, None] - pe[None, :])) > 1e-12
@@ -1014,6 +1014,35 @@ def test_map2d_observable_against_launch_direction(aig):
     cg, tg = aig.aig_map2d(_dev(yg), _dev(vg), _dev(ueg), _dev(peg))
     assert np.array_equal(cg.cpu().numpy(), np.ones((12, 17), dtype=np.int64))
     assert np.array_equal(tg.cpu().numpy(), vg.reshape(12, 17))
+    # the paper's default octant (theta from 0: row 0 is the pole, nphi coincident launch points that all read phi = 0)
+    # with the "thermal" collision type (ion displaced from the trap centre: must not shift a cell), and a phi window
+    # that straddles 0 on random directions: counts and sums equal to the definition
+    wt = inputs.paper_workload(ntheta=31, nphi=23, collisiontype="thermal")
+    yt = inputs.generate_y0(wt)
+    assert np.max(np.abs(yt[0:3])) > 0.0
+    vt = np.arange(wt.N, dtype=float) + 0.25
+    uet, pet = inputs.map_edges(wt)
+    ct, tt = aig.aig_map2d(_dev(yt), _dev(vt), _dev(uet), _dev(pet))
+    want_c = np.ones((31, 23), dtype=np.int64)
+    want_c[0] = 0
+    want_c[0, 0] = 23
+    want_t = vt.reshape(31, 23).copy()
+    want_t[0] = 0.0
+    want_t[0, 0] = vt[:23].sum()
+    assert np.array_equal(ct.cpu().numpy(), want_c) and np.array_equal(tt.cpu().numpy(), want_t)
+    c_ref, t_ref = orc.map2d(yt, vt, uet, pet)
+    assert np.array_equal(c_ref, want_c) and np.array_equal(t_ref, want_t)
+    ws = inputs.paper_workload(ntheta=97, nphi=41, theta=(0.1, 3.0), phi=(0.0, 2 * math.pi), positions="random")
+    ys = inputs.generate_y0(ws)
+    pes = np.linspace(-0.7, 0.9, 9)
+    ues = np.linspace(0.05, 0.95, 7)
+    phis = np.arctan2(ys[7], ys[6])
+    assert np.min(np.abs(phis[:, None] - pes[None, :])) > 1e-12 and np.min(np.abs(phis[:, None] + 2 * math.pi - pes[None, :])) > 1e-12
+    vs = np.cos(np.arange(ws.N))
+    cs, ts = aig.aig_map2d(_dev(ys), _dev(vs), _dev(ues), _dev(pes))
+    c_ref, t_ref = orc.map2d(ys, vs, ues, pes)
+    assert np.array_equal(cs.cpu().numpy(), c_ref) and c_ref[:, :4].sum() > 100 and c_ref[:, 4:].sum() > 100
+    assert np.allclose(ts.cpu().numpy(), t_ref, rtol=1e-12, atol=1e-12)
     # N = 0
     e12 = torch.empty((12, 0), dtype=torch.float64, device="cuda")
     c0, _ = aig.aig_map2d(e12, torch.empty(0, dtype=torch.float64, device="cuda"), _dev(ueg), _dev(peg))

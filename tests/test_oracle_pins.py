@@ -998,9 +998,9 @@ def test_lennard_jones_6_12_conserves_energy_and_angular_momentum():
 def test_map2d_hand_directions_and_grid_reshape():
     # six axis directions: +z is u = 0, -z is u = 1, the equator u = 1/2 with phi = 0, pi/2, pi, 3 pi/2
     y0 = np.zeros((12, 6))
-    y0[0:3] = np.array([[1.0, 2.0, 3.0]]).T                      # the ion is not at the origin: the direction is relative
+    y0[0:3] = np.array([[1.0, 2.0, 3.0]]).T      # the ion is not at the origin: the angles are the ATOM's
     for i, d in enumerate([(0, 0, 1), (0, 0, -1), (1, 0, 0), (0, 1, 0), (-1, 0, 0), (0, -1, 0)]):
-        y0[6:9, i] = y0[0:3, i] + 7.0 * np.array(d)
+        y0[6:9, i] = 7.0 * np.array(d)
     ue = np.array([0.0, 0.25, 0.75, 1.0 + 1e-12])
     pe = np.array([0.0, 1.0, 2.0, 4.0, 2 * math.pi])
     val = np.array([1.0, 2.0, 4.0, 8.0, 16.0, float("nan")])
@@ -1019,6 +1019,33 @@ def test_map2d_hand_directions_and_grid_reshape():
     ue, pe = inputs.map_edges(w)
     count, total = orc.map2d(y0, val, ue, pe)
     assert np.array_equal(count, np.ones((7, 9), dtype=np.int64)) and np.array_equal(total, val.reshape(7, 9))
+    # ... also for the "thermal" collision type, whose ion is displaced from the trap centre: the cells
+    # are those of the atom's own position, so the displacement must not move any trajectory to another cell
+    wt = inputs.paper_workload(ntheta=7, nphi=9, theta=(0.3, 1.4), phi=(0.2, 1.3), collisiontype="thermal")
+    yt = inputs.generate_y0(wt)
+    assert np.max(np.abs(yt[0:3])) > 0.0
+    count, total = orc.map2d(yt, val, ue, pe)
+    assert np.array_equal(count, np.ones((7, 9), dtype=np.int64)) and np.array_equal(total, val.reshape(7, 9))
+    # the paper's default octant starts at theta = 0: the nphi launch points of row 0 are one point, the pole, where
+    # phi reads 0 -- they all fall in the cell of phi = 0; every other row is the reshape
+    wp = inputs.paper_workload(ntheta=6, nphi=5)
+    yp = inputs.generate_y0(wp)
+    vp = np.arange(wp.N, dtype=float) + 0.5
+    count, total = orc.map2d(yp, vp, *inputs.map_edges(wp))
+    want_c = np.ones((6, 5), dtype=np.int64)
+    want_c[0] = [5, 0, 0, 0, 0]
+    want_t = vp.reshape(6, 5).copy()
+    want_t[0] = [vp[:5].sum(), 0, 0, 0, 0]
+    assert np.array_equal(count, want_c) and np.array_equal(total, want_t)
+    # a phi window that straddles 0: directions at phi = -0.3, 0.3 and 6.0 (= -0.283...) with edges [-0.5, 0, 0.5]
+    ys = np.zeros((12, 3))
+    for i, f in enumerate((-0.3, 0.3, 6.0)):
+        ys[6:9, i] = [math.cos(f), math.sin(f), 0.0]
+    count, total = orc.map2d(ys, np.array([1.0, 2.0, 4.0]), np.array([0.0, 1.0]), np.array([-0.5, 0.0, 0.5]))
+    assert np.array_equal(count, [[2, 1]]) and np.array_equal(total, [[5.0, 2.0]])
+    # an atom at the origin has no direction: skipped
+    count, _ = orc.map2d(np.zeros((12, 1)), np.ones(1), np.array([0.0, 1.0]), np.array([0.0, 7.0]))
+    assert count.sum() == 0
 
 
 def test_map2d_equal_solid_angle_cells_fill_uniformly():
