@@ -213,14 +213,16 @@ def _compare_direct(w, y0, g, o, tol=1e-6, kw=None):
     """north_star: on direct (non-complex) trajectories accepted step counts agree to +-2 and final
     states to <= 1e-6.  'Direct' = at most one turning point, stopped on the exit radius.
       * far (never inside the short-range well): final states <= 1e-6 at a common time, angle <= 1e-6,
-        stop times within one maximal step of each other; r_min (a step-end sample) <= 1e-6 where both
-        runs sampled at the same times;
+        stop times equal up to the step-size noise when the step counts agree (>= 95 % of them) and one
+        actual step apart otherwise; r_min (a step-end sample) on all of them within the relative time
+        shift, <= 1e-6 where both runs sampled at the same times;
       * single bounces that reach the well (r ~ 7.6 a0): there the method's truncation error is amplified
         by many orders of magnitude (the oracle at these tolerances is 1e-3 .. 1 away from a DOP853
         solution at rtol = 1e-13) and so is every rounding: the CUDA path must be (a) as close to the
         DOP853 solution as the oracle is (never more than twice as far), and (b) no farther from the
         oracle than twice what the oracle's own answer moves under a 1-ulp change of y0 (median and 90 %
-        quantile of the sample)."""
+        quantile of the sample; the maximum within 15x the oracle's maximum).  What happens BEFORE the
+        amplification is compared pointwise in test_pre_bounce_pointwise_parity."""
     kw = kw or w.params()
     p = orc.make_params(**kw)
     y1 = y0.copy()
@@ -237,18 +239,37 @@ def _compare_direct(w, y0, g, o, tol=1e-6, kw=None):
     assert far.sum() > 0.2 * len(far)
     rel = _final_state_rel(w, g, o, direct, kw)
     assert rel[far].max() <= tol, rel[far].max()
-    # a step is at most hmax = (t_max - t0) / 10 long: the two stops are within one step of each other
-    assert np.max(np.abs(g["t_final"][far] - o["t_final"][far])) <= 0.1 * (w.t_max - p.t0)
+    # Stop times.  The exit stop is a step-end test, and the step sizes of two correct runs differ by the rounding
+    # of the error estimate (a cancelling sum, 1e-3 relative: DESIGN.md "Parity metric"), more so when rtol sits
+    # near the rounding level of that sum.  Same number of steps: the two stops are the same step end, up to that
+    # noise (measured: <= 1e-5 of t at rtol >= 1e-10, 2e-3 at rtol 1e-12).  One step apart (the last step end of
+    # one run fell just inside r_exit): the difference is that one step, whose size the oracle's replay gives.
+    dt = np.abs(g["t_final"] - o["t_final"])
+    eq = far & (g["n_acc"] == o["n_acc"])
+    assert eq.sum() >= 0.95 * far.sum(), (eq.sum(), far.sum())
+    assert np.max(dt[eq] / o["t_final"][eq]) <= (1e-4 if w.rtol >= 1e-10 else 1e-2), np.max(dt[eq] / o["t_final"][eq])
+    for i in np.flatnonzero(far & ~eq)[:200]:
+        tt, _, _ = orc.integrate_trace(p, y0[:, i], w.t_max, w.rtol, w.atol)
+        h_last = tt[-1] - tt[-2]
+        assert dt[i] <= 5.0 * 1.01 * h_last, (i, dt[i], h_last)          # a step grows by at most x5 (ode45)
     # final velocities are asymptotic: the angle does not depend on the stop time
     assert np.max(np.abs(g["angle"][far] - o["angle"][far])) <= 1e-6
-    same = far & (g["n_acc"] == o["n_acc"]) & (np.abs(g["t_final"] / o["t_final"] - 1) <= 1e-6)
+    # r_min is a sample of r at step ends: on EVERY far trajectory that took the same number of steps it moves with
+    # the step times by no more than the relative time shift (|dr/dt| t / r <~ 1 around the closest approach), and
+    # to 1e-6 where the times agree to 1e-6; a run one step longer or shorter elsewhere samples other instants
+    rr = np.abs(g["r_min"] / o["r_min"] - 1)
+    assert np.all(rr[eq] <= 1e-6 + dt[eq] / o["t_final"][eq]), np.max(rr[eq] / (1e-6 + dt[eq] / o["t_final"][eq]))
+    assert np.max(rr[far & ~eq], initial=0.0) <= 1e-4
+    same = eq & (dt <= 1e-6 * o["t_final"])
     assert same.sum() > 0.5 * far.sum()
-    assert np.max(np.abs(g["r_min"][same] / o["r_min"][same] - 1)) <= 1e-6
-    assert np.max(np.abs(g["r_min"][short] / o["r_min"][short] - 1), initial=0.0) <= 1e-3
+    assert np.max(rr[same]) <= 1e-6
+    assert np.max(rr[short], initial=0.0) <= 1e-3
     if short.sum() >= 20:
         ref = _final_state_rel(w, o1, o, short, kw)
         for qt in (0.5, 0.9):
             assert np.quantile(rel[short], qt) <= 2 * np.quantile(ref[short], qt) + 1e-9, (qt, np.quantile(rel[short], qt), np.quantile(ref[short], qt))
+        # ... and the worst one stays within a small factor of the oracle's own worst 1-ulp response (measured: <= 5.1)
+        assert rel[short].max() <= 15 * ref[short].max() + 1e-9, (rel[short].max(), ref[short].max())
         pick = np.flatnonzero(short)[:8]
         e_g, e_o = _dop853_distance(w, y0, g, pick, kw), _dop853_distance(w, y0, o, pick, kw)
         assert np.all(e_g <= 2 * e_o + 1e-9), (e_g, e_o)
@@ -534,6 +555,55 @@ def test_config3_prefix_heavy_light(aig):
     assert g["n_acc"].max() > 20 * np.median(g["n_acc"])   # the imbalance the refill queue is for
 
 
+@pytest.mark.parametrize("cfg,kw,n", [(0, {}, 3072), (3, {}, 6144), (4, {"q_trap": 0.4}, 4096)])
+def test_pre_bounce_pointwise_parity(aig, cfg, kw, n):
+    """Single bounces that reach the short-range well are most of configs[3], and after the bounce
+    only statistics can be compared (_compare_direct).  BEFORE the amplification sets in the two
+    paths are compared point by point: the replay of the CUDA path (aig_trace, bit-identical to aig_integrate)
+    against the oracle's record, accepted step by accepted step, up to the last step end with r > 50 a0 on the
+    way in, for >= 200 such trajectories per config:
+      * the same steps: row counts of the whole run within +-2, step times within 1e-3 relative (the step sizes
+        carry the rounding of the error estimate, DESIGN.md "Parity metric"; measured <= 1.5e-4);
+      * the same states <= 1e-6 in the block metric: every row once the CUDA row is moved to the oracle's time
+        along its own tangent (the shift is a few per cent of a step), and the last row exactly, the earlier of
+        the two continued to the later one's time with the oracle's integrator (measured: <= 3e-8 and <= 3e-9);
+    and the CUDA path CONVERGES: re-run at rtol 1e-12 / atol 1e-18 its final states are >= 100x closer to DOP853
+    (rtol 1e-13) than at the configured tolerances, the bar tests/test_oracle_pins.py sets for the oracle."""
+    w = inputs.config(cfg, **kw)
+    y0 = inputs.generate_y0(w, n=n)
+    g, o = run_gpu(aig, w, y0), run_orc(w, y0)
+    p, po = aig.make_params(**w.params()), orc.make_params(**w.params())
+    short = (o["n_turn"] <= 1) & (g["n_turn"] <= 1) & (o["status"] == 0) & (g["status"] == 0) & \
+            (o["r_min"] <= SHORT_RANGE) & (g["r_min"] <= SHORT_RANGE)
+    idx = np.flatnonzero(short)[:250]
+    assert len(idx) >= 200, len(idx)
+    worst_t = worst_rows = worst_last = 0.0
+    for i in idx:
+        to, yo, st = orc.integrate_trace(po, y0[:, i], w.t_max, w.rtol, w.atol)
+        t, y, nn = aig.aig_trace(p, _dev(y0[:, i].copy()), w.t_max, w.rtol, w.atol, cap=8192)
+        na = int(nn[0].item())
+        assert na == g["n_acc"][i] and abs(na - len(to)) <= 2 and int(nn[1].item()) == st == 0
+        tg, yg = t[:na].cpu().numpy(), y[:, :na].cpu().numpy()
+        ro = np.linalg.norm(yo[:, 6:9] - yo[:, 0:3], axis=1)
+        m = min(int(np.argmax(ro <= SHORT_RANGE)), na)      # rows 0 .. m-1: still outside 50 a0 on the way in
+        assert ro[m] <= SHORT_RANGE and m >= 50, (i, m)
+        worst_t = max(worst_t, np.max(np.abs(tg[:m] / to[:m] - 1)))
+        f = orc.rhs(po, tg[:m], yg[:, :m])
+        worst_rows = max(worst_rows, block_rel(yg[:, :m] + f * (to[:m] - tg[:m])[None, :], yo[:m].T).max())
+        j = m - 1
+        ya, yb = _at_common_time(w, yg[:, j:j + 1].copy(), tg[j:j + 1], yo[j:j + 1].T.copy(), to[j:j + 1])
+        worst_last = max(worst_last, block_rel(ya, yb).max())
+    print(f"cfg {cfg} {kw}: {len(idx)} well-reaching bounces before r = 50 a0: step times {worst_t:.2e}, "
+          f"rows (tangent) {worst_rows:.2e}, last row at a common time {worst_last:.2e}")
+    assert worst_t <= 1e-3 and worst_rows <= 1e-6 and worst_last <= 1e-6, (worst_t, worst_rows, worst_last)
+    pick = idx[:12]
+    e_cfg = _dop853_distance(w, y0, g, pick)
+    wt = w.replace(rtol=1e-12, atol=1e-18)
+    yt = np.ascontiguousarray(y0[:, pick])
+    e_tight = _dop853_distance(wt, yt, run_gpu(aig, wt, yt), np.arange(len(pick)))
+    assert np.all(e_tight < 2e-4) and np.all(e_tight < 1e-2 * e_cfg) and np.all(e_cfg < 0.5), (e_cfg, e_tight)
+
+
 _Y0_CACHE = {}
 
 
@@ -637,8 +707,12 @@ def test_observables_and_outliers(aig):
     # deep bounces amplify rounding but the first bounce is reached before that
     deep = (g["n_acc"] == o["n_acc"]) & (g["n_turn"] >= 1) & (o["n_turn"] >= 1) & (o["r_min"] <= SHORT_RANGE)
     if deep.sum() >= 20:
-        dd = np.linalg.norm(g["x_turn1"] - o["x_turn1"], axis=0)[deep] / np.linalg.norm(o["x_turn1"], axis=0)[deep]
+        scale = np.maximum(np.linalg.norm(o["x_turn1"], axis=0), o["r_min"])
+        dd = (np.linalg.norm(g["x_turn1"] - o["x_turn1"], axis=0) / scale)[deep]
         assert np.median(dd) <= 1e-6, np.median(dd)
+        # the ion barely moves while the atom crosses the well: the recorded point is the ion's position at the step
+        # end after the turn, so even the worst one is bounded by the step-time noise times the ion's speed
+        assert dd.max() <= 1e-4, dd.max()
     allobs = dict(g)
     allobs.update(e)
     want = orc.outliers(allobs)
