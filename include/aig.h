@@ -258,6 +258,22 @@ typedef struct aig_map_spec {
 int aig_map2d(const double *y0, int64_t N, const double *value, const aig_map_spec *spec, uint64_t *count,
               double *sum, void *cuda_stream);
 
+/* The potential front-end of the paper's parameter block (the form V(r) = -C_n/r^n + C_m/r^m at :51):
+ * the user gives two of the four numbers C_n, C_m, D_e (well depth, Hartree), R_e (equilibrium distance, Bohr) and
+ * "the code then analytically calculates" the others from V'(R_e) = 0 and V(R_e) = -D_e.  HOST arithmetic, no
+ * device, no allocation.  mode / meaning of (a, b):
+ *   AIG_POT_CNCM  a = C_n, b = C_m   ("CnCm": both constants known; D_e and R_e follow)
+ *   AIG_POT_CNDE  a = C_n, b = D_e   ("CnDe": C_m and R_e follow)
+ *   AIG_POT_DERE  a = D_e, b = R_e   ("DeRe": C_n and C_m follow)
+ * All four values are written (the two given ones are copied through); an output pointer may be NULL.  The result
+ * goes into aig_params as C4 = C_n, C8 = C_m, n_att = n, n_rep = m.  AIG_ERR_PARAM unless 1 <= n < m <= 32 and a, b
+ * are finite and > 0; AIG_ERR_SIZE for an unknown mode.  The paper's listing (n = 4, m = 8,
+ * C_n = 159.5455, D_e = 1 K) prints C_m = 2.00949488627505397797e+09 and R_e = 70.8448174250339519631. */
+#define AIG_POT_CNCM 0
+#define AIG_POT_CNDE 1
+#define AIG_POT_DERE 2
+int aig_potential(int mode, int n, int m, double a, double b, double *Cn, double *Cm, double *De, double *Re);
+
 /* Measurement aid: run a register-resident FP64 FMA chain kernel on every SM and return the
  * achieved non-tensor FP64 rate in FLOP/s through *flops_per_s (blocking; used by bench.py as
  * the measured ALU roofline denominator). ilp in [1, 16] independent chains per thread. */

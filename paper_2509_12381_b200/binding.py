@@ -19,7 +19,8 @@ _lib = None
 EXPORTS = ["aig_workspace_bytes", "aig_integrate", "aig_histogram", "aig_step_once", "aig_run_host",
            "aig_fp64_peak_probe", "aig_kernel_info", "aig_kernel_launches", "aig_set_schedule", "aig_strerror",
            "aig_version", "aig_observables", "aig_outliers", "aig_outliers_workspace_bytes", "aig_trace",
-           "aig_set_schedule_ex", "aig_get_schedule", "aig_map2d", "aig_outliers_static", "aig_outliers_static_max_n"]
+           "aig_set_schedule_ex", "aig_get_schedule", "aig_map2d", "aig_outliers_static", "aig_outliers_static_max_n",
+           "aig_potential"]
 
 
 class AigError(RuntimeError):
@@ -104,6 +105,20 @@ def make_params(m_ion, m_atom, C4, C8, a, q, omega_rf, t0=0.0, r_exit=0.0, r_tur
         p.q[k] = q[k]
     p.omega_rf, p.t0, p.r_exit, p.r_turn, p.max_steps = omega_rf, t0, r_exit, r_turn, int(max_steps)
     return p
+
+
+POT_CNCM, POT_CNDE, POT_DERE = 0, 1, 2
+
+
+def aig_potential(mode: int, n: int, m: int, a: float, b: float) -> dict:
+    """The paper's potential front-end (include/aig.h: aig_potential): host arithmetic in the library.
+    Returns {"Cn", "Cm", "De", "Re"}."""
+    L = lib()
+    L.aig_potential.restype = C.c_int
+    L.aig_potential.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double] + [C.POINTER(C.c_double)] * 4
+    v = [C.c_double() for _ in range(4)]
+    _check(L.aig_potential(mode, n, m, a, b, *[C.byref(x) for x in v]), "aig_potential")
+    return dict(zip(("Cn", "Cm", "De", "Re"), (x.value for x in v)))
 
 
 def _torch():

@@ -1792,6 +1792,37 @@ const char* aig_strerror(int code)
     }
 }
 
+int aig_potential(int mode, int n, int m, double a, double b, double* Cn, double* Cm, double* De, double* Re)
+{
+    if (mode != AIG_POT_CNCM && mode != AIG_POT_CNDE && mode != AIG_POT_DERE) return AIG_ERR_SIZE;
+    if (n < 1 || m <= n || m > 32) return AIG_ERR_PARAM;
+    if (!std::isfinite(a) || !std::isfinite(b) || !(a > 0.0) || !(b > 0.0)) return AIG_ERR_PARAM;
+    // V'(Re) = 0:  n Cn Re^m = m Cm Re^n;   V(Re) = -De:  De = Cn Re^-n - Cm Re^-m = Cn Re^-n (m - n) / m
+    const double dn = (double)n, dm = (double)m;
+    double cn, cm, de, re;
+    if (mode == AIG_POT_CNCM) {
+        cn = a;
+        cm = b;
+        re = std::pow(dm * cm / (dn * cn), 1.0 / (dm - dn));
+        de = cn * (dm - dn) / (dm * std::pow(re, dn));
+    } else if (mode == AIG_POT_CNDE) {
+        cn = a;
+        de = b;
+        re = std::pow(cn * (dm - dn) / (dm * de), 1.0 / dn);
+        cm = dn * cn * std::pow(re, dm - dn) / dm;
+    } else {
+        de = a;
+        re = b;
+        cn = de * dm * std::pow(re, dn) / (dm - dn);
+        cm = de * dn * std::pow(re, dm) / (dm - dn);
+    }
+    if (Cn) *Cn = cn;
+    if (Cm) *Cm = cm;
+    if (De) *De = de;
+    if (Re) *Re = re;
+    return AIG_OK;
+}
+
 size_t aig_workspace_bytes(int64_t N)
 {
     // counters + work-queue order (8 B per trajectory) + class (1 B) + checkpoint slots for suspended trajectories

@@ -127,3 +127,40 @@ def test_product_does_not_import_oracle():
                 assert not pat.search(text), f
                 seen += 1
     assert seen >= 5
+
+
+def test_potential_front_end_against_the_papers_printed_values(lib):
+    """aig_potential: the "CnDe" mode reproduces the C_m and R_e the paper's listing prints for n = 4,
+    m = 8, C_n = 159.5455, D_e = 1 K (tests/golden/paper_constants.txt), the three modes agree with
+    each other, and the returned numbers are the well they claim to be (V'(R_e) = 0, V(R_e) = -D_e by evaluating V)."""
+    gold = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "paper_constants.txt")):
+        if "=" in line and not line.lstrip().startswith("#"):
+            k, v = line.split("#")[0].split("=")
+            gold[k.strip()] = float(v)
+    De = gold["De_example_K"] * gold["kB_hartree_K"]
+    r = binding.aig_potential(binding.POT_CNDE, 4, 8, gold["C4_example"], De)
+    assert abs(r["Cm"] / gold["Cm_example"] - 1) < 1e-14 and abs(r["Re"] / gold["Re_example"] - 1) < 1e-14
+    assert r["Cn"] == gold["C4_example"] and r["De"] == De
+    for n, m, cn, de in ((4, 8, gold["C4_example"], De), (6, 12, 2.0e4, 3.0e-4), (3, 9, 17.0, 1e-5), (1, 2, 0.5, 0.125)):
+        a = binding.aig_potential(binding.POT_CNDE, n, m, cn, de)
+        b = binding.aig_potential(binding.POT_CNCM, n, m, a["Cn"], a["Cm"])
+        c = binding.aig_potential(binding.POT_DERE, n, m, a["De"], a["Re"])
+        for k in ("Cn", "Cm", "De", "Re"):
+            assert abs(b[k] / a[k] - 1) < 1e-13 and abs(c[k] / a[k] - 1) < 1e-13, (n, m, k)
+        V = lambda x: -a["Cn"] / x ** n + a["Cm"] / x ** m
+        assert abs(V(a["Re"]) / -a["De"] - 1) < 1e-13
+        h = 1e-4 * a["Re"]
+        assert V(a["Re"] - h) > V(a["Re"]) < V(a["Re"] + h)
+        assert abs(V(a["Re"] + h) - V(a["Re"] - h)) < 1e-6 * a["De"]
+    # textbook case: n = 1, m = 2, Cn = 1/2, De = 1/8: V = -1/(2r) + Cm/r^2, Re = 4 Cm, De = 1/(16 Cm) => Cm = 1/2, Re = 2
+    t = binding.aig_potential(binding.POT_CNDE, 1, 2, 0.5, 0.125)
+    assert abs(t["Cm"] - 0.5) < 1e-15 and abs(t["Re"] - 2.0) < 1e-15
+    L = binding.lib()
+    L.aig_potential.restype = C.c_int
+    L.aig_potential.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double] + [C.c_void_p] * 4
+    assert L.aig_potential(1, 4, 8, 1.0, 1.0, None, None, None, None) == 0      # every output is optional
+    assert L.aig_potential(3, 4, 8, 1.0, 1.0, None, None, None, None) == -2
+    for n, m, a, b in ((8, 4, 1.0, 1.0), (4, 4, 1.0, 1.0), (0, 4, 1.0, 1.0), (4, 33, 1.0, 1.0), (4, 8, -1.0, 1.0),
+                       (4, 8, 1.0, 0.0), (4, 8, float("nan"), 1.0), (4, 8, 1.0, float("inf"))):
+        assert L.aig_potential(0, n, m, a, b, None, None, None, None) == -5, (n, m, a, b)
