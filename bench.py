@@ -36,6 +36,8 @@ from paper_2509_12381_b200 import inputs  # noqa: E402  (NumPy only)
 
 # SURVEY.md 8(d) / DESIGN.md "Flop accounting": nominal flops of one attempted DP5(4) step of the
 # 12-component system as the paper states it (6 f-evals x 38 + 240 stage FMAs + error + controller).
+# A LOWER bound on what the kernel executes (ncu counts 996 flops per attempted step, profiles/r02_integrate_full.md):
+# the roofline fraction is algorithmic, so the kernel's extra arithmetic earns nothing.
 FLOPS_PER_ATTEMPT = 900.0
 # 148 SMs x 4 sub-partitions x 16 FP64 FMA lanes x 2 flop x 1.965 GHz (max SM clock)
 FP64_PEAK_NOMINAL = 148 * 4 * 16 * 2 * 1.965e9
@@ -48,6 +50,22 @@ INTEGRATE_DRAM_TRAFFIC_SOURCE = ("constant from the ncu --set full capture summa
 WORKLOAD_NAME = "configs[4] N=4194304 q=0.1 rtol=1e-10 atol=1e-12 seed=4"
 SWEEP_Q = (0.1, 0.2, 0.4)
 SWEEP_RTOL = (1e-8, 1e-10, 1e-12)
+
+
+def _sig(x, digits=5):
+    """Floats to `digits` significant digits, recursively: the driver keeps only the last ~3000 characters of the
+    line, and the blocks at its end (sweep, configs, paper_benchmark) must fit there whole."""
+    if isinstance(x, float):
+        return float(f"{x:.{digits}g}") if np.isfinite(x) else x
+    if isinstance(x, dict):
+        return {k: _sig(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_sig(v, digits) for v in x]
+    if isinstance(x, (np.floating,)):
+        return _sig(float(x), digits)
+    if isinstance(x, (np.integer,)):
+        return int(x)
+    return x
 
 
 def _workload(n, q=0.1, rtol=1e-10):
@@ -243,13 +261,16 @@ def run_ours(args) -> int:
     clocks = sampler.stop() if rank == 0 else None
     launches_timed = aig.kernel_launches() - launches_warm
     ms_total = max_over_ranks(e_begin.elapsed_time(e_end))
-    ms_int = max_over_ranks(float(np.mean([a.elapsed_time(b) for a, b in kev])))
+    ms_each = [a.elapsed_time(b) for a, b in kev]
+    ms_int = max_over_ranks(float(np.mean(ms_each)))
+    ms_stats = {"min": float(np.min(ms_each)), "median": float(np.median(ms_each)), "max": float(np.max(ms_each)),
+                "spread_pct": 100.0 * float(np.max(ms_each) - np.min(ms_each)) / float(np.median(ms_each))}
 
-    def schedule_record():
+    def schedule_record(wsp=None):
         """Stage timeline and hand-over counts of the last aig_integrate call (the %globaltimer stamps and
         counters its kernels leave in the workspace): [start, end] in ms of the bulk pass (per-thread
         integrator), the six-lane pass that streams beside it, and the final six-lane pass."""
-        cnt = ws[:512].view(torch.int64).cpu().numpy()
+        cnt = (ws if wsp is None else wsp)[:512].view(torch.int64).cpu().numpy()
         tl = cnt[32:40].astype(np.float64)
         t_first = min((x for x in tl if x > 0), default=0.0)
         st = {name: [round((tl[2 * i] - t_first) / 1e6, 3), round((tl[2 * i + 1] - t_first) / 1e6, 3)]
@@ -344,11 +365,37 @@ def run_ours(args) -> int:
                "d2h_bytes_per_step": int(sum(v.nbytes for v in host_np.values() if isinstance(v, np.ndarray)) + hist_bytes),
                "steps": ne, "ms_per_step": 1e3 * dt / ne, "host_memory": "pinned",
                "api": "aig_run_host (C ABI, host pointers)"}
+        # where the difference to the device-resident step goes: the two copies timed alone (same pinned buffers, CUDA
+        # events), the kernels alone (the timed region above); the rest is cudaMalloc / cudaFree of the ~2 GB slab,
+        # the launches and the final synchronisation.  aig_run_host runs them one after the other on one stream.
+        def _alone(fn):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b)
+        y0_tmp = torch.empty_like(y0)
+        h2d_ms = min(_alone(lambda: y0_tmp.copy_(y0_host, non_blocking=True)) for _ in range(2))
+        d2h_ms = min(_alone(lambda: [host_out[k].copy_(out[k], non_blocking=True) for k in host_out]) for _ in range(2))
+        del y0_tmp
+        e2e["breakdown_ms"] = {"h2d_alone": h2d_ms, "kernels_alone": ms_total / args.steps, "d2h_alone": d2h_ms,
+                               "rest_malloc_free_launch_sync": e2e["ms_per_step"] - h2d_ms - d2h_ms - ms_total / args.steps}
         del host_out, host_np
 
-    # ---- the other points of configs[4]'s 3x3 sweep, once each, outside the timed region
-    sweep = []
+    # ---- all nine points of configs[4]'s 3x3 sweep, once each, outside the timed region.  Reported as parallel
+    #      arrays (one entry per point, q-major) so that the whole block fits the end of the line.
+    #      tail_floor_ms: no call can end before its longest trajectory has taken its steps one after the other =
+    #      attempted steps of that trajectory x the latency of one six-lane step (measured above on the bench
+    #      workload's longest trajectory, alone on the GPU).  sched_ratio = ms / max(end of the bulk pass, tail floor):
+    #      how far the call is from the larger of its two lower bounds under this schedule.
+    sweep = None
     if not args.no_sweep:
+        cols = ("q", "rtol", "ms", "traj_per_s", "acc_steps_per_s", "frac_fp64_peak", "complex_frac", "complex_frac_r50",
+                "max_steps", "tail_floor_ms", "bulk_end_ms", "streaming_end_ms", "final_end_ms", "sched_ratio",
+                "handed_over", "taken_by_final_pass")
+        sweep = {k: [] for k in cols}
         for q in SWEEP_Q:
             for rtol in SWEEP_RTOL:
                 wl = _workload(N, q, rtol)
@@ -364,16 +411,64 @@ def run_ours(args) -> int:
                 tf = FLOPS_PER_ATTEMPT * (a + r) / world / (ms * 1e-3) / 1e12
                 st, ho = schedule_record()
                 c50 = complex_fraction_r_turn(wl, 50.0)
-                # no call can end before its longest trajectory has taken its steps one after the other:
-                # tail_floor_ms = attempted steps of that trajectory x the latency of one six-lane step
-                # (measured above on the bench workload's longest trajectory, alone on the GPU)
-                sweep.append({"q": q, "rtol": rtol, "atol": wl.atol, "ms_integrate": ms,
-                              "trajectories_per_s": world * N / (ms * 1e-3),
-                              "accepted_steps_per_s": a / (ms * 1e-3),
-                              "alg_tflops_per_gpu": tf, "frac_fp64_peak": tf * 1e12 / FP64_PEAK_NOMINAL,
-                              "complex_fraction": c / (world * N), "complex_fraction_r_turn_50": c50,
-                              "max_attempted_steps": longest, "tail_floor_ms": longest * step_us * 1e-3,
-                              "stages_ms": st, **ho})
+                floor = longest * step_us * 1e-3
+                bulk_end = st.get("bulk", [0.0, 0.0])[1]
+                row = (q, rtol, ms, world * N / (ms * 1e-3), a / (ms * 1e-3), tf * 1e12 / FP64_PEAK_NOMINAL,
+                       c / (world * N), c50, longest, floor, bulk_end, st.get("six_lane_streaming", [0.0, 0.0])[1],
+                       st.get("six_lane_final", [0.0, 0.0])[1], ms / max(bulk_end, floor, 1e-9),
+                       ho["n_handed_over"], ho["taken_by_final_pass"])
+                for k, v in zip(cols, row):
+                    sweep[k].append(v)
+
+    # ---- the other BASELINE.json configs and the paper's own benchmark, outside the timed region (one GPU):
+    #      configs[3] (N = 1,048,576, 174/7 amu, q = 0.3, t_max = 1e12: long-lived complexes, step-count imbalance) is
+    #      the second throughput config (hard part 2): three calls; configs[0..2] once each (256 and
+    #      65,536 trajectories: latency-bound by size); the paper's 2,500-trajectory octant grid.
+    configs_rec, paper_rec = None, None
+    if world == 1 and not args.no_configs:
+        def run_cfg(wl, calls):
+            yc = torch.from_numpy(inputs.generate_y0(wl)).to(dev)
+            oc = aig.alloc_out(wl.N, dev)
+            wc = torch.zeros(aig.workspace_bytes(wl.N), dtype=torch.uint8, device=dev)
+            pc = aig.make_params(**wl.params())
+            aig.aig_integrate(pc, yc, wl.t_max, wl.rtol, wl.atol, out=oc, workspace=wc)      # warm-up
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(calls):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                aig.aig_integrate(pc, yc, wl.t_max, wl.rtol, wl.atol, out=oc, workspace=wc)
+                b.record()
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            ms = float(np.median(ts))
+            na = int(oc["n_acc"].sum(dtype=torch.int64).item())
+            nr = int(oc["n_rej"].sum(dtype=torch.int64).item())
+            longest = int((oc["n_acc"] + oc["n_rej"]).max().item())
+            st, ho = schedule_record(wc)
+            floor = longest * step_us * 1e-3
+            bulk_end = st.get("bulk", [0.0, 0.0])[1]
+            return {"N": wl.N, "calls": calls, "ms": ms, "ms_min": float(np.min(ts)), "ms_max": float(np.max(ts)),
+                    "traj_per_s": wl.N / (ms * 1e-3), "acc_steps_per_s": na / (ms * 1e-3),
+                    "frac_fp64_peak": FLOPS_PER_ATTEMPT * (na + nr) / (ms * 1e-3) / FP64_PEAK_NOMINAL,
+                    "mean_steps": na / wl.N, "max_steps": longest, "tail_floor_ms": floor, "bulk_end_ms": bulk_end,
+                    "sched_ratio": ms / max(bulk_end, floor, 1e-9),
+                    "complex_frac": float(oc["complex_flag"].sum(dtype=torch.int64).item()) / wl.N,
+                    "tmax_frac": float((oc["status"] == 1).sum().item()) / wl.N,
+                    "handed_over": ho["n_handed_over"], "taken_by_final_pass": ho["taken_by_final_pass"]}
+        configs_rec = {"cfg3": run_cfg(inputs.config(3), 3)}
+        for i in (0, 1, 2):
+            rec = run_cfg(inputs.config(i), 1)
+            configs_rec[f"cfg{i}"] = {k: rec[k] for k in ("N", "ms", "traj_per_s", "acc_steps_per_s", "frac_fp64_peak",
+                                                          "max_steps", "tail_floor_ms")}
+            configs_rec[f"cfg{i}"]["note"] = "latency-bound by size"
+        wp = inputs.paper_workload()
+        rec = run_cfg(wp, 1)
+        paper_rec = {"workload": "50 x 50 octant grid, head-on, tmax 1 ms, rtol 1e-10 (PAPER.md:102, :116)", "N": wp.N,
+                     "seconds": rec["ms"] * 1e-3, "acc_steps_per_s": rec["acc_steps_per_s"],
+                     "frac_fp64_peak": rec["frac_fp64_peak"], "mean_steps": rec["mean_steps"],
+                     "max_steps": rec["max_steps"], "tail_floor_s": rec["tail_floor_ms"] * 1e-3,
+                     "complex_frac": rec["complex_frac"]}
 
     # ---- the widening kernels, outside the timed region: aig_observables and
     #      aig_outliers over the bench workload's results, each timed alone with CUDA events, L2 flushed
@@ -390,10 +485,16 @@ def run_ours(args) -> int:
         side = {}
         # algorithmic bytes per trajectory: observables 12 + 3 + 3 doubles in, 4 out; outliers 6 doubles + 2 int32 in
         hist_side = aig.alloc_hist(len(ae) - 1, len(le) - 1, 64, dev)
+        map_ue = torch.linspace(0.0, 1.0 + 1e-12, 65, dtype=torch.float64, device=dev)        # 64 x 128 equal-solid-angle cells
+        map_pe = torch.linspace(0.0, 2.0 * np.pi, 129, dtype=torch.float64, device=dev)
+        map_c = torch.zeros((64, 128), dtype=torch.int64, device=dev)
+        map_t = torch.zeros((64, 128), dtype=torch.float64, device=dev)
         # histogram (hot-path row a10): angle, lifetime, four int32 and the flag = 33 B per trajectory
         for name, fn, bpt in (("histogram_kernel", lambda: aig.aig_histogram(outp, ae_d, le_d, 64, hist=hist_side), 33),
                               ("observables_kernel", lambda: aig.aig_observables(p, y0, outp, extra=extra), 176),
-                              ("outliers_kernel", lambda: aig.aig_outliers(outp, extra), 56)):
+                              ("outliers_kernel", lambda: aig.aig_outliers(outp, extra), 56),
+                              # map2d: the atom's position (3 doubles) and the value in; the cells stay in L2
+                              ("map2d_kernel", lambda: aig.aig_map2d(y0, outp["angle"], map_ue, map_pe, count=map_c, total=map_t), 32)):
             ts = []
             for _ in range(5):
                 flush.zero_()
@@ -456,9 +557,11 @@ def run_ours(args) -> int:
                          "hbm_bytes_algorithmic": 241 * N},
             "kernel": info,
             "e2e": e2e, "gpu_launches": int(launches_timed), "clocks": clocks,
-            "cpu_baseline": cpu, "side_kernels": side, "sweep": sweep,
+            "cpu_baseline": cpu, "side_kernels": side,
+            # the blocks the record must show whole come last (the driver keeps the tail of the line)
+            "ms_integrate_per_step": ms_stats, "paper_benchmark": paper_rec, "configs": configs_rec, "sweep": sweep,
         }
-        print(json.dumps(line), flush=True)
+        print(json.dumps(_sig(line), separators=(",", ":")), flush=True)
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -475,6 +578,7 @@ def main() -> int:
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-side", action="store_true", help="skip timing aig_observables / aig_outliers")
+    ap.add_argument("--no-configs", action="store_true", help="skip configs[0..3] and the paper's own benchmark")
     ap.add_argument("--probe-six-lane", action="store_true",
                     help="run only the latency probe: the workload's longest trajectory alone in the six-lane integrator")
     ap.add_argument("--e2e-steps", type=int, default=3)

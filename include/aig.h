@@ -292,7 +292,7 @@ uint64_t aig_kernel_launches(void);
 
 /* Test / tuning hook: the schedule aig_integrate uses from now on in this process.
  *   tail_iters  iterations a warp of the per-thread integrator keeps stepping after its work
- *               queue ran dry before it hands its trajectories over (default 256)
+ *               queue ran dry before it hands its trajectories over (default 1024)
  *   budget      accepted steps after which a trajectory is offered to the six-lane integrator
  *               (default 2048)
  *   split_sms   SMs the six-lane pass owns while the bulk pass runs beside it (12)

@@ -1434,7 +1434,7 @@ bool aligned(const void* ptr, size_t a) { return (reinterpret_cast<uintptr_t>(pt
 constexpr long long kMinSlots = 1 << 20;
 
 struct SchedConfig {
-    int tail_iters = 256;     // iterations a warp keeps stepping after the queue ran dry
+    int tail_iters = 1024;    // iterations a warp keeps stepping after the queue ran dry (round 3: 256 -> 1024, fewer late hand-overs)
     int budget = 2048;        // accepted steps after which the per-thread integrator offers a trajectory
     int split_sms = 12;       // SMs the streaming six-lane pass takes for itself (one 8-warp block each)
     int split_grid_b = 8;     // final six-lane pass: one-warp blocks per SM (it has the GPU to itself)
