@@ -198,8 +198,11 @@ __device__ __forceinline__ void ckpt_store(const Ckpt& K, long long slot, long l
 }
 
 // trajectory index of a claimed slot, once its writer has published it.  The writer took the slot number
-// while running and publishes within microseconds; a second without it means a broken invariant: trap
-// (a loud failure) rather than hang.
+// while running and publishes within microseconds.  %globaltimer is wall time and keeps running while the
+// context is time-sliced, preempted or replayed by a profiler, so the limit that turns a broken invariant
+// into a loud failure (a trap poisons the context: the whole call is lost) rather than a hang is generous:
+// thirty seconds without the writer is not scheduling noise.
+constexpr unsigned long long kCkptWaitLimitNs = 30000000000ULL;
 __device__ __forceinline__ long long ckpt_wait(const Ckpt& K, long long slot)
 {
     long long idx = *(const volatile long long*)(K.idx + slot);
@@ -207,7 +210,7 @@ __device__ __forceinline__ long long ckpt_wait(const Ckpt& K, long long slot)
         const unsigned long long t0 = global_ns();
         while ((idx = *(const volatile long long*)(K.idx + slot)) < 0) {
             __nanosleep(100);
-            if (global_ns() - t0 > 1000000000ULL) __trap();
+            if (global_ns() - t0 > kCkptWaitLimitNs) __trap();
         }
     }
     __threadfence();
@@ -750,10 +753,11 @@ __device__ __forceinline__ int plan_class(const double* __restrict__ y0, long lo
     return cls * kPlanSub + sub;
 }
 
-// <u^2> over the first min(N, 65536) trajectories (a sample is enough for a scheduling threshold): 64 blocks add
-// their partial sums into counters[kCntMeanU2] (a double, zero from the call's memset); the readers divide by n
+// <u^2> over the first min(N, 65536) trajectories (a sample is enough for a scheduling threshold): 256 blocks of 256
+// threads add their partial sums into counters[kCntMeanU2] (a double, zero from the call's memset); the readers
+// divide by n.  (Blocks of 1024 threads capped the kernel at 64 registers and spilled 84 bytes.)
 constexpr long long kPlanMeanSample = 65536;
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(256)
 plan_mean_kernel(const double* __restrict__ y0, const long long N, unsigned long long* __restrict__ counters)
 {
     __shared__ double part[32];
@@ -1630,7 +1634,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
         A.omega = (float)p->omega_rf;
         A.phase0 = (float)std::fmod(p->omega_rf * p->t0, 6.283185307179586);
         const unsigned pg = (unsigned)((N + 255) / 256);
-        plan_mean_kernel<<<(unsigned)std::min<long long>(64, (N + 1023) / 1024), 1024, 0, st>>>(y0, N, counters);
+        plan_mean_kernel<<<(unsigned)std::min<long long>(256, (N + 255) / 256), 256, 0, st>>>(y0, N, counters);
         plan_kernel<0><<<pg, 256, 0, st>>>(y0, N, A, order, cls_of, counters);
         plan_bounds_kernel<<<1, 1, 0, st>>>(counters, kCntBound, kCntFront);
         plan_kernel<1><<<pg, 256, 0, st>>>(y0, N, A, order, cls_of, counters);
@@ -1662,7 +1666,26 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     T.patience_ns = 2000000ULL;  // 2 ms to see the bulk pass start
     integrate_split_kernel<TRAP, kSplitWarps, 1><<<(unsigned)own, 32 * kSplitWarps, (size_t)smem_optin, side->stream>>>(K, y0, N, O, T);
     g_kernel_launches++;
-    if (cudaEventRecord(side->join, side->stream) != cudaSuccess) return AIG_ERR_CUDA;
+    // From here on the side stream may hold a kernel that polls and writes the caller's workspace and outputs.
+    // Whatever fails below, the caller's stream must not get past this call before that kernel has ended (it gives
+    // up by itself 2 ms after it finds that no bulk pass has started): join the side stream, or, if even that
+    // fails, block the host on it.  Otherwise the caller could free or reuse the buffers under a running kernel
+    // and the next call on this device would find the shared side stream busy.
+    auto leave = [&](int rc) {
+        if (cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) {
+            (void)cudaStreamSynchronize(side->stream);
+            rc = rc ? rc : AIG_ERR_CUDA;
+        }
+        return rc;
+    };
+    if (cudaGetLastError() != cudaSuccess) {  // the streaming launch itself failed: nothing is running on the side stream
+        (void)cudaStreamSynchronize(side->stream);
+        return AIG_ERR_CUDA;
+    }
+    if (cudaEventRecord(side->join, side->stream) != cudaSuccess) {
+        (void)cudaStreamSynchronize(side->stream);
+        return AIG_ERR_CUDA;
+    }
 
     // bulk pass on the caller's stream, behind a short wait for the streaming pass to have taken its SMs
     head_start_kernel<<<1, 1, 0, st>>>(counters + kCntTime + 2 * kStageStream, 200000ULL);
@@ -1689,6 +1712,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     S.timeline = counters + kCntTime + 2 * kStageBulk;
     integrate_kernel<TRAP, kBlock, kBlocksPerSM><<<(unsigned)blocks, kBlock, 0, st>>>(K, y0, N, O, S);
     g_kernel_launches += 2;
+    if (cudaGetLastError() != cudaSuccess) return leave(AIG_ERR_CUDA);  // no bulk pass: the streaming pass gives up; wait for it
 
     // final six-lane pass: the whole GPU on what is left (the bulk pass is complete: nothing to wait for)
     T.timeline = counters + kCntTime + 2 * kStageFinal;
@@ -1697,8 +1721,7 @@ int launch_integrate(const aig_params* p, const KParams& K, const double* y0, lo
     T.capacity = 0;
     integrate_split_kernel<TRAP, 1, kSplitMinBlocks><<<split_last, 32, 0, st>>>(K, y0, N, O, T);
     g_kernel_launches++;
-    if (cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) return AIG_ERR_CUDA;
-    return cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA;
+    return leave(cudaGetLastError() == cudaSuccess ? AIG_OK : AIG_ERR_CUDA);
 }
 
 }  // namespace
