@@ -384,7 +384,8 @@ struct Traj {
 
 // The rarely touched part of a trajectory's state (observables and counters).  The per-thread
 // integrator keeps it in shared memory (ColdShared in aig_kernels.cu: one slot per thread, SoA:
-// it runs at 246 registers, two blocks of 128 threads per SM); ColdRegs is the same thing in registers.
+// that is what lets it run at 168 registers, three blocks of 128 threads per SM, without a spill);
+// ColdRegs is the same thing in registers.
 struct ColdRegs {
     static constexpr bool kInRegisters = true;
     double rmin2_, t_first_, t_last_;

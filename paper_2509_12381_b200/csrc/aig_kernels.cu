@@ -923,7 +923,8 @@ struct HistArgs {
 };
 
 // HBM-bound: 33 B per trajectory (angle, lifetime, four int32, the flag).
-// Grid-stride over N, four trajectories per thread and iteration with all loads issued first; bins
+// Grid-stride over N, kHistUnroll = 2 trajectories per thread and iteration in a two-stage software pipeline
+// (the loads of the next pair are in flight while the current pair is binned); bins
 // privatised in shared memory (edges staged there too).  The 4-valued status and the small n_turn values
 // (0..3: all but a few per mille) are counted in registers and folded once per warp at the end; the
 // angle takes a linear guess of its bin, corrected against the edges (exact for any edges), and a plain

@@ -3,11 +3,13 @@
 // Why: a trajectory that forms a long-lived complex takes 10^2..10^3 times the mean number of steps
 // (BASELINE.json north_star), and steps are sequential, so the run time of an
 // ensemble is bounded below by (steps of the longest trajectory) x (latency of one step).  In the
-// per-thread integrator a step is ~1100 warp instructions, ~600 of them on the half-rate FP64 pipe:
-// a warp cannot finish one in less than ~1.2 us however few of its lanes are alive.  Here the six
+// per-thread integrator a step is ~1200 warp instructions, 680 of them on the FP64 pipe (two cycles
+// each): a warp cannot finish one in less than ~0.7 us however few of its lanes are alive, and takes
+// ~3 us beside the eleven other warps of its SM (measured, profiles/r03_integrate_full.md).  Here the six
 // lanes (k, e), k = x|y|z, e = 0|1 of a group hold component k of both particles and evaluate, at
 // each of the three dependent levels of the Nystrom form, stage 2 lev + 2 + e; the per-lane
-// instruction stream is ~4x shorter and a step costs about its dependent-chain latency (~0.5 us).
+// instruction stream is ~3x shorter (422 instructions on the fast path) and a step costs about its
+// dependent-chain latency: 0.64 us = 1,260 cycles measured (profiles/r02_integrate_full.md).
 // Five groups share a warp (lanes 30, 31 idle).  The FP64 cost per trajectory step is ~2x that of
 // the per-thread integrator (the scalar force factors, the controller and the step end are
 // replicated), so only the few trajectories that outlive the step budget of the per-thread
